@@ -1,0 +1,195 @@
+/*
+ * gtls.h -- C ABI of libgtls: the Transit Least Squares (TLS) period search that GTLS
+ * (arxiv/paper_2607_00348) accelerates, as hand-written CUDA for NVIDIA B200 (sm_100a).
+ *
+ * Citations are to PAPER.md (the paper text) by line, plus the readings G1..G22 listed in
+ * DESIGN.md.  Every step of the search runs in CUDA kernels; there is no CPU fallback: if no
+ * CUDA device is usable the calls return GTLS_ECUDA.
+ *
+ * Conventions
+ *   - Plain C: no exceptions cross the boundary.  Return 0 (GTLS_OK) on success, a negative
+ *     GTLS_E* code on error.  GTLS_EDEGENERATE is a documented partial success (see below).
+ *   - Every pointer is caller-owned.  The library never frees or retains a pointer after the
+ *     call returns.  Outputs are written only on success / GTLS_EDEGENERATE.
+ *   - `opts->pointers_on_device == 0`: all array arguments are HOST pointers; the library
+ *     allocates device memory, copies in, runs, copies out and synchronises.
+ *     `opts->pointers_on_device == 1`: all array arguments (inputs and outputs, but not
+ *     `opts`, `out_summary` or `opts->stats`, which are always host structs) are DEVICE
+ *     pointers on `opts->device`, e.g. `torch.Tensor.data_ptr()`; work is enqueued on
+ *     `opts->stream` (a cudaStream_t; NULL = the legacy default stream).  The call
+ *     synchronises the stream before returning (it reads back a few validation flags and the
+ *     summary), so results are complete on return.
+ *   - Units: `t` and `period_grid` share one time unit (days in all shipped workloads);
+ *     `duration_grid` holds dimensionless fractions q = T14 / P.
+ *   - `t` need not be sorted.  The library does not normalise or detrend: `y`
+ *     must already be normalised to mean ~1.
+ *   - Thread safety: concurrent calls are safe when they use distinct streams and distinct
+ *     workspaces (or let the library allocate its own).
+ */
+#ifndef GTLS_H_
+#define GTLS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GTLS_OK            0
+#define GTLS_EINVAL       (-1)  /* NULL required pointer, n < 3, n_per < 1, n_dur < 1, n_tmpl < 2,
+                                   even / negative sde_kernel, dt0 < 0, unknown option value     */
+#define GTLS_ENONFINITE   (-2)  /* NaN / Inf in t, y, dy, or dy <= 0                            */
+#define GTLS_EGRID        (-3)  /* period <= 0 or non-finite; duration fraction not in (0, 0.5]   */
+#define GTLS_ENOMEM       (-4)  /* device allocation failed / caller workspace too small         */
+#define GTLS_ECUDA        (-5)  /* CUDA error; text via gtls_last_cuda_error()                   */
+#define GTLS_EDEGENERATE  (-6)  /* chi2_min == 0 or sigma_SR == 0: chi2 / best outputs are valid,
+                                   SDE outputs are set to 0                                      */
+#define GTLS_EUNSUPPORTED (-7)  /* option combination not implemented (see field comments)      */
+
+/* Best trial of one period.  `start` is the index, in the phase-sorted
+ * folded curve, of the first in-transit point; the window is sorted positions
+ * (start + j) mod n, j < D, with D = clamp(floor(q * n), 1, n-1) (reading G11).
+ * `depth` is the scaled template depth a = max(rbar, 0) / mean(g_D) (Eq. 12-13).
+ * `t0` is the observed time of the window's middle point, t[sigma[(start + (D-1)/2) mod n]]
+ * (trial mid-transit times coincide with observed points). */
+typedef struct {
+    int32_t dur_idx;
+    int32_t start;
+    double  depth;
+    double  t0;
+} gtls_best;
+
+/* Optional per-stage timing / counters, filled when opts->stats != NULL (host struct).
+ * Times are CUDA-event milliseconds summed over all period tiles of the call. */
+typedef struct {
+    double  ms_total;        /* first kernel to last kernel of the call                           */
+    double  ms_pre;          /* a0: per-curve arrays, validation, duration table                  */
+    double  ms_fold;         /* a1: fold + sortable keys                                          */
+    double  ms_sort;         /* a2: radix sort passes + tie fix-up                                */
+    double  ms_scan;         /* a3+a4: gather, wrap pad, prefix sums                              */
+    double  ms_chi2;         /* a5-a7: depth, out-of-transit, in-transit chi2 per window          */
+    double  ms_reduce;       /* a8: per-period lexicographic argmin                               */
+    double  ms_epilogue;     /* a9: SR, SDE_raw, median detrend, argmax                           */
+    int64_t kernel_launches; /* kernels launched by this call                                     */
+    int64_t chi2_launches;   /* launches of the in-transit chi2 kernel                            */
+    int64_t windows;         /* (period, duration, start) windows evaluated                       */
+    int64_t window_points;   /* sum over evaluated windows of D (in-transit point visits)         */
+    int64_t period_points;   /* n * n_per                                                         */
+    int32_t period_tile;     /* periods in flight per tile                                        */
+    int32_t path;            /* 1 = fused shared-memory path, 2 = general tiled path              */
+    int32_t uniform_dy;      /* 1 when all dy are equal (G is position independent)               */
+    int32_t reserved;
+} gtls_stats;
+
+typedef struct {
+    uint32_t struct_size;        /* sizeof(gtls_opts), for ABI versioning                         */
+    double   dt0;                /* Eq. 18: stride = max(1, floor(D*dt0)); 0 => 1   */
+    int32_t  top_k;              /* 0 => every strided start (paper). K>0 (K deepest windows per
+                                    (period, duration), reading G19) => GTLS_EUNSUPPORTED for now  */
+    int32_t  dur_per_period;     /* 0: duration_grid[n_dur] shared by all periods;
+                                    1: duration_grid[n_per][n_dur] (row per period, reading G12)   */
+    int32_t  sde_kernel;         /* odd window of the moving-median detrend (PAPER.md:279,
+                                    reading G17); 0 or 1 => SDE = SDE_raw                          */
+    int32_t  chi2_fp32;          /* 0 = fp64.  1 (fp32 in-transit variant) => GTLS_EUNSUPPORTED     */
+    int32_t  pointers_on_device; /* see Conventions                                               */
+    int32_t  device;             /* CUDA device ordinal                                           */
+    void*    stream;             /* cudaStream_t                                                  */
+    void*    workspace;          /* optional caller-owned DEVICE scratch (256-byte aligned)        */
+    size_t   workspace_bytes;    /* its size; must be >= gtls_workspace_bytes(...)                 */
+    int32_t  period_tile;        /* periods processed per tile; 0 = automatic                     */
+    int32_t  path;               /* 0 = automatic, 1 = force fused path, 2 = force general path    */
+    gtls_stats* stats;           /* optional, host                                                */
+} gtls_opts;
+
+typedef struct {
+    int64_t best_period_idx;     /* argmin_P chi2(P), ties -> lowest index (= argmax SDE_raw)      */
+    int32_t best_dur_idx;
+    int32_t best_start;
+    double  best_period, best_t0, best_depth;
+    double  chi2_min;            /* min_P chi2(P)                                                 */
+    double  chi2_null;           /* chi2_0 = sum_i ((1 - y_i)/dy_i)^2, the no-transit model        */
+    double  sde_raw_max;         /* SDE_raw at best_period_idx                                    */
+    double  sde_max;             /* max_P SDE(P)                                                  */
+    int64_t sde_argmax;          /* argmax_P SDE(P), ties -> lowest index                         */
+    int64_t windows_evaluated;
+} gtls_summary;
+
+/* Fill `o` with the defaults used when opts == NULL: dt0 = 0.05 (the paper's worked example,
+ * PAPER.md:291), top_k 0, dur_per_period 0, sde_kernel 151, fp64, host pointers, device 0,
+ * default stream, no workspace, automatic tile and path. */
+void gtls_opts_default(gtls_opts* o);
+
+/* The search: for every trial period fold (Eq. 10), sort by phase (PAPER.md:185,
+ * ties by original index), wrap-pad (Fig. 3), prefix sums (Eq. 14),
+ * and for every duration and strided start (Eq. 18) the mean-matched depth (Eq. 12-13) and
+ *   chi2 = chi2_out (Eq. 15 minus the Eq. 11 edge term) + chi2_in (Eq. 16);
+ * then chi2(P) = min over (duration, start) with lexicographic tie-break (chi2, dur_idx, start),
+ * SR(P) = chi2_min / chi2(P), SDE_raw (Eq. 17; population sigma) and the
+ * moving-median detrended SDE.
+ *
+ *   t, y, dy        [n]        light curve: times, normalised flux, 1-sigma uncertainties (> 0)
+ *   period_grid     [n_per]    trial periods (> 0), any order; SDE median runs in this order
+ *   duration_grid   [n_dur] or [n_per][n_dur] fractions T14/P in (0, 0.5]
+ *   tmpl            [n_tmpl]   transit template as a flux DEFICIT on nodes u_k = k/(n_tmpl-1)
+ *                              across first..fourth contact (reading G13); resampled to D points
+ *                              by linear interpolation at cell centres (j+1/2)/D (reading G14)
+ *   out_chi2        [n_per]    required
+ *   out_best        [n_per]    may be NULL
+ *   out_sde_raw, out_sde [n_per] may be NULL
+ *   out_summary     host struct, may be NULL
+ */
+int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
+                const double* period_grid, int64_t n_per,
+                const double* duration_grid, int32_t n_dur,
+                const double* tmpl, int32_t n_tmpl,
+                const gtls_opts* opts,
+                double* out_chi2, gtls_best* out_best,
+                double* out_sde_raw, double* out_sde,
+                gtls_summary* out_summary);
+
+/* Parity / debug export of steps a1-a2: phases (Eq. 10) and the stable phase-sort permutation
+ * for each period.  out_phase [n_per*n] may be NULL; out_perm [n_per*n] (int32) is required.
+ * out_phase[ip*n + i] is the phase of input point i; out_perm[ip*n + s] is the input index at
+ * sorted position s. */
+int gtls_fold_sort(const double* t, int64_t n, const double* periods, int64_t n_per,
+                   const gtls_opts* opts, double* out_phase, int32_t* out_perm);
+
+/* Parity / debug export of steps a3-a4 for ONE period: the gathered, wrap-padded prefix sums
+ * (Eq. 14) of x1 = w r, x0 = w, x2 = w r^2 with w = 1/dy^2, r = 1 - y, in phase order.
+ * Each output holds n + pad + 1 doubles, out[0] = 0, out[s+1] = sum of the first s+1 padded
+ * entries (entries n..n+pad-1 repeat entries 0..pad-1, Fig. 3).  Any output may be NULL. */
+int gtls_fold_scan(const double* t, const double* y, const double* dy, int64_t n, double period,
+                   int64_t pad, const gtls_opts* opts, double* out_s1, double* out_s0,
+                   double* out_s2);
+
+/* Parity / debug export of steps a5-a7 for ONE (period, duration fraction q): for every strided
+ * start k*stride < n writes the start index, the depth a, chi2_out = chi2_0 - (S2[s+D]-S2[s])
+ * (Eq. 15 with the Eq. 11 edge term, reading G4) and chi2_in (Eq. 16).  Arrays must hold
+ * ceil(n/stride) entries (n is always enough).  Returns the number of starts (>= 1) or a
+ * negative error code. */
+int64_t gtls_window_chi2(const double* t, const double* y, const double* dy, int64_t n,
+                         double period, double q, const double* tmpl, int32_t n_tmpl,
+                         const gtls_opts* opts, int32_t* out_start, double* out_depth,
+                         double* out_chi2_out, double* out_chi2_in);
+
+/* Step a9 alone: SR, SDE_raw, SDE and the summary indices from a chi2(P) array (used after a
+ * period-sharded multi-GPU search has gathered chi2).  out_sde_raw / out_sde may be NULL.
+ * Only the chi2 / SDE fields of out_summary are filled. */
+int gtls_sde(const double* chi2, int64_t n_per, const gtls_opts* opts,
+             double* out_sde_raw, double* out_sde, gtls_summary* out_summary);
+
+/* Device scratch needed by gtls_search for these sizes and options (tile = opts->period_tile
+ * or the automatic choice).  Pass a buffer of at least this size in opts->workspace to avoid
+ * allocation inside the call. */
+size_t gtls_workspace_bytes(int64_t n, int64_t n_per, int32_t n_dur, const gtls_opts* opts);
+
+const char* gtls_strerror(int code);
+const char* gtls_version(void);
+/* Text of the last CUDA error seen by the calling thread ("" if none). */
+const char* gtls_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GTLS_H_ */

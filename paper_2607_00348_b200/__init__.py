@@ -1,0 +1,316 @@
+"""paper_2607_00348_b200 -- B200-native Transit Least Squares period search (GTLS hot path).
+
+Thin Python binding over ``libgtls.so`` (C ABI in ``include/gtls.h``): argument marshalling
+only -- every step of the search runs in the library's CUDA kernels.  The functions keep the
+names of the C entry points.  Arrays may be
+
+* ``torch`` CUDA tensors (float64): passed as device pointers; outputs are CUDA tensors and the
+  work is enqueued on torch's current stream (or ``stream=``);
+* ``numpy`` arrays: passed as host pointers; the library copies to / from the device itself.
+
+PyTorch is used for device memory and streams only.  There is no CPU fallback: if the library
+cannot be loaded, or no CUDA device is usable, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass, field
+from typing import Any, Optional
+
+import numpy as np
+
+__all__ = ["gtls_search", "gtls_fold_sort", "gtls_fold_scan", "gtls_window_chi2", "gtls_sde",
+           "gtls_workspace_bytes", "gtls_strerror", "gtls_version", "GtlsError", "SearchResult",
+           "BEST_DTYPE", "lib_path", "load_library"]
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_PKG, "libgtls.so")
+
+GTLS_OK = 0
+GTLS_EDEGENERATE = -6
+
+BEST_DTYPE = np.dtype([("dur_idx", np.int32), ("start", np.int32), ("depth", np.float64),
+                       ("t0", np.float64)], align=True)
+
+
+class GtlsStats(C.Structure):
+    _fields_ = [("ms_total", C.c_double), ("ms_pre", C.c_double), ("ms_fold", C.c_double),
+                ("ms_sort", C.c_double), ("ms_scan", C.c_double), ("ms_chi2", C.c_double),
+                ("ms_reduce", C.c_double), ("ms_epilogue", C.c_double),
+                ("kernel_launches", C.c_int64), ("chi2_launches", C.c_int64),
+                ("windows", C.c_int64), ("window_points", C.c_int64), ("period_points", C.c_int64),
+                ("period_tile", C.c_int32), ("path", C.c_int32), ("uniform_dy", C.c_int32),
+                ("reserved", C.c_int32)]
+
+    def as_dict(self) -> dict:
+        return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved"}
+
+
+class GtlsOpts(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("dt0", C.c_double), ("top_k", C.c_int32),
+                ("dur_per_period", C.c_int32), ("sde_kernel", C.c_int32), ("chi2_fp32", C.c_int32),
+                ("pointers_on_device", C.c_int32), ("device", C.c_int32), ("stream", C.c_void_p),
+                ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
+                ("period_tile", C.c_int32), ("path", C.c_int32), ("stats", C.POINTER(GtlsStats))]
+
+
+class GtlsSummary(C.Structure):
+    _fields_ = [("best_period_idx", C.c_int64), ("best_dur_idx", C.c_int32), ("best_start", C.c_int32),
+                ("best_period", C.c_double), ("best_t0", C.c_double), ("best_depth", C.c_double),
+                ("chi2_min", C.c_double), ("chi2_null", C.c_double), ("sde_raw_max", C.c_double),
+                ("sde_max", C.c_double), ("sde_argmax", C.c_int64), ("windows_evaluated", C.c_int64)]
+
+    def as_dict(self) -> dict:
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class GtlsError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        lib = load_library()
+        msg = lib.gtls_strerror(code).decode()
+        cuda = lib.gtls_last_cuda_error().decode()
+        super().__init__(f"{where}: {msg} [{code}]" + (f" -- {cuda}" if cuda else ""))
+        self.code = code
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def load_library():
+    """Load libgtls.so (built in-tree by ``python -m paper_2607_00348_b200.build``).  Raises if it
+    is missing: there is deliberately no fallback implementation."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(f"{_LIB_PATH} not found: build it with "
+                          "`python -m paper_2607_00348_b200.build` (nvcc, sm_100a); "
+                          "there is no CPU fallback")
+    lib = C.CDLL(_LIB_PATH)
+    vp, dp, ip = C.c_void_p, C.c_void_p, C.c_void_p
+    lib.gtls_opts_default.argtypes = [C.POINTER(GtlsOpts)]
+    lib.gtls_opts_default.restype = None
+    lib.gtls_search.argtypes = [dp, dp, dp, C.c_int64, dp, C.c_int64, dp, C.c_int32, dp, C.c_int32,
+                                C.POINTER(GtlsOpts), dp, vp, dp, dp, C.POINTER(GtlsSummary)]
+    lib.gtls_search.restype = C.c_int
+    lib.gtls_fold_sort.argtypes = [dp, C.c_int64, dp, C.c_int64, C.POINTER(GtlsOpts), dp, ip]
+    lib.gtls_fold_sort.restype = C.c_int
+    lib.gtls_fold_scan.argtypes = [dp, dp, dp, C.c_int64, C.c_double, C.c_int64, C.POINTER(GtlsOpts),
+                                   dp, dp, dp]
+    lib.gtls_fold_scan.restype = C.c_int
+    lib.gtls_window_chi2.argtypes = [dp, dp, dp, C.c_int64, C.c_double, C.c_double, dp, C.c_int32,
+                                     C.POINTER(GtlsOpts), ip, dp, dp, dp]
+    lib.gtls_window_chi2.restype = C.c_int64
+    lib.gtls_sde.argtypes = [dp, C.c_int64, C.POINTER(GtlsOpts), dp, dp, C.POINTER(GtlsSummary)]
+    lib.gtls_sde.restype = C.c_int
+    lib.gtls_workspace_bytes.argtypes = [C.c_int64, C.c_int64, C.c_int32, C.POINTER(GtlsOpts)]
+    lib.gtls_workspace_bytes.restype = C.c_size_t
+    lib.gtls_strerror.argtypes = [C.c_int]
+    lib.gtls_strerror.restype = C.c_char_p
+    lib.gtls_version.restype = C.c_char_p
+    lib.gtls_last_cuda_error.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+# ---------------------------------------------------------------------------------------------
+# marshalling helpers
+# ---------------------------------------------------------------------------------------------
+def _is_torch(x) -> bool:
+    return type(x).__module__.startswith("torch")
+
+
+def _prep(x, dtype=np.float64):
+    """Return (object kept alive, pointer int, is_device)."""
+    if _is_torch(x):
+        import torch
+        want = {np.float64: torch.float64, np.int32: torch.int32}[dtype]
+        if not x.is_cuda:
+            raise ValueError("torch inputs must be CUDA tensors (use numpy arrays for host data)")
+        x = x.contiguous()
+        if x.dtype != want:
+            x = x.to(want)
+        return x, x.data_ptr(), True
+    a = np.ascontiguousarray(x, dtype=dtype)
+    return a, a.ctypes.data, False
+
+
+def _opts(device_mode: bool, like=None, stream=None, **kw) -> GtlsOpts:
+    o = GtlsOpts()
+    load_library().gtls_opts_default(C.byref(o))
+    o.pointers_on_device = 1 if device_mode else 0
+    if device_mode:
+        import torch
+        o.device = like.device.index if like.device.index is not None else torch.cuda.current_device()
+        s = stream if stream is not None else torch.cuda.current_stream(like.device)
+        o.stream = int(getattr(s, "cuda_stream", s))
+    for k, v in kw.items():
+        setattr(o, k, v)
+    return o
+
+
+def _empty(shape, like, dtype=np.float64):
+    if _is_torch(like):
+        import torch
+        td = {np.float64: torch.float64, np.int32: torch.int32, np.uint8: torch.uint8}[dtype]
+        return torch.empty(shape, dtype=td, device=like.device)
+    return np.empty(shape, dtype=dtype)
+
+
+def _ptr(x) -> int:
+    return x.data_ptr() if _is_torch(x) else x.ctypes.data
+
+
+# ---------------------------------------------------------------------------------------------
+# entry points (same names as include/gtls.h)
+# ---------------------------------------------------------------------------------------------
+@dataclass
+class SearchResult:
+    chi2: Any                      # [n_per]
+    sde_raw: Any                   # [n_per]
+    sde: Any                       # [n_per]
+    best_raw: Any                  # [n_per, 24] bytes: gtls_best records
+    summary: dict
+    code: int                      # GTLS_OK or GTLS_EDEGENERATE
+    stats: Optional[dict] = None
+    _keep: list = field(default_factory=list, repr=False)
+
+    def best(self) -> np.ndarray:
+        """gtls_best records as a numpy structured array (copies from the device)."""
+        raw = self.best_raw.cpu().numpy() if _is_torch(self.best_raw) else self.best_raw
+        return np.ascontiguousarray(raw).view(BEST_DTYPE).reshape(-1)
+
+
+def gtls_version() -> str:
+    return load_library().gtls_version().decode()
+
+
+def gtls_strerror(code: int) -> str:
+    return load_library().gtls_strerror(int(code)).decode()
+
+
+def gtls_workspace_bytes(n: int, n_per: int, n_dur: int, period_tile: int = 0) -> int:
+    o = GtlsOpts()
+    lib = load_library()
+    lib.gtls_opts_default(C.byref(o))
+    o.period_tile = int(period_tile)
+    return int(lib.gtls_workspace_bytes(int(n), int(n_per), int(n_dur), C.byref(o)))
+
+
+def gtls_search(t, y, dy, period_grid, duration_grid, tmpl, *, dt0: float = 0.05,
+                sde_kernel: int = 151, top_k: int = 0, chi2_fp32: int = 0, period_tile: int = 0,
+                path: int = 0, workspace=None, stats: bool = False, stream=None) -> SearchResult:
+    """TLS period search (``gtls_search`` in include/gtls.h).  ``duration_grid`` is [n_dur]
+    (shared) or [n_per, n_dur] (one row per period)."""
+    lib = load_library()
+    kt, pt, dev = _prep(t)
+    ky, py, d2 = _prep(y)
+    kd, pd, d3 = _prep(dy)
+    kp, pp, d4 = _prep(period_grid)
+    kq, pq, d5 = _prep(duration_grid)
+    km, pm, d6 = _prep(tmpl)
+    if len({dev, d2, d3, d4, d5, d6}) != 1:
+        raise ValueError("all arrays must be either CUDA tensors or host arrays")
+    n, n_per, n_tmpl = int(kt.shape[0]), int(kp.shape[0]), int(km.shape[0])
+    per_period = 1 if kq.ndim == 2 else 0
+    n_dur = int(kq.shape[-1])
+    if per_period and int(kq.shape[0]) != n_per:
+        raise ValueError("duration_grid rows must match period_grid")
+    st = GtlsStats()
+    o = _opts(dev, kt, stream, dt0=float(dt0), sde_kernel=int(sde_kernel), top_k=int(top_k),
+              chi2_fp32=int(chi2_fp32), dur_per_period=per_period, period_tile=int(period_tile),
+              path=int(path))
+    if stats:
+        o.stats = C.pointer(st)
+    if workspace is not None:
+        if not (_is_torch(workspace) and workspace.is_cuda):
+            raise ValueError("workspace must be a CUDA uint8 tensor")
+        o.workspace = workspace.data_ptr()
+        o.workspace_bytes = workspace.numel() * workspace.element_size()
+    chi2 = _empty((n_per,), kt)
+    sde_raw = _empty((n_per,), kt)
+    sde = _empty((n_per,), kt)
+    best = _empty((n_per, BEST_DTYPE.itemsize), kt, np.uint8)
+    summ = GtlsSummary()
+    rc = lib.gtls_search(pt, py, pd, n, pp, n_per, pq, n_dur, pm, n_tmpl, C.byref(o), _ptr(chi2),
+                         _ptr(best), _ptr(sde_raw), _ptr(sde), C.byref(summ))
+    if rc not in (GTLS_OK, GTLS_EDEGENERATE):
+        raise GtlsError(rc, "gtls_search")
+    return SearchResult(chi2, sde_raw, sde, best, summ.as_dict(), rc,
+                        st.as_dict() if stats else None, [kt, ky, kd, kp, kq, km])
+
+
+def gtls_fold_sort(t, periods, *, want_phase: bool = True, period_tile: int = 0, stream=None):
+    """Phases (Eq. 10) and stable phase-sort permutations for each period: (phase, perm)."""
+    lib = load_library()
+    kt, pt, dev = _prep(t)
+    kp, pp, d2 = _prep(periods)
+    if dev != d2:
+        raise ValueError("all arrays must be either CUDA tensors or host arrays")
+    n, n_per = int(kt.shape[0]), int(kp.shape[0])
+    o = _opts(dev, kt, stream, period_tile=int(period_tile))
+    phase = _empty((n_per, n), kt) if want_phase else None
+    perm = _empty((n_per, n), kt, np.int32)
+    rc = lib.gtls_fold_sort(pt, n, pp, n_per, C.byref(o), _ptr(phase) if want_phase else None, _ptr(perm))
+    if rc != GTLS_OK:
+        raise GtlsError(rc, "gtls_fold_sort")
+    return phase, perm
+
+
+def gtls_fold_scan(t, y, dy, period: float, pad: int, *, stream=None):
+    """Wrap-padded prefix sums (S1 of w r, S0 of w, S2 of w r^2) for one period, each of
+    length n + pad + 1."""
+    lib = load_library()
+    kt, pt, dev = _prep(t)
+    ky, py, d2 = _prep(y)
+    kd, pd, d3 = _prep(dy)
+    if len({dev, d2, d3}) != 1:
+        raise ValueError("all arrays must be either CUDA tensors or host arrays")
+    n = int(kt.shape[0])
+    o = _opts(dev, kt, stream)
+    outs = [_empty((n + int(pad) + 1,), kt) for _ in range(3)]
+    rc = lib.gtls_fold_scan(pt, py, pd, n, float(period), int(pad), C.byref(o), *[_ptr(x) for x in outs])
+    if rc != GTLS_OK:
+        raise GtlsError(rc, "gtls_fold_scan")
+    return tuple(outs)
+
+
+def gtls_window_chi2(t, y, dy, period: float, q: float, tmpl, *, dt0: float = 0.0, stream=None):
+    """Per-window terms for one (period, duration fraction): (start, depth, chi2_out, chi2_in)."""
+    lib = load_library()
+    kt, pt, dev = _prep(t)
+    ky, py, d2 = _prep(y)
+    kd, pd, d3 = _prep(dy)
+    km, pm, d4 = _prep(tmpl)
+    if len({dev, d2, d3, d4}) != 1:
+        raise ValueError("all arrays must be either CUDA tensors or host arrays")
+    n = int(kt.shape[0])
+    o = _opts(dev, kt, stream, dt0=float(dt0))
+    start = _empty((n,), kt, np.int32)
+    depth, c_out, c_in = (_empty((n,), kt) for _ in range(3))
+    k = lib.gtls_window_chi2(pt, py, pd, n, float(period), float(q), pm, int(km.shape[0]), C.byref(o),
+                             _ptr(start), _ptr(depth), _ptr(c_out), _ptr(c_in))
+    if k < 0:
+        raise GtlsError(int(k), "gtls_window_chi2")
+    k = int(k)
+    return start[:k], depth[:k], c_out[:k], c_in[:k]
+
+
+def gtls_sde(chi2, *, sde_kernel: int = 151, stream=None):
+    """SR/SDE epilogue alone: returns (sde_raw, sde, summary dict, code)."""
+    lib = load_library()
+    kc, pc, dev = _prep(chi2)
+    n_per = int(kc.shape[0])
+    o = _opts(dev, kc, stream, sde_kernel=int(sde_kernel))
+    raw = _empty((n_per,), kc)
+    sde = _empty((n_per,), kc)
+    summ = GtlsSummary()
+    rc = lib.gtls_sde(pc, n_per, C.byref(o), _ptr(raw), _ptr(sde), C.byref(summ))
+    if rc not in (GTLS_OK, GTLS_EDEGENERATE):
+        raise GtlsError(rc, "gtls_sde")
+    return raw, sde, summ.as_dict(), rc

@@ -1,0 +1,170 @@
+// Step a9: chi2_min over the grid, SR(P) = chi2_min / chi2(P) (reading G15), its mean and
+// population standard deviation (G16), SDE_raw (Eq. 17), the moving-median
+// detrend with edge replication (G17/G18) and the argmax.
+#include "gtls_internal.cuh"
+
+namespace gtls {
+
+namespace {
+
+constexpr int kRedThreads = 1024;
+
+__device__ __forceinline__ double block_sum(double v, double* s_buf) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __syncthreads();
+    if (lane == 0) s_buf[warp] = v;
+    __syncthreads();
+    v = lane < (int)(blockDim.x >> 5) ? s_buf[lane] : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;   // every thread of warp 0 holds the total; broadcast below
+}
+
+// One CTA: argmin (lowest index on ties), mean and population sigma of SR.  Fixed reduction
+// shape => deterministic.
+__global__ void __launch_bounds__(kRedThreads) k_sde_stats(const double* __restrict__ chi2,
+                                                           long long n, SdeScratch* sc) {
+    __shared__ double s_buf[32];
+    __shared__ double s_val[32];
+    __shared__ long long s_idx[32];
+    __shared__ double s_bcast[2];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double mv = __longlong_as_double(0x7ff0000000000000LL);   // +inf
+    long long mi = 0x7fffffffffffffffLL;
+    for (long long i = threadIdx.x; i < n; i += blockDim.x) {
+        const double c = chi2[i];
+        if (c < mv || (c == mv && i < mi)) { mv = c; mi = i; }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const double ov = __shfl_xor_sync(0xffffffffu, mv, o);
+        const long long oi = __shfl_xor_sync(0xffffffffu, mi, o);
+        if (ov < mv || (ov == mv && oi < mi)) { mv = ov; mi = oi; }
+    }
+    if (lane == 0) { s_val[warp] = mv; s_idx[warp] = mi; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int k = 1; k < (int)(blockDim.x >> 5); ++k)
+            if (s_val[k] < mv || (s_val[k] == mv && s_idx[k] < mi)) { mv = s_val[k]; mi = s_idx[k]; }
+        s_bcast[0] = mv;
+        sc->chi2_min = mv; sc->argmin = mi;
+    }
+    __syncthreads();
+    const double cmin = s_bcast[0];
+    if (!(cmin > 0.0)) {
+        if (threadIdx.x == 0) { sc->degenerate = 1; sc->mean_sr = 0.0; sc->sd_sr = 0.0; }
+        return;
+    }
+    double acc = 0.0;
+    for (long long i = threadIdx.x; i < n; i += blockDim.x) acc += __ddiv_rn(cmin, chi2[i]);
+    acc = block_sum(acc, s_buf);
+    if (threadIdx.x == 0) s_bcast[1] = __ddiv_rn(acc, (double)n);
+    __syncthreads();
+    const double mean = s_bcast[1];
+    acc = 0.0;
+    for (long long i = threadIdx.x; i < n; i += blockDim.x) {
+        const double d = __ddiv_rn(cmin, chi2[i]) - mean;
+        acc = fma(d, d, acc);
+    }
+    acc = block_sum(acc, s_buf);
+    if (threadIdx.x == 0) {
+        const double var = __ddiv_rn(acc, (double)n);
+        sc->mean_sr = mean;
+        sc->sd_sr = var > 0.0 ? sqrt(var) : 0.0;
+        sc->degenerate = var > 0.0 ? 0 : 1;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_sde_raw(const double* __restrict__ chi2, long long n,
+                                                 const SdeScratch* __restrict__ sc,
+                                                 double* __restrict__ sde_raw) {
+    const bool deg = sc->degenerate != 0;
+    const double cmin = sc->chi2_min, mean = sc->mean_sr, sd = sc->sd_sr;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x)
+        sde_raw[i] = deg ? 0.0 : __ddiv_rn(__ddiv_rn(cmin, chi2[i]) - mean, sd);
+}
+
+// order-preserving map double -> u64
+__device__ __forceinline__ u64 ord(double x) {
+    const u64 b = (u64)__double_as_longlong(x);
+    return (b & 0x8000000000000000ull) ? ~b : (b | 0x8000000000000000ull);
+}
+__device__ __forceinline__ double unord(u64 k) {
+    const u64 b = (k & 0x8000000000000000ull) ? (k & 0x7fffffffffffffffull) : ~k;
+    return __longlong_as_double((long long)b);
+}
+
+// Median of the K-window around i (indices clamped = edge replication) by MSB-first radix
+// select on the ordered bit pattern: 64 counting passes over the window, no local arrays.
+__global__ void __launch_bounds__(128) k_sde_median(const double* __restrict__ sde_raw, long long n,
+                                                    int kernel, const SdeScratch* __restrict__ sc,
+                                                    double* __restrict__ sde) {
+    const int h = (kernel - 1) / 2;
+    const bool deg = sc->degenerate != 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x) {
+        if (deg) { sde[i] = 0.0; continue; }
+        if (kernel <= 1) { sde[i] = sde_raw[i]; continue; }
+        u64 prefix = 0;
+        for (int bit = 63; bit >= 0; --bit) {
+            const u64 cand = prefix | (1ull << bit);
+            int below = 0;
+            for (int k = -h; k <= h; ++k) {
+                long long j = i + k;
+                j = j < 0 ? 0 : (j > n - 1 ? n - 1 : j);
+                below += ord(sde_raw[j]) < cand ? 1 : 0;
+            }
+            if (below <= h) prefix = cand;      // the h-th order statistic is >= cand
+        }
+        sde[i] = sde_raw[i] - unord(prefix);
+    }
+}
+
+__global__ void __launch_bounds__(kRedThreads) k_sde_argmax(const double* __restrict__ sde,
+                                                            const double* __restrict__ sde_raw,
+                                                            long long n, SdeScratch* sc) {
+    __shared__ double s_val[32];
+    __shared__ long long s_idx[32];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double mv = __longlong_as_double((long long)0xfff0000000000000ULL);   // -inf
+    long long mi = 0x7fffffffffffffffLL;
+    for (long long i = threadIdx.x; i < n; i += blockDim.x) {
+        const double c = sde[i];
+        if (c > mv || (c == mv && i < mi)) { mv = c; mi = i; }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const double ov = __shfl_xor_sync(0xffffffffu, mv, o);
+        const long long oi = __shfl_xor_sync(0xffffffffu, mi, o);
+        if (ov > mv || (ov == mv && oi < mi)) { mv = ov; mi = oi; }
+    }
+    if (lane == 0) { s_val[warp] = mv; s_idx[warp] = mi; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int k = 1; k < (int)(blockDim.x >> 5); ++k)
+            if (s_val[k] > mv || (s_val[k] == mv && s_idx[k] < mi)) { mv = s_val[k]; mi = s_idx[k]; }
+        if (sc->degenerate) { mi = sc->argmin; mv = 0.0; }
+        sc->sde_max = mv; sc->sde_argmax = mi;
+        sc->sde_raw_best = sde_raw[sc->argmin];
+    }
+}
+
+}  // namespace
+
+void launch_sde(const double* chi2, long long n_per, int kernel, double* sde_raw, double* sde,
+                SdeScratch* scratch, cudaStream_t st, int* n_launches) {
+    long long b = (n_per + 255) / 256;
+    const int blocks = (int)(b > 148 * 16 ? 148 * 16 : b);
+    long long bm = (n_per + 127) / 128;
+    const int mblocks = (int)(bm > 148 * 64 ? 148 * 64 : bm);
+    k_sde_stats<<<1, kRedThreads, 0, st>>>(chi2, n_per, scratch);
+    k_sde_raw<<<blocks, 256, 0, st>>>(chi2, n_per, scratch, sde_raw);
+    k_sde_median<<<mblocks, 128, 0, st>>>(sde_raw, n_per, kernel, scratch, sde);
+    k_sde_argmax<<<1, kRedThreads, 0, st>>>(sde, sde_raw, n_per, scratch);
+    if (n_launches) *n_launches += 4;
+}
+
+}  // namespace gtls

@@ -1,0 +1,570 @@
+// C ABI of libgtls (include/gtls.h): argument validation, device memory, the period-tile
+// loop and the epilogue.  All arithmetic of the search runs in the kernels of pre.cu,
+// fold_sort.cu, scan.cu, chi2.cu and epilogue.cu; there is no CPU fallback.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "gtls_internal.cuh"
+
+using namespace gtls;
+
+namespace {
+
+thread_local char g_cuda_err[512] = "";
+
+int cuda_fail(cudaError_t e, const char* what) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s (%s)", what, cudaGetErrorString(e),
+             cudaGetErrorName(e));
+    return GTLS_ECUDA;
+}
+#define CU(call)                                                   \
+    do {                                                           \
+        cudaError_t e_ = (call);                                   \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call);        \
+    } while (0)
+
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+// Bump allocator over one device block.
+struct Arena {
+    char* base = nullptr;
+    size_t size = 0, off = 0;
+    bool owned = false;
+    template <typename T>
+    T* take(size_t count) {
+        off = align_up(off);
+        T* p = reinterpret_cast<T*>(base + off);
+        off += count * sizeof(T);
+        return off <= size ? p : nullptr;
+    }
+    ~Arena() { if (owned && base) cudaFree(base); }
+};
+
+struct Sizes {
+    size_t fixed;        // per-call arrays
+    size_t per_period;   // per period in flight
+};
+
+// pitch of the padded folded arrays for a largest duration fraction q_max
+inline int pitch_for(long long n, double q_max) {
+    long long dmax = (long long)(q_max * (double)n);
+    if (dmax < 1) dmax = 1;
+    if (dmax > n - 1) dmax = n - 1;
+    return (int)((n + dmax + 7) / 8 * 8);
+}
+
+Sizes workspace_sizes(long long n, long long n_per, int n_dur, double q_max, bool uniform) {
+    Sizes s;
+    const int pitch = pitch_for(n, q_max);
+    const int spitch = pitch + 8;
+    const int nt = (int)((n + kRadixTile - 1) / kRadixTile);
+    s.fixed = 3 * align_up(n * sizeof(double)) + align_up(sizeof(CurveInfo)) +
+              align_up(sizeof(SdeScratch)) + align_up(2 * sizeof(unsigned long long)) +
+              2 * align_up(n_per * sizeof(double)) + align_up(n_per * sizeof(gtls_best)) + 4096;
+    s.per_period = 2 * n * sizeof(u64) + 256ull * nt * sizeof(u32) + n_dur * sizeof(DurEntry) +
+                   n_dur * sizeof(Partial) +
+                   (uniform ? 1 : 2) * ((size_t)pitch + spitch) * sizeof(double);
+    return s;
+}
+
+int auto_tile(long long n_per, const Sizes& s, size_t budget) {
+    long long t = (long long)(budget / s.per_period);
+    if (t > 4096) t = 4096;
+    if (t > n_per) t = n_per;
+    if (t < 1) t = 1;
+    return (int)t;
+}
+
+constexpr size_t kDefaultTileBudget = 3ull << 30;   // bytes of per-tile scratch when automatic
+
+gtls_opts resolve_opts(const gtls_opts* in) {
+    gtls_opts o;
+    gtls_opts_default(&o);
+    if (in) {
+        size_t sz = in->struct_size ? in->struct_size : sizeof(gtls_opts);
+        if (sz > sizeof(gtls_opts)) sz = sizeof(gtls_opts);
+        memcpy(&o, in, sz);
+        o.struct_size = sizeof(gtls_opts);
+    }
+    return o;
+}
+
+struct Timer {       // optional per-stage CUDA-event timing (opts->stats)
+    bool on = false;
+    cudaStream_t st = nullptr;
+    cudaEvent_t ev[9] = {};
+    void init(bool enable, cudaStream_t s) {
+        on = enable; st = s;
+        if (on) for (auto& e : ev) cudaEventCreate(&e);
+    }
+    void mark(int k) { if (on) cudaEventRecord(ev[k], st); }
+    double ms(int a, int b) { float f = 0.f; cudaEventElapsedTime(&f, ev[a], ev[b]); return f; }
+    ~Timer() { if (on) for (auto& e : ev) cudaEventDestroy(e); }
+};
+
+// Copies (host mode) or aliases (device mode) an input array.
+template <typename T>
+int stage_in(const T* src, size_t count, bool on_device, Arena& ar, cudaStream_t st, const T** out) {
+    if (on_device) { *out = src; return GTLS_OK; }
+    T* d = ar.take<T>(count);
+    if (!d) return GTLS_ENOMEM;
+    CU(cudaMemcpyAsync(d, src, count * sizeof(T), cudaMemcpyHostToDevice, st));
+    *out = d;
+    return GTLS_OK;
+}
+
+int alloc_arena(Arena& ar, size_t bytes) {
+    cudaError_t e = cudaMalloc((void**)&ar.base, bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); snprintf(g_cuda_err, sizeof(g_cuda_err), "cudaMalloc(%zu): %s", bytes, cudaGetErrorString(e)); return GTLS_ENOMEM; }
+    ar.size = bytes; ar.off = 0; ar.owned = true;
+    return GTLS_OK;
+}
+
+// Shared front end of the debug exports: curve arrays + sorted keys for `tile` periods.
+struct CurveDev {
+    const double *t = nullptr, *y = nullptr, *dy = nullptr;
+    double *wr = nullptr, *w = nullptr, *wr2 = nullptr;
+    CurveInfo* info = nullptr;
+};
+
+}  // namespace
+
+extern "C" {
+
+void gtls_opts_default(gtls_opts* o) {
+    if (!o) return;
+    memset(o, 0, sizeof(*o));
+    o->struct_size = sizeof(gtls_opts);
+    o->dt0 = 0.05;
+    o->sde_kernel = 151;
+}
+
+const char* gtls_version(void) { return "gtls-b200 0.1.0 (sm_100a)"; }
+const char* gtls_last_cuda_error(void) { return g_cuda_err; }
+
+const char* gtls_strerror(int code) {
+    switch (code) {
+        case GTLS_OK: return "ok";
+        case GTLS_EINVAL: return "invalid argument";
+        case GTLS_ENONFINITE: return "non-finite value in t/y/dy, or dy <= 0";
+        case GTLS_EGRID: return "period <= 0 or duration fraction outside (0, 0.5]";
+        case GTLS_ENOMEM: return "out of device memory or workspace too small";
+        case GTLS_ECUDA: return "CUDA error (see gtls_last_cuda_error)";
+        case GTLS_EDEGENERATE: return "degenerate spectrum (chi2_min == 0 or sigma_SR == 0); SDE set to 0";
+        case GTLS_EUNSUPPORTED: return "option not supported";
+        default: return "unknown error code";
+    }
+}
+
+size_t gtls_workspace_bytes(int64_t n, int64_t n_per, int32_t n_dur, const gtls_opts* opts) {
+    if (n < 3 || n_per < 1 || n_dur < 1) return 0;
+    const gtls_opts o = resolve_opts(opts);
+    const Sizes s = workspace_sizes(n, n_per, n_dur, 0.5, false);     // worst case
+    const int tile = o.period_tile > 0 ? (int)(o.period_tile < n_per ? o.period_tile : n_per)
+                                       : auto_tile(n_per, s, kDefaultTileBudget);
+    return s.fixed + (size_t)tile * align_up(s.per_period) + 64 * 256;
+}
+
+int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
+                const double* period_grid, int64_t n_per, const double* duration_grid,
+                int32_t n_dur, const double* tmpl, int32_t n_tmpl, const gtls_opts* opts,
+                double* out_chi2, gtls_best* out_best, double* out_sde_raw, double* out_sde,
+                gtls_summary* out_summary) {
+    g_cuda_err[0] = 0;
+    const gtls_opts o = resolve_opts(opts);
+    if (!t || !y || !dy || !period_grid || !duration_grid || !tmpl || !out_chi2) return GTLS_EINVAL;
+    if (n < 3 || n > 0x3fffffff || n_per < 1 || n_dur < 1 || n_dur > 4096 || n_tmpl < 2) return GTLS_EINVAL;
+    if (!(o.dt0 >= 0.0) || o.sde_kernel < 0 || (o.sde_kernel > 1 && o.sde_kernel % 2 == 0)) return GTLS_EINVAL;
+    if (o.path < 0 || o.path > 2 || o.period_tile < 0) return GTLS_EINVAL;
+    if (o.top_k != 0 || o.chi2_fp32 != 0) return GTLS_EUNSUPPORTED;
+    if (o.path == 1) return GTLS_EUNSUPPORTED;   // fused shared-memory path: not built yet
+    CU(cudaSetDevice(o.device));
+    cudaStream_t st = (cudaStream_t)o.stream;
+    const bool dev = o.pointers_on_device != 0;
+    const long long n_durs_total = o.dur_per_period ? n_per * (long long)n_dur : n_dur;
+
+    // ---- device memory -----------------------------------------------------------------
+    Arena io;          // host mode: staged inputs and outputs
+    if (!dev) {
+        size_t bytes = 3 * align_up(n * 8) + align_up(n_per * 8) + align_up(n_durs_total * 8) +
+                       align_up(n_tmpl * 8) + 3 * align_up(n_per * 8) +
+                       align_up(n_per * sizeof(gtls_best)) + 16 * 256;
+        int rc = alloc_arena(io, bytes);
+        if (rc) return rc;
+    }
+    const double *d_t, *d_y, *d_dy, *d_per, *d_dur, *d_tmpl;
+    int rc;
+    if ((rc = stage_in(t, n, dev, io, st, &d_t))) return rc;
+    if ((rc = stage_in(y, n, dev, io, st, &d_y))) return rc;
+    if ((rc = stage_in(dy, n, dev, io, st, &d_dy))) return rc;
+    if ((rc = stage_in(period_grid, n_per, dev, io, st, &d_per))) return rc;
+    if ((rc = stage_in(duration_grid, n_durs_total, dev, io, st, &d_dur))) return rc;
+    if ((rc = stage_in(tmpl, n_tmpl, dev, io, st, &d_tmpl))) return rc;
+    double* d_chi2 = dev ? out_chi2 : io.take<double>(n_per);
+    double* d_sde_raw_out = dev ? out_sde_raw : (out_sde_raw ? io.take<double>(n_per) : nullptr);
+    double* d_sde_out = dev ? out_sde : (out_sde ? io.take<double>(n_per) : nullptr);
+    gtls_best* d_best_out = dev ? out_best : (out_best ? io.take<gtls_best>(n_per) : nullptr);
+    if (!d_chi2) return GTLS_ENOMEM;
+
+    Arena ws;
+    const Sizes worst = workspace_sizes(n, n_per, n_dur, 0.5, false);
+    if (o.workspace) {
+        ws.base = (char*)o.workspace; ws.size = o.workspace_bytes; ws.owned = false;
+        if (((uintptr_t)ws.base & 255) != 0) return GTLS_EINVAL;
+        if (ws.size < worst.fixed + align_up(worst.per_period)) return GTLS_ENOMEM;
+    } else {
+        const size_t need = gtls_workspace_bytes(n, n_per, n_dur, &o);
+        if ((rc = alloc_arena(ws, need))) return rc;
+    }
+    double* d_wr = ws.take<double>(n);
+    double* d_w = ws.take<double>(n);
+    double* d_wr2 = ws.take<double>(n);
+    CurveInfo* d_info = ws.take<CurveInfo>(1);
+    SdeScratch* d_sde_sc = ws.take<SdeScratch>(1);
+    unsigned long long* d_counters = ws.take<unsigned long long>(2);
+    double* d_sde_raw = d_sde_raw_out ? d_sde_raw_out : ws.take<double>(n_per);
+    double* d_sde = d_sde_out ? d_sde_out : ws.take<double>(n_per);
+    gtls_best* d_best = d_best_out ? d_best_out : ws.take<gtls_best>(n_per);
+    if (!d_best) return GTLS_ENOMEM;
+
+    Timer tm;
+    tm.init(o.stats != nullptr, st);
+    cudaEvent_t ev_begin = nullptr, ev_end = nullptr;
+    if (o.stats) { cudaEventCreate(&ev_begin); cudaEventCreate(&ev_end); cudaEventRecord(ev_begin, st); }
+    gtls_stats stats;
+    memset(&stats, 0, sizeof(stats));
+
+    // ---- a0: per-curve arrays + validation ----------------------------------------------
+    tm.mark(0);
+    CU(cudaMemsetAsync(d_info, 0, sizeof(CurveInfo), st));
+    CU(cudaMemsetAsync(d_counters, 0, 2 * sizeof(unsigned long long), st));
+    launch_curve_pre(d_t, d_y, d_dy, (int)n, d_wr, d_w, d_wr2, d_info, st);
+    launch_grid_check(d_per, n_per, d_dur, n_durs_total, d_info, st);
+    stats.kernel_launches += 2;
+    CurveInfo info;
+    CU(cudaMemcpyAsync(&info, d_info, sizeof(info), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    CU(cudaGetLastError());
+    if (info.bad_curve) return GTLS_ENONFINITE;
+    if (info.bad_period || info.bad_duration) return GTLS_EGRID;
+    tm.mark(1);
+    if (o.stats) { CU(cudaStreamSynchronize(st)); stats.ms_pre += tm.ms(0, 1); }
+    const bool uniform = info.w_min == info.w_max;
+
+    // ---- tile geometry -------------------------------------------------------------------
+    const Sizes sz = workspace_sizes(n, n_per, n_dur, info.q_max, uniform);
+    const size_t avail = ws.size - align_up(ws.off) - 32 * 256;
+    long long tile_cap = (long long)(avail / align_up(sz.per_period + 8 * 256));
+    int tile = o.period_tile > 0 ? o.period_tile : auto_tile(n_per, sz, kDefaultTileBudget);
+    if (tile > tile_cap) tile = (int)tile_cap;
+    if (tile > n_per) tile = (int)n_per;
+    if (tile < 1) return GTLS_ENOMEM;
+    TileArgs a;
+    memset(&a, 0, sizeof(a));
+    a.n = (int)n; a.n_dur = n_dur; a.n_tmpl = n_tmpl; a.dur_per_period = o.dur_per_period;
+    a.dt0 = o.dt0; a.uniform = uniform ? 1 : 0; a.w_uniform = info.w_min;
+    a.pitch = pitch_for(n, info.q_max); a.spitch = a.pitch + 8;
+    a.t = d_t; a.wr = d_wr; a.w = d_w; a.wr2 = d_wr2; a.periods = d_per; a.durs = d_dur;
+    a.tmpl = d_tmpl; a.chi2_0 = &d_info->chi2_0;
+    const int nt = (int)((n + kRadixTile - 1) / kRadixTile);
+    a.keys_a = ws.take<u64>((size_t)tile * n);
+    a.keys_b = ws.take<u64>((size_t)tile * n);
+    a.counts = ws.take<u32>((size_t)tile * 256 * nt);
+    a.durtab = ws.take<DurEntry>((size_t)tile * n_dur);
+    a.partial = ws.take<Partial>((size_t)tile * n_dur);
+    a.x1 = ws.take<double>((size_t)tile * a.pitch);
+    a.s1 = ws.take<double>((size_t)tile * a.spitch);
+    if (!uniform) {
+        a.x0 = ws.take<double>((size_t)tile * a.pitch);
+        a.s0 = ws.take<double>((size_t)tile * a.spitch);
+    }
+    if (!a.s1 || (!uniform && !a.s0)) return GTLS_ENOMEM;
+
+    // ---- period tiles ----------------------------------------------------------------------
+    for (long long p0 = 0; p0 < n_per; p0 += tile) {
+        a.p0 = p0;
+        a.tile = (int)((n_per - p0) < tile ? (n_per - p0) : tile);
+        int launches = 0;
+        tm.mark(0);
+        launch_durtab(a, st);
+        tm.mark(1);
+        launch_fold_keys(a, nullptr, st);
+        tm.mark(2);
+        const u64* sorted = launch_phase_sort(a, st, &launches);
+        tm.mark(3);
+        launch_gather_scan(a, sorted, nullptr, nullptr, -1, st);
+        tm.mark(4);
+        launch_chi2(a, st);
+        tm.mark(5);
+        launch_reduce(a, sorted, d_chi2, d_best, d_counters, st);
+        tm.mark(6);
+        stats.kernel_launches += launches + 5;
+        stats.chi2_launches += 1;
+        if (o.stats) {
+            CU(cudaStreamSynchronize(st));
+            stats.ms_pre += tm.ms(0, 1); stats.ms_fold += tm.ms(1, 2); stats.ms_sort += tm.ms(2, 3);
+            stats.ms_scan += tm.ms(3, 4); stats.ms_chi2 += tm.ms(4, 5); stats.ms_reduce += tm.ms(5, 6);
+        }
+    }
+    CU(cudaGetLastError());
+
+    // ---- a9: SR / SDE epilogue --------------------------------------------------------------
+    tm.mark(0);
+    int launches = 0;
+    launch_sde(d_chi2, n_per, o.sde_kernel, d_sde_raw, d_sde, d_sde_sc, st, &launches);
+    stats.kernel_launches += launches;
+    tm.mark(1);
+    SdeScratch sc;
+    unsigned long long counters[2];
+    CU(cudaMemcpyAsync(&sc, d_sde_sc, sizeof(sc), cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(counters, d_counters, sizeof(counters), cudaMemcpyDeviceToHost, st));
+    if (o.stats) cudaEventRecord(ev_end, st);
+    CU(cudaStreamSynchronize(st));
+    CU(cudaGetLastError());
+    if (o.stats) stats.ms_epilogue = tm.ms(0, 1);
+
+    if (out_summary) {
+        gtls_best b;
+        double period = 0.0;
+        CU(cudaMemcpyAsync(&b, d_best + sc.argmin, sizeof(b), cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(&period, d_per + sc.argmin, sizeof(double), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        out_summary->best_period_idx = sc.argmin;
+        out_summary->best_dur_idx = b.dur_idx;
+        out_summary->best_start = b.start;
+        out_summary->best_period = period;
+        out_summary->best_t0 = b.t0;
+        out_summary->best_depth = b.depth;
+        out_summary->chi2_min = sc.chi2_min;
+        out_summary->chi2_null = info.chi2_0;
+        out_summary->sde_raw_max = sc.sde_raw_best;
+        out_summary->sde_max = sc.sde_max;
+        out_summary->sde_argmax = sc.sde_argmax;
+        out_summary->windows_evaluated = (int64_t)counters[0];
+    }
+    if (!dev) {
+        CU(cudaMemcpyAsync(out_chi2, d_chi2, n_per * sizeof(double), cudaMemcpyDeviceToHost, st));
+        if (out_best) CU(cudaMemcpyAsync(out_best, d_best, n_per * sizeof(gtls_best), cudaMemcpyDeviceToHost, st));
+        if (out_sde_raw) CU(cudaMemcpyAsync(out_sde_raw, d_sde_raw, n_per * sizeof(double), cudaMemcpyDeviceToHost, st));
+        if (out_sde) CU(cudaMemcpyAsync(out_sde, d_sde, n_per * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+    }
+    if (o.stats) {
+        float f = 0.f;
+        cudaEventElapsedTime(&f, ev_begin, ev_end);
+        stats.ms_total = f;
+        stats.windows = (int64_t)counters[0];
+        stats.window_points = (int64_t)counters[1];
+        stats.period_points = n * n_per;
+        stats.period_tile = tile;
+        stats.path = 2;
+        stats.uniform_dy = uniform ? 1 : 0;
+        *o.stats = stats;
+        cudaEventDestroy(ev_begin); cudaEventDestroy(ev_end);
+    }
+    return sc.degenerate ? GTLS_EDEGENERATE : GTLS_OK;
+}
+
+int gtls_fold_sort(const double* t, int64_t n, const double* periods, int64_t n_per,
+                   const gtls_opts* opts, double* out_phase, int32_t* out_perm) {
+    g_cuda_err[0] = 0;
+    const gtls_opts o = resolve_opts(opts);
+    if (!t || !periods || !out_perm || n < 1 || n > 0x3fffffff || n_per < 1) return GTLS_EINVAL;
+    CU(cudaSetDevice(o.device));
+    cudaStream_t st = (cudaStream_t)o.stream;
+    const bool dev = o.pointers_on_device != 0;
+    const int nt = (int)((n + kRadixTile - 1) / kRadixTile);
+    const size_t per_period = 2 * n * sizeof(u64) + 256ull * nt * sizeof(u32) +
+                              (dev ? 0 : n * (sizeof(double) + sizeof(int32_t))) + 1024;
+    long long tile = (long long)((1ull << 30) / per_period);
+    if (o.period_tile > 0) tile = o.period_tile;
+    if (tile > n_per) tile = n_per;
+    if (tile < 1) tile = 1;
+    Arena ar;
+    int rc = alloc_arena(ar, align_up(n * 8) + align_up(n_per * 8) + tile * align_up(per_period) + 16 * 256);
+    if (rc) return rc;
+    const double *d_t, *d_per;
+    if ((rc = stage_in(t, n, dev, ar, st, &d_t))) return rc;
+    if ((rc = stage_in(periods, n_per, dev, ar, st, &d_per))) return rc;
+    TileArgs a;
+    memset(&a, 0, sizeof(a));
+    a.n = (int)n; a.t = d_t; a.periods = d_per;
+    a.keys_a = ar.take<u64>((size_t)tile * n);
+    a.keys_b = ar.take<u64>((size_t)tile * n);
+    a.counts = ar.take<u32>((size_t)tile * 256 * nt);
+    double* d_phase = dev ? nullptr : (out_phase ? ar.take<double>((size_t)tile * n) : nullptr);
+    int32_t* d_perm = dev ? nullptr : ar.take<int32_t>((size_t)tile * n);
+    if (!a.counts || (!dev && !d_perm)) return GTLS_ENOMEM;
+    for (long long p0 = 0; p0 < n_per; p0 += tile) {
+        a.p0 = p0;
+        a.tile = (int)((n_per - p0) < tile ? (n_per - p0) : tile);
+        const size_t cnt = (size_t)a.tile * n;
+        double* ph = dev ? (out_phase ? out_phase + p0 * n : nullptr) : d_phase;
+        int32_t* pm = dev ? out_perm + p0 * n : d_perm;
+        launch_fold_keys(a, ph, st);
+        const u64* sorted = launch_phase_sort(a, st, nullptr);
+        launch_perm_export(sorted, (long long)cnt, pm, st);
+        if (!dev) {
+            if (out_phase) CU(cudaMemcpyAsync(out_phase + p0 * n, ph, cnt * sizeof(double), cudaMemcpyDeviceToHost, st));
+            CU(cudaMemcpyAsync(out_perm + p0 * n, pm, cnt * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+            CU(cudaStreamSynchronize(st));
+        }
+    }
+    CU(cudaStreamSynchronize(st));
+    CU(cudaGetLastError());
+    return GTLS_OK;
+}
+
+// Front end shared by the single-period debug exports: curve arrays, sorted keys, padded
+// prefix sums of x1, x0, x2 for one period with `pad` wrap entries.
+static int one_period_scan(const double* t, const double* y, const double* dy, int64_t n,
+                           double period, int64_t pad, const gtls_opts& o, Arena& ar, TileArgs& a,
+                           double** d_s2) {
+    cudaStream_t st = (cudaStream_t)o.stream;
+    const bool dev = o.pointers_on_device != 0;
+    const int nt = (int)((n + kRadixTile - 1) / kRadixTile);
+    const int pitch = (int)((n + pad + 7) / 8 * 8), spitch = pitch + 8;
+    size_t bytes = 8 * align_up(n * 8) + 2 * align_up(n * sizeof(u64)) + align_up(256ull * nt * 4) +
+                   3 * align_up((size_t)pitch * 8) + 3 * align_up((size_t)spitch * 8) +
+                   6 * align_up((size_t)n * 8) + 64 * 256;
+    int rc = alloc_arena(ar, bytes);
+    if (rc) return rc;
+    const double *d_t, *d_y, *d_dy;
+    if ((rc = stage_in(t, n, dev, ar, st, &d_t))) return rc;
+    if ((rc = stage_in(y, n, dev, ar, st, &d_y))) return rc;
+    if ((rc = stage_in(dy, n, dev, ar, st, &d_dy))) return rc;
+    double* d_wr = ar.take<double>(n);
+    double* d_w = ar.take<double>(n);
+    double* d_wr2 = ar.take<double>(n);
+    CurveInfo* d_info = ar.take<CurveInfo>(1);
+    double* d_period = ar.take<double>(1);
+    CU(cudaMemsetAsync(d_info, 0, sizeof(CurveInfo), st));
+    CU(cudaMemcpyAsync(d_period, &period, sizeof(double), cudaMemcpyHostToDevice, st));
+    launch_curve_pre(d_t, d_y, d_dy, (int)n, d_wr, d_w, d_wr2, d_info, st);
+    CurveInfo info;
+    CU(cudaMemcpyAsync(&info, d_info, sizeof(info), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    if (info.bad_curve) return GTLS_ENONFINITE;
+    memset(&a, 0, sizeof(a));
+    a.n = (int)n; a.tile = 1; a.p0 = 0; a.t = d_t; a.wr = d_wr; a.w = d_w; a.wr2 = d_wr2;
+    a.periods = d_period; a.chi2_0 = &d_info->chi2_0; a.pitch = pitch; a.spitch = spitch;
+    a.dt0 = o.dt0; a.uniform = 0;
+    a.keys_a = ar.take<u64>(n); a.keys_b = ar.take<u64>(n); a.counts = ar.take<u32>(256ull * nt);
+    a.x1 = ar.take<double>(pitch); a.x0 = ar.take<double>(pitch);
+    double* x2 = ar.take<double>(pitch);
+    a.s1 = ar.take<double>(spitch); a.s0 = ar.take<double>(spitch);
+    *d_s2 = ar.take<double>(spitch);
+    if (!*d_s2) return GTLS_ENOMEM;
+    launch_fold_keys(a, nullptr, st);
+    const u64* sorted = launch_phase_sort(a, st, nullptr);
+    launch_gather_scan(a, sorted, x2, *d_s2, (int)pad, st);
+    return GTLS_OK;
+}
+
+int gtls_fold_scan(const double* t, const double* y, const double* dy, int64_t n, double period,
+                   int64_t pad, const gtls_opts* opts, double* out_s1, double* out_s0,
+                   double* out_s2) {
+    g_cuda_err[0] = 0;
+    const gtls_opts o = resolve_opts(opts);
+    if (!t || !y || !dy || n < 1 || n > 0x3fffffff || pad < 0 || pad > n || !(period > 0.0)) return GTLS_EINVAL;
+    CU(cudaSetDevice(o.device));
+    cudaStream_t st = (cudaStream_t)o.stream;
+    Arena ar;
+    TileArgs a;
+    double* d_s2 = nullptr;
+    int rc = one_period_scan(t, y, dy, n, period, pad, o, ar, a, &d_s2);
+    if (rc) return rc;
+    const size_t cnt = (size_t)(n + pad + 1) * sizeof(double);
+    const cudaMemcpyKind kind = o.pointers_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    if (out_s1) CU(cudaMemcpyAsync(out_s1, a.s1, cnt, kind, st));
+    if (out_s0) CU(cudaMemcpyAsync(out_s0, a.s0, cnt, kind, st));
+    if (out_s2) CU(cudaMemcpyAsync(out_s2, d_s2, cnt, kind, st));
+    CU(cudaStreamSynchronize(st));
+    CU(cudaGetLastError());
+    return GTLS_OK;
+}
+
+int64_t gtls_window_chi2(const double* t, const double* y, const double* dy, int64_t n,
+                         double period, double q, const double* tmpl, int32_t n_tmpl,
+                         const gtls_opts* opts, int32_t* out_start, double* out_depth,
+                         double* out_chi2_out, double* out_chi2_in) {
+    g_cuda_err[0] = 0;
+    const gtls_opts o = resolve_opts(opts);
+    if (!t || !y || !dy || !tmpl || !out_start || !out_depth || !out_chi2_out || !out_chi2_in) return GTLS_EINVAL;
+    if (n < 3 || n > 0x3fffffff || n_tmpl < 2 || !(period > 0.0) || !(q > 0.0) || !(q <= 0.5) || !(o.dt0 >= 0.0)) return GTLS_EINVAL;
+    CU(cudaSetDevice(o.device));
+    cudaStream_t st = (cudaStream_t)o.stream;
+    const bool dev = o.pointers_on_device != 0;
+    long long D = (long long)(q * (double)n);
+    D = D < 1 ? 1 : (D > n - 1 ? n - 1 : D);
+    long long stride = o.dt0 > 0.0 ? (long long)((double)D * o.dt0) : 1;
+    if (stride < 1) stride = 1;
+    const long long nW = (n + stride - 1) / stride;
+    Arena ar;
+    TileArgs a;
+    double* d_s2 = nullptr;
+    int rc = one_period_scan(t, y, dy, n, period, D, o, ar, a, &d_s2);
+    if (rc) return rc;
+    const double* d_tmpl;
+    Arena ar2;
+    if ((rc = alloc_arena(ar2, align_up(n_tmpl * 8) + 4 * align_up(nW * 8) + 16 * 256))) return rc;
+    if ((rc = stage_in(tmpl, n_tmpl, dev, ar2, st, &d_tmpl))) return rc;
+    a.tmpl = d_tmpl; a.n_tmpl = n_tmpl;
+    int32_t* ds = dev ? out_start : ar2.take<int32_t>(nW);
+    double* dd = dev ? out_depth : ar2.take<double>(nW);
+    double* dco = dev ? out_chi2_out : ar2.take<double>(nW);
+    double* dci = dev ? out_chi2_in : ar2.take<double>(nW);
+    if (!dci) return GTLS_ENOMEM;
+    launch_window_export(a, d_s2, q, ds, dd, dco, dci, st);
+    if (!dev) {
+        CU(cudaMemcpyAsync(out_start, ds, nW * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(out_depth, dd, nW * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(out_chi2_out, dco, nW * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(out_chi2_in, dci, nW * sizeof(double), cudaMemcpyDeviceToHost, st));
+    }
+    CU(cudaStreamSynchronize(st));
+    CU(cudaGetLastError());
+    return nW;
+}
+
+int gtls_sde(const double* chi2, int64_t n_per, const gtls_opts* opts, double* out_sde_raw,
+             double* out_sde, gtls_summary* out_summary) {
+    g_cuda_err[0] = 0;
+    const gtls_opts o = resolve_opts(opts);
+    if (!chi2 || n_per < 1) return GTLS_EINVAL;
+    if (o.sde_kernel < 0 || (o.sde_kernel > 1 && o.sde_kernel % 2 == 0)) return GTLS_EINVAL;
+    CU(cudaSetDevice(o.device));
+    cudaStream_t st = (cudaStream_t)o.stream;
+    const bool dev = o.pointers_on_device != 0;
+    Arena ar;
+    int rc = alloc_arena(ar, 3 * align_up(n_per * 8) + 8 * 256);
+    if (rc) return rc;
+    const double* d_chi2;
+    if ((rc = stage_in(chi2, n_per, dev, ar, st, &d_chi2))) return rc;
+    double* d_raw = (dev && out_sde_raw) ? out_sde_raw : ar.take<double>(n_per);
+    double* d_sde = (dev && out_sde) ? out_sde : ar.take<double>(n_per);
+    SdeScratch* d_sc = ar.take<SdeScratch>(1);
+    if (!d_sc) return GTLS_ENOMEM;
+    launch_sde(d_chi2, n_per, o.sde_kernel, d_raw, d_sde, d_sc, st, nullptr);
+    SdeScratch sc;
+    CU(cudaMemcpyAsync(&sc, d_sc, sizeof(sc), cudaMemcpyDeviceToHost, st));
+    if (!dev) {
+        if (out_sde_raw) CU(cudaMemcpyAsync(out_sde_raw, d_raw, n_per * 8, cudaMemcpyDeviceToHost, st));
+        if (out_sde) CU(cudaMemcpyAsync(out_sde, d_sde, n_per * 8, cudaMemcpyDeviceToHost, st));
+    }
+    CU(cudaStreamSynchronize(st));
+    CU(cudaGetLastError());
+    if (out_summary) {
+        memset(out_summary, 0, sizeof(*out_summary));
+        out_summary->best_period_idx = sc.argmin;
+        out_summary->chi2_min = sc.chi2_min;
+        out_summary->sde_raw_max = sc.sde_raw_best;
+        out_summary->sde_max = sc.sde_max;
+        out_summary->sde_argmax = sc.sde_argmax;
+    }
+    return sc.degenerate ? GTLS_EDEGENERATE : GTLS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,145 @@
+// Internal declarations shared by the libgtls translation units (sm_100a only).
+// Not part of the ABI; see include/gtls.h for the boundary.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "gtls.h"
+
+namespace gtls {
+
+typedef unsigned long long u64;
+typedef unsigned int u32;
+
+// One (period, duration) trial, step a5 prerequisites.
+struct DurEntry {
+    int32_t D;        // points per duration: clamp(floor(q*n), 1, n-1)      (G11)
+    int32_t stride;   // max(1, floor(D*dt0))                                (Eq. 18, G9)
+    double  gbar;     // mean of the resampled template g_D                  (Eq. 12-13, G5/G6)
+    double  gg2;      // sum_j g_D[j]^2  (G = w * gg2 when dy is uniform)
+    int32_t skip;     // 1 when an earlier duration index of this period has the same D
+    int32_t pad_;
+};
+
+// Per-(period, duration) partial result of the window scan (a8 input).
+struct Partial {
+    double  dchi2;    // chi2 - chi2_0 of the best window of this trial
+    double  depth;
+    int32_t start;
+    int32_t valid;
+};
+
+// Flags and scalars produced by the a0 kernels and read back once by the host.
+struct CurveInfo {
+    double chi2_0;        // sum_i w_i r_i^2
+    double w_min, w_max;  // uniform-dy detection
+    double q_max;         // largest duration fraction in the grid
+    int32_t bad_curve;    // count of non-finite t/y/dy or dy <= 0
+    int32_t bad_period;   // count of non-finite or <= 0 periods
+    int32_t bad_duration; // count of fractions outside (0, 0.5]
+    int32_t pad_;
+};
+
+constexpr int kRadixThreads = 256;
+constexpr int kRadixItems = 8;
+constexpr int kRadixTile = kRadixThreads * kRadixItems;   // 2048 keys per CTA
+constexpr int kRadixWarps = kRadixThreads / 32;
+
+// ---- phase / template arithmetic shared by kernels -------------------------------------
+// Eq. 10: one IEEE fp64 division, floor, exact subtraction.  No reciprocal
+// multiply and no fast-math anywhere in this library, so phases are bit-identical to any
+// IEEE-754 host evaluation of the same expression.
+__device__ __forceinline__ double fold_phase(double t, double period) {
+    const double q = __ddiv_rn(t, period);
+    return q - floor(q);
+}
+
+// Sortable key: floor(phase * 2^32) is a monotone (non-strict) map of the phase, so ordering
+// by (key32, full phase, index) equals ordering by (phase, index).  The rare equal-key runs
+// are re-ordered by the full fp64 phase in the tie fix-up kernel.
+__device__ __forceinline__ u32 phase_key32(double phase) {
+    const double s = phase * 4294967296.0;
+    return s >= 4294967295.0 ? 0xFFFFFFFFu : (u32)(u64)s;
+}
+
+// Template deficit resampled to D points by linear interpolation at cell centres (G14).
+__device__ __forceinline__ double tmpl_at(const double* __restrict__ tmpl, int n_tmpl, int j, int D) {
+    const double u = __ddiv_rn((double)j + 0.5, (double)D) * (double)(n_tmpl - 1);
+    int k = (int)floor(u);
+    k = k > n_tmpl - 2 ? n_tmpl - 2 : k;
+    k = k < 0 ? 0 : k;
+    const double frac = u - (double)k;
+    const double a = tmpl[k];
+    return a + frac * (tmpl[k + 1] - a);
+}
+
+__device__ __forceinline__ int points_in_duration(double q, int n) {
+    double d = floor(q * (double)n);
+    d = d < 1.0 ? 1.0 : d;
+    d = d > (double)(n - 1) ? (double)(n - 1) : d;
+    return (int)d;
+}
+
+__device__ __forceinline__ int t0_stride(int D, double dt0) {
+    if (!(dt0 > 0.0)) return 1;
+    const double s = floor((double)D * dt0);
+    return s < 1.0 ? 1 : (int)s;
+}
+
+// ---- host-side launchers (one per kernel family) ----------------------------------------
+struct TileArgs {
+    int n;                 // points in the light curve
+    int n_dur;
+    int n_tmpl;
+    int tile;              // periods in this tile
+    long long p0;          // index of the first period of the tile
+    int dur_per_period;
+    double dt0;
+    int uniform;           // all dy equal
+    double w_uniform;      // the common weight when uniform
+    int pitch;             // doubles per period in x1/x0 (>= n + Dmax)
+    int spitch;            // doubles per period in S1/S0 (= pitch + 1 rounded up)
+    const double* t;       // [n]
+    const double* wr;      // [n]  w_i r_i
+    const double* w;       // [n]  w_i
+    const double* wr2;     // [n]  w_i r_i^2 (debug exports only)
+    const double* periods; // [n_per]
+    const double* durs;    // duration grid
+    const double* tmpl;    // [n_tmpl]
+    const double* chi2_0;  // device scalar (CurveInfo::chi2_0)
+    u64* keys_a;           // [tile*n]
+    u64* keys_b;           // [tile*n]
+    u32* counts;           // [tile*256*nt]
+    DurEntry* durtab;      // [tile*n_dur]
+    double* x1; double* x0;   // [tile*pitch]
+    double* s1; double* s0;   // [tile*spitch]
+    Partial* partial;      // [tile*n_dur]
+};
+
+void launch_curve_pre(const double* t, const double* y, const double* dy, int n, double* wr,
+                      double* w, double* wr2, CurveInfo* info, cudaStream_t st);
+void launch_grid_check(const double* periods, long long n_per, const double* durs,
+                       long long n_durs_total, CurveInfo* info, cudaStream_t st);
+void launch_durtab(const TileArgs& a, cudaStream_t st);
+void launch_fold_keys(const TileArgs& a, double* phase_out, cudaStream_t st);
+// sorts keys_a (in place semantics: result is returned in the pointer the function returns)
+u64* launch_phase_sort(const TileArgs& a, cudaStream_t st, int* n_launches);
+void launch_gather_scan(const TileArgs& a, const u64* sorted, double* x2, double* s2,
+                        int pad_override, cudaStream_t st);
+void launch_chi2(const TileArgs& a, cudaStream_t st);
+// counters[0] += windows of all trials, counters[1] += sum of D over evaluated windows
+void launch_reduce(const TileArgs& a, const u64* sorted, double* out_chi2, gtls_best* out_best,
+                   unsigned long long* counters, cudaStream_t st);
+void launch_window_export(const TileArgs& a, const double* s2, double q, int32_t* out_start,
+                          double* out_depth, double* out_c_out, double* out_c_in, cudaStream_t st);
+void launch_perm_export(const u64* sorted, long long count, int32_t* out_perm, cudaStream_t st);
+
+struct SdeScratch {      // device scalars of the epilogue
+    double chi2_min, mean_sr, sd_sr, sde_raw_best, sde_max;
+    long long argmin, sde_argmax;
+    int degenerate, pad_;
+};
+void launch_sde(const double* chi2, long long n_per, int kernel, double* sde_raw, double* sde,
+                SdeScratch* scratch, cudaStream_t st, int* n_launches);
+
+}  // namespace gtls

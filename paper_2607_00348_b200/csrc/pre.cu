@@ -1,0 +1,146 @@
+// Step a0: per-curve arrays (w, w r, w r^2, chi2_0), input validation, and the per-tile
+// duration table (D, stride, mean(g_D), sum g_D^2) -- SURVEY 8(a) row a0, 8(c) step 3.
+#include "gtls_internal.cuh"
+
+namespace gtls {
+
+namespace {
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// One CTA of 1024 threads: deterministic strided accumulation + fixed-shape tree.
+__global__ void __launch_bounds__(1024) k_curve_pre(const double* __restrict__ t,
+                                                    const double* __restrict__ y,
+                                                    const double* __restrict__ dy, int n,
+                                                    double* __restrict__ wr, double* __restrict__ w,
+                                                    double* __restrict__ wr2, CurveInfo* info) {
+    __shared__ double s_sum[32], s_min[32], s_max[32];
+    __shared__ int s_bad[32];
+    double acc = 0.0, wmin = 1e300, wmax = 0.0;
+    int bad = 0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        const double ti = t[i], yi = y[i], di = dy[i];
+        const bool ok = isfinite(ti) && isfinite(yi) && isfinite(di) && di > 0.0;
+        bad += ok ? 0 : 1;
+        const double wi = __ddiv_rn(1.0, di * di);     // w_i = 1/dy_i^2
+        const double ri = 1.0 - yi;                    // flux deficit (model == 1)
+        const double wri = wi * ri;
+        const double wr2i = wri * ri;
+        w[i] = wi; wr[i] = wri; wr2[i] = wr2i;
+        acc += wr2i;
+        wmin = fmin(wmin, wi); wmax = fmax(wmax, wi);
+    }
+    acc = warp_sum(acc);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        wmin = fmin(wmin, __shfl_xor_sync(0xffffffffu, wmin, o));
+        wmax = fmax(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
+        bad += __shfl_xor_sync(0xffffffffu, bad, o);
+    }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) { s_sum[warp] = acc; s_min[warp] = wmin; s_max[warp] = wmax; s_bad[warp] = bad; }
+    __syncthreads();
+    if (warp == 0) {
+        const int nw = blockDim.x >> 5;
+        acc = lane < nw ? s_sum[lane] : 0.0;
+        wmin = lane < nw ? s_min[lane] : 1e300;
+        wmax = lane < nw ? s_max[lane] : 0.0;
+        bad = lane < nw ? s_bad[lane] : 0;
+        acc = warp_sum(acc);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            wmin = fmin(wmin, __shfl_xor_sync(0xffffffffu, wmin, o));
+            wmax = fmax(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
+            bad += __shfl_xor_sync(0xffffffffu, bad, o);
+        }
+        if (lane == 0) {
+            info->chi2_0 = acc; info->w_min = wmin; info->w_max = wmax; info->bad_curve = bad;
+        }
+    }
+}
+
+// Many CTAs; integer counters and the max are order independent, so atomics keep it exact.
+__global__ void __launch_bounds__(256) k_grid_check(const double* __restrict__ periods,
+                                                    long long n_per,
+                                                    const double* __restrict__ durs,
+                                                    long long n_durs, CurveInfo* info) {
+    int bp = 0, bd = 0;
+    double qmax = 0.0;
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long nth = (long long)gridDim.x * blockDim.x;
+    for (long long i = tid; i < n_per; i += nth) {
+        const double p = periods[i];
+        bp += (isfinite(p) && p > 0.0) ? 0 : 1;
+    }
+    for (long long i = tid; i < n_durs; i += nth) {
+        const double q = durs[i];
+        const bool ok = isfinite(q) && q > 0.0 && q <= 0.5;
+        bd += ok ? 0 : 1;
+        if (ok) qmax = fmax(qmax, q);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        bp += __shfl_xor_sync(0xffffffffu, bp, o);
+        bd += __shfl_xor_sync(0xffffffffu, bd, o);
+        qmax = fmax(qmax, __shfl_xor_sync(0xffffffffu, qmax, o));
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (bp) atomicAdd(&info->bad_period, bp);
+        if (bd) atomicAdd(&info->bad_duration, bd);
+        // positive doubles order like their bit patterns
+        atomicMax((unsigned long long*)&info->q_max, (unsigned long long)__double_as_longlong(qmax));
+    }
+}
+
+// One warp per (period, duration): D, stride, mean(g_D), sum g_D^2, duplicate-D flag.
+__global__ void __launch_bounds__(256) k_durtab(TileArgs a) {
+    const int warp_global = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (warp_global >= a.tile * a.n_dur) return;
+    const int pl = warp_global / a.n_dur, jd = warp_global % a.n_dur;
+    const double* qrow = a.dur_per_period ? a.durs + (a.p0 + pl) * (long long)a.n_dur : a.durs;
+    const int D = points_in_duration(qrow[jd], a.n);
+    int skip = 0;
+    for (int k = 0; k < jd; ++k) skip |= (points_in_duration(qrow[k], a.n) == D);
+    double sg = 0.0, sg2 = 0.0;
+    if (!skip) {
+        for (int j = lane; j < D; j += 32) {
+            const double g = tmpl_at(a.tmpl, a.n_tmpl, j, D);
+            sg += g; sg2 += g * g;
+        }
+        sg = warp_sum(sg); sg2 = warp_sum(sg2);
+    }
+    if (lane == 0) {
+        DurEntry e;
+        e.D = D; e.stride = t0_stride(D, a.dt0);
+        e.gbar = __ddiv_rn(sg, (double)D); e.gg2 = sg2; e.skip = skip; e.pad_ = 0;
+        a.durtab[(long long)pl * a.n_dur + jd] = e;
+    }
+}
+
+}  // namespace
+
+void launch_curve_pre(const double* t, const double* y, const double* dy, int n, double* wr,
+                      double* w, double* wr2, CurveInfo* info, cudaStream_t st) {
+    k_curve_pre<<<1, 1024, 0, st>>>(t, y, dy, n, wr, w, wr2, info);
+}
+
+void launch_grid_check(const double* periods, long long n_per, const double* durs,
+                       long long n_durs_total, CurveInfo* info, cudaStream_t st) {
+    long long work = n_durs_total > n_per ? n_durs_total : n_per;
+    int blocks = (int)((work + 256 * 8 - 1) / (256 * 8));
+    blocks = blocks < 1 ? 1 : (blocks > 1184 ? 1184 : blocks);
+    k_grid_check<<<blocks, 256, 0, st>>>(periods, n_per, durs, n_durs_total, info);
+}
+
+void launch_durtab(const TileArgs& a, cudaStream_t st) {
+    const long long warps = (long long)a.tile * a.n_dur;
+    const int blocks = (int)((warps * 32 + 255) / 256);
+    k_durtab<<<blocks, 256, 0, st>>>(a);
+}
+
+}  // namespace gtls

@@ -1,0 +1,260 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on
+the same seeded inputs.  Bars (BASELINE.json north_star): sort permutations and best
+(period, duration, start) indices bit-exact; chi2(P) within 1e-9 relative; SDE within 1e-6
+absolute.  Phases are compared bit for bit."""
+import numpy as np
+import pytest
+
+import gtls_inputs as gi
+import oracle
+import paper_2607_00348_b200 as g
+
+pytestmark = pytest.mark.gpu
+
+CHI2_RTOL = 1e-9
+SDE_ATOL = 1e-6
+
+
+def _cuda():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    return torch
+
+
+def _check_search(w, res, ora, sde_kernel=151, label=""):
+    chi2 = np.asarray(res.chi2)
+    best = res.best()
+    rel = np.abs(chi2 - ora.chi2) / np.maximum(np.abs(ora.chi2), 1e-300)
+    assert rel.max() <= CHI2_RTOL, f"{label}: chi2 rel err {rel.max():.3e}"
+    # near-tie rule: where the oracle's best / runner-up gap is below 1e-12 chi2
+    # either candidate is valid; everywhere else indices must match exactly
+    strict = ora.gap > 1e-12 * np.abs(ora.chi2)
+    mism = (best["dur_idx"] != ora.best["dur_idx"]) | (best["start"] != ora.best["start"])
+    assert not np.any(mism & strict), f"{label}: {np.sum(mism & strict)} index mismatches"
+    ok = ~mism
+    assert np.array_equal(best["t0"][ok], ora.best["t0"][ok]), f"{label}: t0"
+    drel = np.abs(best["depth"] - ora.best["depth"])[ok]
+    assert np.all(drel <= 1e-9 * np.abs(ora.best["depth"][ok]) + 1e-18), f"{label}: depth"
+    s = oracle.sde(ora.chi2, sde_kernel)
+    assert np.abs(np.asarray(res.sde_raw) - s.sde_raw).max() <= SDE_ATOL, f"{label}: sde_raw"
+    assert np.abs(np.asarray(res.sde) - s.sde).max() <= SDE_ATOL, f"{label}: sde"
+    assert res.summary["best_period_idx"] == s.best_period_idx
+    assert res.summary["sde_argmax"] == s.sde_argmax
+    assert abs(res.summary["chi2_null"] / ora.chi2_null - 1) < 1e-12
+    assert res.summary["windows_evaluated"] == ora.windows
+    return rel.max(), int(np.sum(mism))
+
+
+# ------------------------------------------------------------------------- a1 + a2
+@pytest.mark.parametrize("cfg,every", [(1, 97), (2, 331), (3, 20011)])
+def test_fold_sort_bit_exact(cfg, every):
+    _cuda()
+    w = gi.make_workload(cfg)
+    periods = np.ascontiguousarray(w.periods[::every])
+    phase, perm = g.gtls_fold_sort(w.lc.t, periods)
+    ph_o, pm_o = oracle.fold_sort(w.lc.t, periods)
+    assert np.array_equal(phase.view(np.uint64), ph_o.view(np.uint64))     # bit-exact phases
+    assert np.array_equal(perm, pm_o)
+
+
+def test_fold_sort_ties_and_tiny_inputs():
+    _cuda()
+    t = np.arange(64) / 2.0                                 # phases in {0, 1/4, 1/2, 3/4}
+    _, perm = g.gtls_fold_sort(t, np.array([2.0]))
+    assert np.array_equal(perm[0], np.concatenate([np.arange(r, 64, 4) for r in range(4)]))
+    t = np.arange(50) * 3.0                                 # all phases equal => identity
+    _, perm = g.gtls_fold_sort(t, np.array([3.0]))
+    assert np.array_equal(perm[0], np.arange(50))
+    # many equal 32-bit keys but distinct fp64 phases: exercises the tie fix-up
+    rng = np.random.default_rng(0)
+    t = np.sort(rng.uniform(0, 1e-7, 300)) + np.repeat(np.arange(3), 100) * 1.0
+    ph, perm = g.gtls_fold_sort(t, np.array([1.0, 0.5]))
+    ph_o, pm_o = oracle.fold_sort(t, np.array([1.0, 0.5]))
+    assert np.array_equal(perm, pm_o) and np.array_equal(ph.view(np.uint64), ph_o.view(np.uint64))
+    for n in (1, 2, 3, 31, 33, 2047, 2048, 2049):           # ragged tails around the radix tile
+        t = np.sort(rng.uniform(0, 50, n))
+        _, perm = g.gtls_fold_sort(t, np.array([0.7, 3.3]))
+        _, pm_o = oracle.fold_sort(t, np.array([0.7, 3.3]))
+        assert np.array_equal(perm, pm_o), n
+
+
+def test_fold_sort_unsorted_and_negative_times():
+    _cuda()
+    rng = np.random.default_rng(5)
+    t = rng.uniform(-40, 40, 5000)
+    ph, perm = g.gtls_fold_sort(t, np.array([0.9, 7.7]))
+    ph_o, pm_o = oracle.fold_sort(t, np.array([0.9, 7.7]))
+    assert np.array_equal(ph.view(np.uint64), ph_o.view(np.uint64)) and np.array_equal(perm, pm_o)
+
+
+def test_fold_sort_device_pointers_match_host():
+    torch = _cuda()
+    w = gi.make_workload(2)
+    periods = np.ascontiguousarray(w.periods[::997])
+    ph_h, pm_h = g.gtls_fold_sort(w.lc.t, periods)
+    ph_d, pm_d = g.gtls_fold_sort(torch.from_numpy(w.lc.t).cuda(), torch.from_numpy(periods).cuda())
+    assert np.array_equal(ph_d.cpu().numpy(), ph_h) and np.array_equal(pm_d.cpu().numpy(), pm_h)
+
+
+# ------------------------------------------------------------------------- a3 + a4
+@pytest.mark.parametrize("cfg,period,pad", [(1, 3.7, 220), (2, 0.731, 628), (3, 127.0, 9752), (3, 1.01, 0)])
+def test_prefix_sums_match_cumsum(cfg, period, pad):
+    _cuda()
+    w = gi.make_workload(cfg, hetero=True)
+    s1, s0, s2 = g.gtls_fold_scan(w.lc.t, w.lc.y, w.lc.dy, period, pad)
+    _, perm = oracle.fold_sort(w.lc.t, [period], want_phase=False)
+    sig = perm[0]
+    wt = 1.0 / w.lc.dy ** 2
+    r = 1.0 - w.lc.y
+    for got, x in ((s1, wt * r), (s0, wt), (s2, wt * r * r)):
+        xs = x[sig]
+        padded = np.concatenate([xs, xs[:pad]])
+        ref = np.concatenate([[0.0], np.cumsum(padded)])
+        scale = np.abs(padded).sum()
+        assert got.shape == ref.shape
+        assert np.abs(got - ref).max() <= 1e-13 * scale
+
+
+# ------------------------------------------------------------------------- a5-a7 per window
+@pytest.mark.parametrize("dt0", [0.0, 0.1])
+def test_window_terms_match_literal_oracle(dt0, tmpl512):
+    _cuda()
+    rng = np.random.default_rng(9)
+    n = 300
+    t = np.sort(rng.uniform(0, 30, n))
+    y = 1 + rng.normal(0, 1e-3, n)
+    dy = 1e-3 * rng.uniform(0.5, 2, n)
+    for period, q in ((2.3, 0.021), (7.9, 0.11), (0.61, 0.33)):
+        st, dep, c_out, c_in = g.gtls_window_chi2(t, y, dy, period, q, tmpl512, dt0=dt0)
+        st_o, dep_o, co_o, ci_o = oracle.window_chi2_literal(t, y, dy, period, q, tmpl512, dt0)
+        assert np.array_equal(st, st_o)
+        assert np.allclose(dep, dep_o, rtol=1e-9, atol=1e-15)
+        assert np.allclose(c_out, co_o, rtol=1e-11, atol=0)
+        assert np.allclose(c_in, ci_o, rtol=1e-9, atol=1e-9 * co_o.max())
+        assert np.allclose(c_out + c_in, co_o + ci_o, rtol=1e-10, atol=0)
+
+
+# ------------------------------------------------------------------------- whole path
+def test_search_c1_full():
+    _cuda()
+    w = gi.make_workload(1)
+    ora = oracle.search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05)
+    res = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05, stats=True)
+    _check_search(w, res, ora, label="c1")
+    assert res.code == 0 and res.stats["uniform_dy"] == 1
+    # recovered the injected planet (P3 on the GPU path)
+    assert abs(res.summary["best_period"] - w.lc.meta["period"]) < 0.01
+
+
+@pytest.mark.parametrize("cfg,every,hetero,dt0", [
+    (1, 7, True, 0.05), (1, 31, False, 0.0), (1, 31, True, 0.0), (1, 13, False, 0.01),
+    (2, 41, False, 0.05), (2, 101, True, 0.05), (2, 211, False, 0.1), (2, 499, True, 0.0),
+])
+def test_search_subsets(cfg, every, hetero, dt0):
+    _cuda()
+    w = gi.make_workload(cfg, hetero=hetero).subset(every)
+    ora = oracle.search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=dt0)
+    res = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=dt0,
+                        sde_kernel=31, stats=True)
+    _check_search(w, res, ora, sde_kernel=31, label=w.name)
+    assert res.stats["uniform_dy"] == (0 if hetero else 1)
+
+
+@pytest.mark.parametrize("cfg,count", [(3, 24), (4, 16)])
+def test_search_large_curves_sampled_periods(cfg, count):
+    """Full-size light curves (65k / 132k points) on a deterministic sample of periods spread
+    over the grid, in the same tiled launch configuration bench.py times."""
+    _cuda()
+    w0 = gi.make_workload(cfg)
+    w = w0.subset(w0.n_per // count)
+    ora = oracle.search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05)
+    res = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05,
+                        sde_kernel=5)
+    _check_search(w, res, ora, sde_kernel=5, label=w.name)
+    # the sort itself, bit for bit, on a few of those periods
+    _, perm = g.gtls_fold_sort(w.lc.t, w.periods[:4], want_phase=False)
+    _, pm_o = oracle.fold_sort(w.lc.t, w.periods[:4], want_phase=False)
+    assert np.array_equal(perm, pm_o)
+
+
+def test_search_shared_duration_grid_and_small_tiles(tmpl512):
+    _cuda()
+    w = gi.make_workload(1).subset(61)
+    qs = np.array([0.004, 0.004001, 0.01, 0.03, 0.1, 0.5])        # duplicates D, and q = 0.5
+    ora = oracle.search(w.lc.t, w.lc.y, w.lc.dy, w.periods, qs, tmpl512, dt0=0.05)
+    for tile in (0, 1, 7):
+        res = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, qs, tmpl512, dt0=0.05,
+                            sde_kernel=3, period_tile=tile)
+        _check_search(w, res, ora, sde_kernel=3, label=f"shared/tile{tile}")
+
+
+def test_search_device_pointers_and_workspace():
+    torch = _cuda()
+    w = gi.make_workload(2).subset(301)
+    host = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    ws = torch.empty(g.gtls_workspace_bytes(w.lc.n, w.n_per, w.n_dur), dtype=torch.uint8, device="cuda")
+    res = g.gtls_search(dev(w.lc.t), dev(w.lc.y), dev(w.lc.dy), dev(w.periods), dev(w.durations),
+                        dev(w.tmpl), workspace=ws)
+    assert np.array_equal(res.chi2.cpu().numpy(), host.chi2)          # same kernels, same bits
+    assert np.array_equal(res.best(), host.best())
+    assert np.array_equal(res.sde.cpu().numpy(), host.sde)
+    assert res.summary == host.summary
+
+
+def test_tiny_and_degenerate_inputs(tmpl512):
+    _cuda()
+    rng = np.random.default_rng(3)
+    for n in (3, 4, 9, 40):
+        t = np.sort(rng.uniform(0, 10, n)); y = 1 + rng.normal(0, 1e-3, n); dy = np.full(n, 1e-3)
+        per = np.array([1.1, 2.7, 4.9]); qs = np.array([0.1, 0.3, 0.5])
+        ora = oracle.search(t, y, dy, per, qs, tmpl512, dt0=0.0)
+        res = g.gtls_search(t, y, dy, per, qs, tmpl512, dt0=0.0, sde_kernel=3)
+        assert np.allclose(res.chi2, ora.chi2, rtol=CHI2_RTOL, atol=0), n
+        b = res.best()
+        assert np.array_equal(b["dur_idx"], ora.best["dur_idx"]) and np.array_equal(b["start"], ora.best["start"])
+    # flat curve: chi2 == 0 everywhere -> GTLS_EDEGENERATE, chi2 outputs valid, SDE zero (G22)
+    t = np.linspace(0, 10, 40)
+    res = g.gtls_search(t, np.ones(40), np.full(40, 1e-3), np.array([1.1, 2.2]), np.array([0.1, 0.2]), tmpl512)
+    assert res.code == -6 and np.all(res.chi2 == 0) and np.all(res.sde == 0) and np.all(res.sde_raw == 0)
+    b = res.best()
+    assert np.all(b["dur_idx"] == 0) and np.all(b["start"] == 0)
+    # brightening-only curve: every window scores chi2_0 exactly (G7)
+    y = 1.0 + np.abs(rng.normal(0, 1e-3, 40))
+    res = g.gtls_search(t, y, np.full(40, 1e-3), np.array([1.7]), np.array([0.1, 0.3]), tmpl512, dt0=0.0)
+    assert res.chi2[0] == res.summary["chi2_null"] and res.best()["depth"][0] == 0.0
+
+
+def test_input_validation_on_device(tmpl512):
+    _cuda()
+    t = np.linspace(0, 10, 50); y = np.ones(50); y[3] = 0.999; dy = np.full(50, 1e-3)
+    per = np.array([1.0, 2.0]); qs = np.array([0.1])
+    bad = y.copy(); bad[7] = np.nan
+    with pytest.raises(g.GtlsError) as e:
+        g.gtls_search(t, bad, dy, per, qs, tmpl512)
+    assert e.value.code == -2
+    bad = dy.copy(); bad[0] = 0.0
+    with pytest.raises(g.GtlsError) as e:
+        g.gtls_search(t, y, bad, per, qs, tmpl512)
+    assert e.value.code == -2
+    with pytest.raises(g.GtlsError) as e:
+        g.gtls_search(t, y, dy, np.array([1.0, -2.0]), qs, tmpl512)
+    assert e.value.code == -3
+    with pytest.raises(g.GtlsError) as e:
+        g.gtls_search(t, y, dy, per, np.array([0.7]), tmpl512)
+    assert e.value.code == -3
+
+
+# ------------------------------------------------------------------------- a9 alone
+@pytest.mark.parametrize("kernel,n", [(151, 10483), (31, 200), (151, 60), (1, 50), (0, 50), (1001, 3000)])
+def test_sde_epilogue_matches_oracle(kernel, n):
+    _cuda()
+    rng = np.random.default_rng(kernel + n)
+    chi2 = 4000.0 + np.cumsum(rng.normal(0, 0.2, n)) + rng.normal(0, 1, n)
+    chi2[n // 3] -= 40.0
+    raw, sde, summ, code = g.gtls_sde(chi2, sde_kernel=kernel)
+    s = oracle.sde(chi2, kernel)
+    assert code == 0
+    assert np.abs(raw - s.sde_raw).max() <= 1e-9 and np.abs(sde - s.sde).max() <= 1e-9
+    assert summ["best_period_idx"] == s.best_period_idx and summ["sde_argmax"] == s.sde_argmax
+    assert abs(summ["sde_max"] - s.sde.max()) <= 1e-9
