@@ -1,0 +1,329 @@
+#!/usr/bin/env python
+"""Benchmark of the TLS period-search hot path (libgtls, sm_100a) -- one JSON line on stdout.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c1..c4] [--impl reference]
+
+A "step" is one pass of the whole hot path (fold, sort, pad + scans, per-window chi2, argmin,
+SR/SDE) over one synthetic light curve.  Metric: (period x duration) trials per second
+(BASELINE.json), plus seconds per light curve.  `value` is measured with all inputs resident in
+HBM; `e2e` is the same metric through the C ABI with host buffers (H2D + D2H inside the timed
+region).  `roofline` describes the dominant kernel (the in-transit chi2 kernel, fp64 ALU bound);
+`cpu_baseline` is the CPU oracle timed on a bounded sample of the same workload.
+
+For N > 1 (torchrun, one rank per GPU) every rank searches its own light curve of the same
+shape (independent problems, weak scaling, no data-path collective); time is the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import gtls_inputs as gi  # noqa: E402
+
+METRIC = "TLS (period x duration) trials/sec"
+UNIT = "trials/s"
+SM_COUNT = 148
+DFMA_PER_CLK_PER_SM = 64            # fp64 FMA lanes per SM (B200_PROFILING.md / B300_MICROARCH.md unit counts)
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return json.load(open(p)), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.idx = gpu_index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.idx}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2])); pw.append(float(f[3]))
+            except ValueError:
+                continue
+            for name, v in zip(names, f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        load = [s for s, p in zip(sm, pw) if p > 0.5 * max(pw)] or sm
+        return {"sm_mhz": float(np.median(load)), "sm_max_mhz": float(max(mx)),
+                "power_w_max": float(max(pw)), "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def build_workload(name: str, curve: int = 0):
+    cfg = int(name[1])
+    return gi.make_workload(cfg, curve=curve)
+
+
+def oracle_sample(w, target_s: float):
+    """Deterministic period subset sized so the oracle runs for about target_s seconds."""
+    import oracle
+    cores = oracle.num_threads()
+    # ~1.2e-8 s per window-point per core measured for the plain oracle; refine with a probe
+    probe = w.subset(max(1, w.n_per // 64))
+    t0 = time.perf_counter()
+    r = oracle.search(probe.lc.t, probe.lc.y, probe.lc.dy, probe.periods, probe.durations, probe.tmpl,
+                      dt0=w.dt0)
+    dt = time.perf_counter() - t0
+    per_period = dt / probe.n_per
+    want = int(max(8, min(w.n_per, target_s / max(per_period, 1e-9))))
+    every = max(1, w.n_per // want)
+    return w.subset(every), cores, every
+
+
+def run_reference(args, w):
+    """--impl reference: the CPU oracle, as it stands, on a bounded sample per step."""
+    import oracle
+    sample, cores, every = oracle_sample(w, args.ref_seconds)
+    times = []
+    for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        r = oracle.search(sample.lc.t, sample.lc.y, sample.lc.dy, sample.periods, sample.durations,
+                          sample.tmpl, dt0=w.dt0)
+        oracle.sde(r.chi2, 151)
+        if i >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    ms = 1e3 * float(np.mean(times))
+    value = sample.trials / (ms / 1e3)
+    desc = f"every {every}th period of {w.name} ({sample.n_per} of {w.n_per} periods, all {w.n_dur} durations)"
+    return {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_desc(w), "sample": desc, "dt0": w.dt0},
+        "s_per_light_curve_extrapolated": w.trials / value,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+
+
+def workload_desc(w) -> str:
+    return (f"{w.name}: {w.lc.n} points, {w.n_per} periods (Ofir grid, OS=3), {w.n_dur} durations/period, "
+            f"dt0={w.dt0}, template 512 nodes")
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default=os.environ.get("GTLS_BENCH_WORKLOAD", "c4"))
+    ap.add_argument("--impl", default="gtls", choices=["gtls", "reference"])
+    ap.add_argument("--ref-seconds", type=float, default=20.0, help="CPU seconds per oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--period-tile", type=int, default=0)
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        w = build_workload(args.workload)
+        print(json.dumps(run_reference(args, w)), flush=True)
+        return 0
+
+    import torch
+    import torch.distributed as dist
+    import paper_2607_00348_b200 as g
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    devname = f"cuda:{local_rank}"
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(devname))
+    g.load_library()
+
+    # every rank searches its own curve of the same shape (independent problems)
+    w = build_workload(args.workload, curve=rank)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(devname)
+    d_in = [dev(x) for x in (w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl)]
+    ws = torch.empty(g.gtls_workspace_bytes(w.lc.n, w.n_per, w.n_dur, args.period_tile), dtype=torch.uint8,
+                     device=devname)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=devname)     # > 126 MB L2
+
+    def step(stats=False):
+        return g.gtls_search(*d_in, dt0=w.dt0, sde_kernel=151, workspace=ws, stats=stats,
+                             period_tile=args.period_tile)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        res = step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    st_acc = {}
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        flush.zero_()                                   # L2 flush between timed iterations
+        res = step(stats=True)
+        for k, v in res.stats.items():
+            st_acc[k] = st_acc.get(k, 0) + v if k.startswith("ms_") or k.endswith("launches") else v
+    ev1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms_total = ev0.elapsed_time(ev1)
+    if world > 1:
+        tt = torch.tensor([ms_total], dtype=torch.float64, device=devname)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms_total = float(tt.item())
+    ms_step = ms_total / args.steps
+    value = world * w.trials / (ms_step / 1e3)
+
+    out = None
+    if rank == 0:
+        peaks, peak_src = measured_peaks()
+        # ---- roofline of the dominant kernel (in-transit chi2, fp64 FMA pipe) -------------------
+        chi2_ms_per_launch = st_acc["ms_chi2"] / max(1, st_acc["chi2_launches"])
+        flop_per_wp = 2.0 if st_acc["uniform_dy"] else 4.0          # 1 or 2 DFMA per window point
+        flops_per_launch = st_acc["window_points"] * flop_per_wp / max(1, st_acc["chi2_launches"] / args.steps)
+        achieved = flops_per_launch / (chi2_ms_per_launch * 1e-3) / 1e12
+        sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+        peak = SM_COUNT * DFMA_PER_CLK_PER_SM * 2 * sm_max * 1e6 / 1e12
+        roofline = {"bound": "alu", "kernel": "k_chi2 (in-transit chi2, a5-a8)", "achieved": achieved,
+                    "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                    "peak_source": f"derived: {SM_COUNT} SMs x {DFMA_PER_CLK_PER_SM} DFMA/clk x 2 flop x "
+                                   f"{sm_max:.0f} MHz ({peak_src} sm_max_mhz); DFMA microbenchmark on this "
+                                   f"pool: 36.8 TFLOP/s",
+                    "algorithmic_flops_per_launch": flops_per_launch,
+                    "ms_per_launch": chi2_ms_per_launch,
+                    "share_of_step": st_acc["ms_chi2"] / max(1e-9, st_acc["ms_total"])}
+        stages = {k: st_acc[k] / args.steps for k in st_acc if k.startswith("ms_")}
+        hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+        pp = float(st_acc["period_points"])
+        stage_roof = {
+            "fold_GBps": pp * 12 / (stages["ms_fold"] * 1e-3) / 1e9 if stages["ms_fold"] else None,
+            "sort_GBps": pp * 16 * 4 / (stages["ms_sort"] * 1e-3) / 1e9 if stages["ms_sort"] else None,
+            "scan_GBps": pp * (8 + 16 * (1 if st_acc["uniform_dy"] else 2)) / (stages["ms_scan"] * 1e-3) / 1e9
+            if stages["ms_scan"] else None,
+            "hbm_peak_GBps": hbm_peak, "peak_source": peak_src,
+        }
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_desc(w), "l2_flush": "256 MiB memset between timed steps",
+                       "period_tile": st_acc["period_tile"], "path": st_acc["path"],
+                       "uniform_dy": st_acc["uniform_dy"],
+                       "multi_gpu": "one independent light curve per rank, no collective"},
+            "s_per_light_curve": ms_step / 1e3,
+            "clocks": clocks,
+            "gpu_launches": int(st_acc["kernel_launches"]),
+            "stage_ms_per_step": stages, "stage_bandwidth": stage_roof,
+            "roofline": roofline,
+            "summary": res.summary,
+            "paper_context": {"gtls_rtx4090_s": 138.0, "tls_cpu_7950x_s": 3289.0,
+                              "note": "PAPER.md:411, 3000-d curve, other hardware: context only"},
+        }
+
+    # ---- e2e: host buffers through the C ABI, H2D + D2H inside the timed region ------------------
+    if not args.no_e2e:
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+        h_in = [pin(x) for x in (w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl)]
+        del ws
+        torch.cuda.empty_cache()
+        barrier()
+        n_e2e = max(1, min(2, args.steps))
+        g.gtls_search(*h_in, dt0=w.dt0, sde_kernel=151)          # warm-up (allocations)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            r2 = g.gtls_search(*h_in, dt0=w.dt0, sde_kernel=151)
+        torch.cuda.synchronize()
+        dt = (time.perf_counter() - t0) / n_e2e
+        if world > 1:
+            tt = torch.tensor([dt], dtype=torch.float64, device=devname)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            dt = float(tt.item())
+        if rank == 0:
+            h2d = int(sum(x.nbytes for x in h_in))
+            d2h = int(w.n_per * (8 * 3 + 24))
+            out["e2e"] = {"value": world * w.trials / dt, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                          "d2h_bytes_per_step": d2h, "ms_per_step": dt * 1e3, "steps": n_e2e,
+                          "note": "gtls_search with host pointers: cudaMalloc + H2D + search + D2H per call"}
+
+    if rank == 0:
+        if not args.no_cpu_baseline:
+            import oracle
+            sample, cores, every = oracle_sample(w, args.ref_seconds)
+            t0 = time.perf_counter()
+            ro = oracle.search(sample.lc.t, sample.lc.y, sample.lc.dy, sample.periods, sample.durations,
+                               sample.tmpl, dt0=w.dt0)
+            dt = time.perf_counter() - t0
+            out["cpu_baseline"] = {
+                "value": sample.trials / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                "sample": f"every {every}th period of {w.name} ({sample.n_per} of {w.n_per} periods), {dt:.1f} s",
+                "s_per_light_curve_extrapolated": w.trials / (sample.trials / dt)}
+            # parity spot check on the sample while we are here (not timed)
+            got = np.asarray(res.chi2.cpu())[::every][:sample.n_per]
+            out["cpu_baseline"]["chi2_max_rel_err_vs_gpu"] = float(np.max(np.abs(got - ro.chi2) / ro.chi2))
+        print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
