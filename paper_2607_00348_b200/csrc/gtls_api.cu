@@ -2,6 +2,7 @@
 // loop and the epilogue.  All arithmetic of the search runs in the kernels of pre.cu,
 // fold_sort.cu, scan.cu, chi2.cu and epilogue.cu; there is no CPU fallback.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -282,6 +283,9 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     }
     if (!a.s1 || (!uniform && !a.s0)) return GTLS_ENOMEM;
 
+    // GTLS_CHI2_KERNEL=v1 selects the simple warp-per-window kernel (debugging / A-B runs)
+    const char* kenv = getenv("GTLS_CHI2_KERNEL");
+    const bool use_v1 = kenv && strcmp(kenv, "v1") == 0;
     // ---- period tiles ----------------------------------------------------------------------
     for (long long p0 = 0; p0 < n_per; p0 += tile) {
         a.p0 = p0;
@@ -296,7 +300,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
         tm.mark(3);
         launch_gather_scan(a, sorted, nullptr, nullptr, -1, st);
         tm.mark(4);
-        launch_chi2(a, st);
+        if (use_v1) launch_chi2(a, st); else launch_chi2_rows(a, st);
         tm.mark(5);
         launch_reduce(a, sorted, d_chi2, d_best, d_counters, st);
         tm.mark(6);

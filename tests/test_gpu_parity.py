@@ -258,3 +258,13 @@ def test_sde_epilogue_matches_oracle(kernel, n):
     assert np.abs(raw - s.sde_raw).max() <= 1e-9 and np.abs(sde - s.sde).max() <= 1e-9
     assert summ["best_period_idx"] == s.best_period_idx and summ["sde_argmax"] == s.sde_argmax
     assert abs(summ["sde_max"] - s.sde.max()) <= 1e-9
+
+
+def test_v1_kernel_still_matches(monkeypatch):
+    """The simple warp-per-window chi2 kernel (GTLS_CHI2_KERNEL=v1) stays a valid A/B path."""
+    _cuda()
+    monkeypatch.setenv("GTLS_CHI2_KERNEL", "v1")
+    w = gi.make_workload(2, hetero=True).subset(257)
+    ora = oracle.search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05)
+    res = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05, sde_kernel=5)
+    _check_search(w, res, ora, sde_kernel=5, label="v1")
