@@ -26,7 +26,8 @@ namespace {
 constexpr int kA = 15;                    // windows per thread
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
-constexpr int kSmemDoubles = 13824;       // 110.6 KB dynamic shared memory -> 2 CTAs per SM
+constexpr int kSmemDoubles = 12800;       // 102.4 KB dynamic + 8 KB template -> 2 CTAs per SM
+constexpr int kTmplSmem = 1024;           // template nodes cached in shared memory
 constexpr int kMaxColsT = 64;             // columns staged per stage (WC * cw)
 
 struct Geom {
@@ -49,8 +50,7 @@ __device__ __forceinline__ void cand_offer(Cand& b, double d, int s, double dept
     if (!b.has || d < b.d || (d == b.d && s < b.s)) { b.d = d; b.s = s; b.depth = depth; b.has = 1; }
 }
 
-__device__ __forceinline__ void cp_async8(double* dst_smem, const double* src, bool valid) {
-    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+__device__ __forceinline__ void cp_async8(unsigned d, const double* src, bool valid) {
     const int sz = valid ? 8 : 0;
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(d), "l"(src), "r"(sz));
 }
@@ -127,10 +127,11 @@ __device__ __forceinline__ void rows_fma(const double* __restrict__ xs, int pitc
                                          const double* __restrict__ gs, int gp, double (&acc)[kA]) {
     double g[MB];
 #pragma unroll
-    for (int m = 0; m < MB; ++m) g[m] = gs[m * gp];
+    for (int m = 0; m < MB; ++m) { g[m] = *gs; gs += gp; }
 #pragma unroll
     for (int gam = 0; gam < kA + MB - 1; ++gam) {
-        const double x = xs[gam * pitch];
+        const double x = *xs;
+        xs += pitch;
 #pragma unroll
         for (int al = 0; al < kA; ++al) {
             const int m = gam - al;
@@ -148,6 +149,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_chi2_rows(TileArgs a) {
     extern __shared__ double smem[];
     __shared__ Geom s_q;
     __shared__ Cand s_best[kWarps];
+    __shared__ double s_tmpl[kTmplSmem];
 
     const int jd = blockIdx.x, pl = blockIdx.y;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -158,9 +160,16 @@ __global__ void __launch_bounds__(kThreads, 2) k_chi2_rows(TileArgs a) {
         return;
     }
     if (tid == 0) make_geom(s_q, a.n, e.D, e.stride, a.n_tmpl, UNIFORM);
+    const bool tmpl_in_smem = a.n_tmpl <= kTmplSmem;
+    if (tmpl_in_smem) for (int k = tid; k < a.n_tmpl; k += kThreads) s_tmpl[k] = a.tmpl[k];
+    const double* __restrict__ tm = tmpl_in_smem ? s_tmpl : a.tmpl;
     __syncthreads();
     const Geom& q = s_q;
-    const int D = q.D, st = q.st;
+    // fields used inside loops are copied to registers (shared memory would be re-read after
+    // every barrier); the rest is read from s_q once per stage
+    const int D = q.D, st = q.st, g_pitch = q.pitch, g_colsT = q.colsT, g_rows = q.rows,
+              g_MB = q.MB, g_cw = q.cw, g_WC = q.WC, g_nc = q.nc;
+    const double g_tscale = q.tscale;
     const double* __restrict__ x1 = a.x1 + (long long)pl * a.pitch;
     const double* __restrict__ x0 = a.x0 + (long long)pl * a.pitch;
     const double* __restrict__ s1 = a.s1 + (long long)pl * a.spitch;
@@ -173,6 +182,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_chi2_rows(TileArgs a) {
     const int ld_r0 = tid / q.colsT, ld_col = tid - ld_r0 * q.colsT;
     const int ld_wc = ld_col / q.cw, ld_c = ld_col - ld_wc * q.cw;
     const bool ld_on = ld_r0 < ld_rpp;
+    const int ld_iters = ld_on ? (g_rows - ld_r0 + ld_rpp - 1) / ld_rpp : 0;   // rows this thread copies
     // compute role: warp -> (wr, wc), lane -> (g, c)
     const int wr = warp / q.WC, wc = warp - wr * q.WC;
     const int lg = lane / q.cw, lc = lane - lg * q.cw;
@@ -183,34 +193,43 @@ __global__ void __launch_bounds__(kThreads, 2) k_chi2_rows(TileArgs a) {
         double* XS = smem + q.xs_off[buf];
         double* GS = smem + q.gs_off[buf];
         const double* __restrict__ src = (UNIFORM || pass == 0) ? x1 : x0;
-        const long long row0 = (long long)rt * q.RT + (long long)mb * q.MB;
+        const long long row0 = (long long)rt * q.RT + (long long)mb * g_MB;
         if (ld_on) {
-            const int cc = ccs * q.WC + ld_wc;
-            const int i = cc * q.cw + ld_c;
-            const bool colv = cc < q.nc && i < st;
-            for (int r = ld_r0; r < q.rows; r += ld_rpp) {
-                const long long ee = (row0 + r) * st + i;
-                const bool v = colv && ee < lim;
-                cp_async8(XS + r * q.pitch + ld_col, src + (v ? ee : 0), v);
+            const int cc = ccs * g_WC + ld_wc;
+            const int i = cc * g_cw + ld_c;
+            const bool colv = cc < g_nc && i < st;
+            const long long ee = (row0 + ld_r0) * st + i;
+            const long long estep = (long long)ld_rpp * st;
+            const double* sp = src + ee;
+            unsigned dst = (unsigned)__cvta_generic_to_shared(XS + ld_r0 * g_pitch + ld_col);
+            const unsigned dstep = (unsigned)(ld_rpp * g_pitch * 8);
+            // rows of this thread's column that lie inside the curve come first, then zero fill
+            int nvalid = 0;
+            if (colv && ee < lim) {
+                const long long nv = (lim - ee + estep - 1) / estep;
+                nvalid = nv > ld_iters ? ld_iters : (int)nv;
             }
-        }
-        for (int idx = tid; idx < q.MB * q.colsT; idx += kThreads) {
-            const int m = idx / q.colsT, col = idx - m * q.colsT;
-            const int w2 = col / q.cw, c2 = col - w2 * q.cw;
-            const int cc = ccs * q.WC + w2;
-            const int i = cc * q.cw + c2;
-            const long long j = (long long)(mb * q.MB + m) * st + i;
-            double gv = 0.0;
-            if (cc < q.nc && i < st && j < D) {
-                const double u = ((double)j + 0.5) * q.tscale;
-                int k = (int)floor(u);
-                k = k > a.n_tmpl - 2 ? a.n_tmpl - 2 : k;
-                const double fr = u - (double)k;
-                const double t0 = a.tmpl[k];
-                gv = t0 + fr * (a.tmpl[k + 1] - t0);
-                if (!UNIFORM && pass == 1) gv *= gv;
+            int k = 0;
+            for (; k < nvalid; ++k) { cp_async8(dst, sp, true); sp += estep; dst += dstep; }
+            for (; k < ld_iters; ++k) { cp_async8(dst, src, false); dst += dstep; }
+            // template values of the same column, rows m = ld_r0, ld_r0 + ld_rpp, ...
+            double* gd = GS + ld_r0 * g_colsT + ld_col;
+            const int gstep = ld_rpp * g_colsT;
+            long long j = (long long)(mb * g_MB + ld_r0) * st + i;
+            for (int m = ld_r0; m < g_MB; m += ld_rpp) {
+                double gv = 0.0;
+                if (colv && j < D) {
+                    const double u = ((double)(int)j + 0.5) * g_tscale;
+                    int kk = (int)u;                       // u >= 0: truncation == floor
+                    kk = kk > a.n_tmpl - 2 ? a.n_tmpl - 2 : kk;
+                    const double fr = u - (double)kk;
+                    const double t0 = tm[kk];
+                    gv = t0 + fr * (tm[kk + 1] - t0);
+                    if (!UNIFORM && pass == 1) gv *= gv;
+                }
+                *gd = gv;
+                gd += gstep; j += estep;
             }
-            GS[idx] = gv;
         }
         cp_async_commit();
     };
@@ -231,24 +250,23 @@ __global__ void __launch_bounds__(kThreads, 2) k_chi2_rows(TileArgs a) {
 
     for (int s = 0; s < S; ++s) {
         const int buf = s & 1;
-        if (s + 1 < S) {
+        // stage s has landed for every thread; everyone is also done reading the other buffer
+        cp_async_wait<0>();
+        __syncthreads();
+        if (s + 1 < S) {      // staging of stage s+1 overlaps the FMAs of stage s (no barrier between)
             issue_stage(n_rt, n_pass, n_ccs, n_mb, buf ^ 1);
             advance(n_rt, n_pass, n_ccs, n_mb);
-            cp_async_wait<1>();
-        } else {
-            cp_async_wait<0>();
         }
-        __syncthreads();
         if (c_ccs == 0 && c_mb == 0) {
 #pragma unroll
             for (int al = 0; al < kA; ++al) acc[al] = 0.0;
         }
         if (cmp_on) {
-            const double* xs = smem + q.xs_off[buf] + (grp * kA) * q.pitch + wc * q.cw + lc;
-            const double* gs = smem + q.gs_off[buf] + wc * q.cw + lc;
-            if (q.MB == 21) rows_fma<21>(xs, q.pitch, gs, q.colsT, acc);
-            else if (q.MB == 14) rows_fma<14>(xs, q.pitch, gs, q.colsT, acc);
-            else rows_fma<7>(xs, q.pitch, gs, q.colsT, acc);
+            const double* xs = smem + q.xs_off[buf] + (grp * kA) * g_pitch + wc * g_cw + lc;
+            const double* gs = smem + q.gs_off[buf] + wc * g_cw + lc;
+            if (g_MB == 21) rows_fma<21>(xs, g_pitch, gs, g_colsT, acc);
+            else if (g_MB == 14) rows_fma<14>(xs, g_pitch, gs, g_colsT, acc);
+            else rows_fma<7>(xs, g_pitch, gs, g_colsT, acc);
         }
         const bool end_pass = (c_ccs == q.nccs - 1) && (c_mb == q.nmb - 1);
         if (end_pass) {
@@ -258,7 +276,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_chi2_rows(TileArgs a) {
 #pragma unroll
                 for (int al = 0; al < kA; ++al) {
                     const double v = __shfl_down_sync(0xffffffffu, acc[al], off);
-                    if (lc + off < q.cw && lane + off < 32) acc[al] += v;
+                    if (lc + off < g_cw) acc[al] += v;
                 }
             }
             if (cmp_on && lc == 0) {
@@ -288,8 +306,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_chi2_rows(TileArgs a) {
                 }
             }
         }
-        __syncthreads();
-        advance(c_rt, c_pass, c_ccs, c_mb);
+        advance(c_rt, c_pass, c_ccs, c_mb);      // the barrier at the top of the next stage orders buffer reuse
     }
 
     // CTA-wide lexicographic min on (d, s)
