@@ -100,9 +100,10 @@ class ClockSampler:
                 "power_w_max": float(max(pw)), "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def build_workload(name: str, curve: int = 0):
+def build_workload(name: str, curve: int = 0, every: int = 1):
     cfg = int(name[1])
-    return gi.make_workload(cfg, curve=curve)
+    w = gi.make_workload(cfg, curve=curve)
+    return w.subset(every) if every > 1 else w
 
 
 def oracle_sample(w, target_s: float):
@@ -164,6 +165,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--period-tile", type=int, default=0)
+    ap.add_argument("--every", type=int, default=1,
+                    help="profiling aid: search only every k-th period of the workload (default 1 = the "
+                         "full workload; any other value is named in config.workload)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -173,7 +177,7 @@ def main():
     if args.impl == "reference":
         if rank != 0:
             return 0
-        w = build_workload(args.workload)
+        w = build_workload(args.workload, every=args.every)
         print(json.dumps(run_reference(args, w)), flush=True)
         return 0
 
@@ -190,7 +194,7 @@ def main():
     g.load_library()
 
     # every rank searches its own curve of the same shape (independent problems)
-    w = build_workload(args.workload, curve=rank)
+    w = build_workload(args.workload, curve=rank, every=args.every)
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(devname)
     d_in = [dev(x) for x in (w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl)]
     ws = torch.empty(g.gtls_workspace_bytes(w.lc.n, w.n_per, w.n_dur, args.period_tile), dtype=torch.uint8,
