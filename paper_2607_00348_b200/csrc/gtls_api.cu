@@ -283,9 +283,10 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     }
     if (!a.s1 || (!uniform && !a.s0)) return GTLS_ENOMEM;
 
-    // GTLS_CHI2_KERNEL=v1 selects the simple warp-per-window kernel (debugging / A-B runs)
+    // GTLS_CHI2_KERNEL=v1 / rows select the older chi2 kernels (debugging / A-B runs)
     const char* kenv = getenv("GTLS_CHI2_KERNEL");
     const bool use_v1 = kenv && strcmp(kenv, "v1") == 0;
+    const bool use_rows = kenv && strcmp(kenv, "rows") == 0;
     // ---- period tiles ----------------------------------------------------------------------
     for (long long p0 = 0; p0 < n_per; p0 += tile) {
         a.p0 = p0;
@@ -300,7 +301,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
         tm.mark(3);
         launch_gather_scan(a, sorted, nullptr, nullptr, -1, st);
         tm.mark(4);
-        if (use_v1) launch_chi2(a, st); else launch_chi2_rows(a, st);
+        if (use_v1) launch_chi2(a, st); else if (use_rows) launch_chi2_rows(a, st); else launch_chi2_ring(a, st);
         tm.mark(5);
         launch_reduce(a, sorted, d_chi2, d_best, d_counters, st);
         tm.mark(6);

@@ -127,7 +127,8 @@ u64* launch_phase_sort(const TileArgs& a, cudaStream_t st, int* n_launches);
 void launch_gather_scan(const TileArgs& a, const u64* sorted, double* x2, double* s2,
                         int pad_override, cudaStream_t st);
 void launch_chi2(const TileArgs& a, cudaStream_t st);        // v1: warp per window (fallback / A-B)
-void launch_chi2_rows(const TileArgs& a, cudaStream_t st);   // register-tiled rows kernel
+void launch_chi2_rows(const TileArgs& a, cudaStream_t st);   // register-tiled rows kernel (A-B)
+void launch_chi2_ring(const TileArgs& a, cudaStream_t st);   // register-ring correlation kernel (default)
 // counters[0] += windows of all trials, counters[1] += sum of D over evaluated windows
 void launch_reduce(const TileArgs& a, const u64* sorted, double* out_chi2, gtls_best* out_best,
                    unsigned long long* counters, cudaStream_t st);
