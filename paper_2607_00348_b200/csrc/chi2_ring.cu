@@ -32,8 +32,6 @@ namespace {
 
 constexpr int kRT = 128;                 // threads per CTA
 constexpr int kRW = kRT / 32;            // warps per CTA
-constexpr int kPartPitch = 33;           // doubles per slot row of the per-warp emit buffer
-constexpr int kMBMax = 21;
 constexpr int kCDoubles = 5120;          // Cpart capacity (40 KB)
 constexpr int kTmplSmem = 1024;          // template nodes cached in shared memory
 constexpr int kMaxSeg = 512;
@@ -62,71 +60,111 @@ __device__ __forceinline__ void pick_mb(int M, int& MB, int& nmb) {
     }
 }
 
-struct Item {                            // one warp work item: 32 flat (segment, column) slots
-    int f0;                              // first flat slot
-    int seg_first, ng;                   // segments touched by this warp
-    int idx;                             // item index (= f0 / 32)
+constexpr int kPartPitch = 33;           // doubles per slot row of the per-warp emit buffer
+constexpr int kMBMax = 21;
+
+// rows prefetched ahead of the FMAs (divides MB)
+template <int MB> struct PfRows { static constexpr int v = (MB % 7 == 0) ? 7 : (MB >= 8 ? MB / 2 : MB); };
+
+__device__ __forceinline__ double lds64(const unsigned addr) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void sts64(const unsigned addr, const double v) {
+    asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory");
+}
+
+struct EmitCtx {                         // where completed window sums of one item go
+    int idx, f0, seg_first, ng;          // item index, first flat slot, segments touched by the warp
+    int slots, st, L, nWt, Kt;
+    bool first;                          // first tap block: store, else accumulate
+    double* cpart;
+    unsigned part;                       // shared-space address of the per-warp [MB][kPartPitch] buffer
 };
 
+__device__ __forceinline__ void cpart_put(const EmitCtx& c, const int seg, const int kw, const double sum) {
+    const int w = seg * c.L + kw;
+    if (kw >= 0 && kw < c.L && w < c.nWt) {
+        const int j = c.idx - ((seg * c.st) >> 5);
+        double* dst = c.cpart + j * c.Kt + w;
+        *dst = c.first ? sum : *dst + sum;
+    }
+}
+
+// The MB completed window sums of every lane sit in part[slot][lane]; sum them over the lanes of
+// each segment in fixed order.  One segment per warp (the common case): lane = slot, 32 loads in
+// four independent chains.  Otherwise: one (segment, slot) task per lane and round.
+template <int MB>
+__device__ __forceinline__ void reduce_block(const EmitCtx& c, const int kw0, const int lane) {
+    __syncwarp();
+    if (c.ng == 1) {
+        if (lane < MB) {
+            const unsigned pr = c.part + (unsigned)(lane * kPartPitch * 8);
+            double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+#pragma unroll
+            for (int q = 0; q < 32; q += 4) {
+                s0 += lds64(pr + 8 * q);
+                s1 += lds64(pr + 8 * q + 8);
+                s2 += lds64(pr + 8 * q + 16);
+                s3 += lds64(pr + 8 * q + 24);
+            }
+            cpart_put(c, c.seg_first, kw0 + lane, (s0 + s1) + (s2 + s3));
+        }
+    } else {
+        for (int t = lane; t < c.ng * MB; t += 32) {
+            const int gi = t / MB, sl = t - gi * MB;
+            const int seg = c.seg_first + gi;
+            int lo = seg * c.st - c.f0, hi = lo + c.st;
+            lo = lo < 0 ? 0 : lo;
+            hi = hi > 32 ? 32 : hi;
+            hi = hi > c.slots - c.f0 ? c.slots - c.f0 : hi;
+            const unsigned pr = c.part + (unsigned)(sl * kPartPitch * 8);
+            double s0 = 0.0, s1 = 0.0;
+            int q = lo;
+            for (; q + 1 < hi; q += 2) { s0 += lds64(pr + 8 * q); s1 += lds64(pr + 8 * q + 8); }
+            if (q < hi) s0 += lds64(pr + 8 * q);
+            cpart_put(c, seg, kw0 + sl, s0 + s1);
+        }
+    }
+    __syncwarp();
+}
+
 // One tap block of one item: march `nblk` blocks of MB rows.  `xp` points at this lane's X value of
-// the first row, rows >= rows_valid read as 0.  After each block the MB completed window sums of
-// every lane sit in `part` (slot-major); the warp reduces them over the lanes of each segment and
-// stores / accumulates into cpart[j * Kt + window].
+// the first row; rows >= rows_valid read as 0.  PF rows are in flight ahead of the FMAs; after every
+// block of MB rows the MB completed window sums are reduced over the lanes of each segment.
 template <int MB>
 __device__ __forceinline__ void march(const double* __restrict__ xp, const int st, const int rows_valid,
-                                      const int nblk, const double (&T)[MB], double* __restrict__ part,
-                                      const int lane, const Item it, const int slots, const int L,
-                                      const int nWt, const int Kt, double* __restrict__ cpart,
-                                      const bool first) {
-    double acc[MB], xc[MB], xn[MB];
+                                      const int nblk, const double (&T)[MB], const int lane,
+                                      const EmitCtx& c) {
+    constexpr int PF = PfRows<MB>::v;
+    double acc[MB], xr[PF];
 #pragma unroll
-    for (int u = 0; u < MB; ++u) {
-        acc[u] = 0.0;
-        xn[u] = u < rows_valid ? __ldg(xp) : 0.0;
+    for (int u = 0; u < MB; ++u) acc[u] = 0.0;
+#pragma unroll
+    for (int u = 0; u < PF; ++u) {
+        xr[u] = u < rows_valid ? __ldg(xp) : 0.0;
         xp += st;
     }
-    double* const pl = part + lane;
+    int row_pf = PF;                               // row index the next prefetch belongs to
+    const unsigned pl = c.part + (unsigned)(lane * 8);
+#pragma unroll 1
     for (int blk = 0; blk < nblk; ++blk) {
-        const int gnext = (blk + 1) * MB;
 #pragma unroll
         for (int u = 0; u < MB; ++u) {
-            xc[u] = xn[u];
-            xn[u] = (blk + 1 < nblk && gnext + u < rows_valid) ? __ldg(xp) : 0.0;   // next block, in flight
+            const double x = xr[u % PF];
+            xr[u % PF] = row_pf < rows_valid ? __ldg(xp) : 0.0;
             xp += st;
-        }
-#pragma unroll
-        for (int u = 0; u < MB; ++u) {
+            ++row_pf;
 #pragma unroll
             for (int m = 0; m < MB; ++m) {
                 const int a = (u - m + MB) % MB;
-                if (m == 0) acc[a] = T[0] * xc[u];                  // window gamma starts at this row
-                else acc[a] = fma(T[m], xc[u], acc[a]);
+                if (m == 0) acc[a] = T[0] * x;                      // window gamma starts at this row
+                else acc[a] = fma(T[m], x, acc[a]);
             }
-            pl[u * kPartPitch] = acc[(u + 1) % MB];                 // window gamma - (MB-1) is complete
+            sts64(pl + (unsigned)(u * kPartPitch * 8), acc[(u + 1) % MB]);   // window gamma-(MB-1) complete
         }
-        __syncwarp();
-        for (int t = lane; t < it.ng * MB; t += 32) {
-            const int gi = t / MB, slot = t - gi * MB;
-            const int seg = it.seg_first + gi;
-            const int kw = blk * MB + slot - (MB - 1);
-            const int w = seg * L + kw;
-            if (kw >= 0 && kw < L && w < nWt) {
-                int lo = seg * st - it.f0, hi = lo + st;
-                lo = lo < 0 ? 0 : lo;
-                hi = hi > 32 ? 32 : hi;
-                hi = hi > slots - it.f0 ? slots - it.f0 : hi;
-                const double* pr = part + slot * kPartPitch;
-                double s0 = 0.0, s1 = 0.0;
-                int q = lo;
-                for (; q + 1 < hi; q += 2) { s0 += pr[q]; s1 += pr[q + 1]; }
-                if (q < hi) s0 += pr[q];
-                const double sum = s0 + s1;
-                const int j = it.idx - ((seg * st) >> 5);
-                double* dst = cpart + j * Kt + w;
-                *dst = first ? sum : *dst + sum;
-            }
-        }
-        __syncwarp();
+        reduce_block<MB>(c, blk * MB - (MB - 1), lane);
     }
 }
 
@@ -141,11 +179,16 @@ __device__ __forceinline__ double tmpl_lerp(const double* __restrict__ tm, int n
 
 template <int MB>
 __device__ __forceinline__ void run_item(const TileArgs& a, const RGeom& q, const double* __restrict__ tm,
-                                         const double* __restrict__ x, const bool square,
-                                         const Item it, const int lane, const int slots, const int L,
-                                         const int nWt, const int k0, double* __restrict__ part,
-                                         double* __restrict__ cpart) {
-    const int f = it.f0 + lane;
+                                         const double* __restrict__ x, const bool square, const int item,
+                                         const int lane, const int slots, const int L, const int nWt,
+                                         const int k0, const unsigned part, double* __restrict__ cpart) {
+    EmitCtx c;
+    c.idx = item; c.f0 = item << 5;
+    c.seg_first = c.f0 / q.st;
+    c.ng = min(c.f0 + 31, slots - 1) / q.st - c.seg_first + 1;
+    c.slots = slots; c.st = q.st; c.L = L; c.nWt = nWt; c.Kt = q.Kt;
+    c.cpart = cpart; c.part = part;
+    const int f = c.f0 + lane;
     const bool active = f < slots;
     const int seg = active ? f / q.st : 0;
     const int col = active ? f - seg * q.st : 0;
@@ -166,13 +209,13 @@ __device__ __forceinline__ void run_item(const TileArgs& a, const RGeom& q, cons
             const long long rv = (lim - ebase + q.st - 1) / q.st;
             rows_valid = rv > (long long)nblk * MB ? nblk * MB : (int)rv;
         }
-        march<MB>(x + (active ? ebase : 0), q.st, rows_valid, nblk, T, part, lane, it, slots, L, nWt,
-                  q.Kt, cpart, b == 0);
+        c.first = b == 0;
+        march<MB>(x + (active ? ebase : 0), q.st, rows_valid, nblk, T, lane, c);
     }
 }
 
 template <bool UNIFORM>
-__global__ void __launch_bounds__(kRT) k_chi2_ring(TileArgs a) {
+__global__ void __launch_bounds__(kRT, 3) k_chi2_ring(TileArgs a) {
     extern __shared__ double dsm[];                 // [kRW][kMBMax*kPartPitch] emit buffers, then Cpart
     __shared__ __align__(16) double s_tmpl[kTmplSmem];
     double* const s_cpart = dsm + kRW * kMBMax * kPartPitch;
@@ -233,7 +276,7 @@ __global__ void __launch_bounds__(kRT) k_chi2_ring(TileArgs a) {
     const double* __restrict__ s1 = a.s1 + (long long)pl * a.spitch;
     const double* __restrict__ s0 = a.s0 + (long long)pl * a.spitch;
     const double G_u = a.w_uniform * e.gg2, sw_u = (double)q.D * a.w_uniform;
-    double* part = dsm + warp * (kMBMax * kPartPitch);
+    const unsigned part = (unsigned)__cvta_generic_to_shared(dsm + warp * (kMBMax * kPartPitch));
     Cand best; best.has = 0; best.d = 0.0; best.s = 0; best.depth = 0.0;
 
     for (int k0 = 0; k0 < q.nW; k0 += q.Kt) {
@@ -266,17 +309,12 @@ __global__ void __launch_bounds__(kRT) k_chi2_ring(TileArgs a) {
             const double* __restrict__ x = pass == 0 ? x1 : x0;
             double* cpart = s_cpart + pass * q.J * q.Kt;
             for (int i = warp; i < items; i += kRW) {
-                Item it;
-                it.idx = i; it.f0 = i << 5;
-                it.seg_first = it.f0 / q.st;
-                const int last = min(it.f0 + 31, slots - 1) / q.st;
-                it.ng = last - it.seg_first + 1;
                 switch (q.MB) {
-                    case 21: run_item<21>(a, q, tm, x, pass == 1, it, lane, slots, L, nWt, k0, part, cpart); break;
-                    case 16: run_item<16>(a, q, tm, x, pass == 1, it, lane, slots, L, nWt, k0, part, cpart); break;
-                    case 12: run_item<12>(a, q, tm, x, pass == 1, it, lane, slots, L, nWt, k0, part, cpart); break;
-                    case 8: run_item<8>(a, q, tm, x, pass == 1, it, lane, slots, L, nWt, k0, part, cpart); break;
-                    default: run_item<4>(a, q, tm, x, pass == 1, it, lane, slots, L, nWt, k0, part, cpart); break;
+                    case 21: run_item<21>(a, q, tm, x, pass == 1, i, lane, slots, L, nWt, k0, part, cpart); break;
+                    case 16: run_item<16>(a, q, tm, x, pass == 1, i, lane, slots, L, nWt, k0, part, cpart); break;
+                    case 12: run_item<12>(a, q, tm, x, pass == 1, i, lane, slots, L, nWt, k0, part, cpart); break;
+                    case 8: run_item<8>(a, q, tm, x, pass == 1, i, lane, slots, L, nWt, k0, part, cpart); break;
+                    default: run_item<4>(a, q, tm, x, pass == 1, i, lane, slots, L, nWt, k0, part, cpart); break;
                 }
             }
         }
