@@ -287,6 +287,8 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     const char* kenv = getenv("GTLS_CHI2_KERNEL");
     const bool use_v1 = kenv && strcmp(kenv, "v1") == 0;
     const bool use_rows = kenv && strcmp(kenv, "rows") == 0;
+    a.dbg_min_st = getenv("GTLS_DBG_MIN_ST") ? atoi(getenv("GTLS_DBG_MIN_ST")) : 0;
+    a.dbg_max_st = getenv("GTLS_DBG_MAX_ST") ? atoi(getenv("GTLS_DBG_MAX_ST")) : 0x7fffffff;
     // ---- period tiles ----------------------------------------------------------------------
     for (long long p0 = 0; p0 < n_per; p0 += tile) {
         a.p0 = p0;

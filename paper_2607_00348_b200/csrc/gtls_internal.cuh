@@ -114,6 +114,7 @@ struct TileArgs {
     double* x1; double* x0;   // [tile*pitch]
     double* s1; double* s0;   // [tile*spitch]
     Partial* partial;      // [tile*n_dur]
+    int dbg_min_st, dbg_max_st;   // timing experiments only (GTLS_DBG_MIN_ST / GTLS_DBG_MAX_ST): skip other trials
 };
 
 void launch_curve_pre(const double* t, const double* y, const double* dy, int n, double* wr,
