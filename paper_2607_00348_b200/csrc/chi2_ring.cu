@@ -7,24 +7,30 @@
 // is, per column i, a 1-D correlation along the rows with the M taps g[m*st+i].
 //
 // A lane owns ONE column and marches down its rows holding MB taps and a ring of MB window
-// accumulators in registers: every X value is loaded from L2 exactly once (coalesced across the
-// lanes of a warp, software-prefetched a few rows ahead) and feeds MB DFMAs; each row step starts
-// one window (DMUL) and completes one.  There is no shared-memory staging of X: the FP64 pipe
-// (64 DFMA/clk/SM) is the only busy resource, 1 LDG.64 + 1 STS.64 per MB DFMAs.  After every MB
-// rows the MB completed per-column sums of the 32 lanes are summed over the columns of a window in
-// fixed order (deterministic) through a per-warp shared-memory buffer and added to the warp's
-// window table C[k]; M > MB is handled by looping tap blocks.
+// accumulators in registers: every X value is fetched from L2 exactly once and feeds MB DFMAs;
+// each row step starts one window (DMUL) and completes one.  X is not staged as tiles: each lane
+// streams its column through a private shared-memory FIFO filled by 8-byte cp.async copies issued
+// ~20 rows ahead, so neither L2 nor DRAM latency reaches the FMAs and the FP64 pipe
+// (64 DFMA/clk/SM) is the only busy resource.  Every PF rows the PF completed per-column sums of
+// the 32 lanes are summed over the columns of a window in fixed order (deterministic) through a
+// small per-warp buffer and land in the warp's window table.
+//
+// More than 21 taps never occur: a trial with M > 21 is split into c = ceil(M/21) window classes
+// r = 0..c-1 (windows k = kappa*c + r), each of which is the same problem with stride c*st,
+// ceil(D/(c*st)) <= 21 taps and the array shifted by r*st.
 //
 // ONE WARP OWNS ONE TRIAL (period, duration) from its first row to its argmin: there is no CTA
-// barrier after the template nodes are staged, so the warps of an SM (3 CTAs x 4 warps) sit in
-// different phases and the scoring epilogue of one hides behind the DFMAs of the others.
-// Lanes are assigned from a flat list of (row segment, column) pairs, so warps are full for every
-// st; the segment count is chosen per trial to balance lane use against the MB-1 halo rows each
-// segment needs before its first window completes.
+// barrier after the template nodes are staged, so the warps of an SM sit in different phases and
+// the scoring of one hides behind the DFMAs of the others.
+//   stride > 16 ("wide"): lanes are assigned from a flat list of (row segment, column) pairs, so
+//     warps are full for every stride; windows are processed in tiles of the table size.
+//   stride <= 16 ("narrow", short durations, very many windows): floor(32/stride) segments sit
+//     side by side in the warp, the whole class is ONE march of ~n/32 rows, and the table is a
+//     time slice that is scored and recycled every few blocks.
 //
 // a5 (depth from the prefix sums, Eq. 12-14), the score dchi2 = -2 a C + a^2 G (a6+a7; the
 // S2 window term of Eq. 15 cancels against the same term of Eq. 16) and the lexicographic
-// (dchi2, start) argmin (a8) run per window tile from C[k].
+// (dchi2, start) argmin (a8) run from the table.
 // The template nodes are staged in shared memory with one TMA bulk copy (cp.async.bulk).
 #include "gtls_internal.cuh"
 
@@ -34,13 +40,13 @@ namespace {
 
 constexpr int kRT = 128;                 // threads per CTA
 constexpr int kRW = kRT / 32;            // warps (= trials) per CTA
-constexpr int kPartPitch = 33;           // doubles per slot row of the per-warp emit buffer
-constexpr int kMBMax = 21;
-constexpr int kCW = 672;                 // window-table doubles per warp
-constexpr int kTmplSmem = 1024;          // template nodes cached in shared memory
+constexpr int kPartPitch = 36;           // doubles per slot row of the per-warp emit buffer
+constexpr int kPartRows = 8;             // >= max PfRows
 constexpr int kFifoBatches = 3;          // batches of PfRows rows per lane in the cp.async FIFO
 constexpr int kFifoRows = 24;            // >= kFifoBatches * max PfRows
-constexpr int kWarpSmem = kMBMax * kPartPitch + kFifoRows * 32 + kCW;   // doubles of dynamic smem per warp
+constexpr int kCW = 1056;                // window-table doubles per warp (>= 32 * 21)
+constexpr int kTmplSmem = 1024;          // template nodes cached in shared memory
+constexpr int kWarpSmem = kPartRows * kPartPitch + kFifoRows * 32 + kCW;   // doubles per warp
 
 struct Cand { double d; double depth; int s; int has; };
 
@@ -48,25 +54,7 @@ __device__ __forceinline__ void cand_offer(Cand& b, double d, int s, double dept
     if (!b.has || d < b.d || (d == b.d && s < b.s)) { b.d = d; b.s = s; b.depth = depth; b.has = 1; }
 }
 
-struct RGeom {
-    int D, st, nW, M, MB, nmb, Kt;
-    double tscale;                       // (n_tmpl - 1) / D
-};
-
-// tap-block size for M taps: the instantiated MB that wastes the fewest padded taps
-__device__ __forceinline__ void pick_mb(int M, int& MB, int& nmb) {
-    const int cand[5] = {21, 16, 12, 8, 4};
-    int best = 1 << 30;
-    MB = 21; nmb = 1;
-#pragma unroll
-    for (int c = 0; c < 5; ++c) {
-        const int nb = (M + cand[c] - 1) / cand[c];
-        const int cost = nb * cand[c] + (nb - 1);        // slight preference for fewer blocks
-        if (cost < best) { best = cost; MB = cand[c]; nmb = nb; }
-    }
-}
-
-// rows prefetched ahead of the FMAs (divides MB)
+// rows per FIFO batch = completed windows reduced at once (divides MB)
 template <int MB> struct PfRows { static constexpr int v = (MB % 7 == 0) ? 7 : (MB >= 8 ? MB / 2 : MB); };
 
 __device__ __forceinline__ double lds64(const unsigned addr) {
@@ -77,116 +65,202 @@ __device__ __forceinline__ double lds64(const unsigned addr) {
 __device__ __forceinline__ void sts64(const unsigned addr, const double v) {
     asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory");
 }
-
 // 8-byte asynchronous global -> shared copy; `valid == false` writes zeros without reading
 __device__ __forceinline__ void cp_async8(const unsigned dst, const double* src, const bool valid) {
     const int sz = valid ? 8 : 0;
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(src), "r"(sz) : "memory");
 }
+__device__ __forceinline__ void cp_async8(const unsigned dst, const double* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-struct EmitCtx {                         // where completed window sums of one item go
-    int f0, seg_first, ng;               // first flat slot, first segment / segments touched by the warp
-    int split;                           // ng <= 2: first lane of the second segment (32 if none)
-    int slots, st, L, nWt;
-    unsigned ctab;                       // shared-space address of the window table (C or G)
-    unsigned part;                       // shared-space address of the per-warp [MB][kPartPitch] buffer
-    unsigned fifo;                       // shared-space address of the per-warp [kFifoRows][32] X FIFO
+// One window class of one trial, as seen by the owning warp.
+struct Cls {
+    int D, stp, off, nWr;                // window length, class stride, element offset, windows
+    bool uniform;
+    double G_u, den_u, gbar;             // uniform dy: G and sw*gbar are constants
+    const double* s1; const double* s0;  // prefix sums of this period
+    unsigned ctab;                       // shared-space address of the window table
+    unsigned part;                       // shared-space address of the [kPartRows][kPartPitch] emit buffer
+    unsigned fifo;                       // shared-space address of the [kFifoRows][32] X FIFO
+    int Kt;                              // table entries per quantity (C, and G when dy is not uniform)
 };
 
-__device__ __forceinline__ void ctab_add(const EmitCtx& c, const int seg, const int kw, const double sum) {
-    const int w = seg * c.L + kw;
-    if (kw >= 0 && kw < c.L && w < c.nWt) {
-        const unsigned a = c.ctab + (unsigned)(w * 8);
-        sts64(a, lds64(a) + sum);
+// a5 + a8 for one window kappa of the class (start s = off + kappa*stp): hi/lo are the prefix sums
+// at s+D and s.  a = max(rbar, 0) / mean(g_D) with rbar = swr / sw, taken as ONE division.
+__device__ __forceinline__ void score_one(const Cls& c, Cand& best, const int s, const double hi1,
+                                          const double lo1, const double hi0, const double lo0,
+                                          const double C, const double Gt) {
+    const double swr = hi1 - lo1;
+    const double den = c.uniform ? c.den_u : (hi0 - lo0) * c.gbar;
+    const double depth = __ddiv_rn(fmax(swr, 0.0), den);
+    const double Gv = c.uniform ? c.G_u : Gt;
+    const double d = -2.0 * depth * C + (depth * depth) * Gv;
+    cand_offer(best, d, s, depth);
+}
+
+// Wide path: score the windows [k0, k0 + nWt) of the class from table entries [0, nWt).
+__device__ __forceinline__ void score_wide(const Cls& c, Cand& best, const int lane, const int k0,
+                                           const int nWt) {
+    for (int i0 = 0; i0 < nWt; i0 += 128) {
+        double hi1[4], lo1[4], hi0[4], lo0[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int w = i0 + 32 * u + lane;
+            const int s = c.off + (k0 + w) * c.stp;
+            const bool ok = w < nWt;
+            hi1[u] = ok ? __ldg(c.s1 + s + c.D) : 0.0;
+            lo1[u] = ok ? __ldg(c.s1 + s) : 0.0;
+            hi0[u] = 1.0; lo0[u] = 0.0;
+            if (!c.uniform) {
+                hi0[u] = ok ? __ldg(c.s0 + s + c.D) : 1.0;
+                lo0[u] = ok ? __ldg(c.s0 + s) : 0.0;
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int w = i0 + 32 * u + lane;
+            if (w < nWt) {
+                const unsigned ta = c.ctab + (unsigned)(w * 8);
+                score_one(c, best, c.off + (k0 + w) * c.stp, hi1[u], lo1[u], hi0[u], lo0[u], lds64(ta),
+                          c.uniform ? 0.0 : lds64(ta + (unsigned)(c.Kt * 8)));
+            }
+        }
     }
 }
 
-// The MB completed window sums of every lane sit in part[slot][lane]; sum them over the lanes of
-// each segment in fixed order and add to the window table.  Up to two segments per warp (every
-// st >= 31): lane = slot, one unrolled pass over the 32 lanes split at `split`.  Otherwise one
-// (segment, slot) task per lane and round.
-template <int MB>
-__device__ __forceinline__ void reduce_block(const EmitCtx& c, const int kw0, const int lane) {
+// Narrow path: table entry seg*SL + o holds window kw = kw_base + o of segment seg (kappa = seg*L + kw).
+__device__ __forceinline__ void score_narrow(const Cls& c, Cand& best, const int lane, const int G,
+                                             const int SL, const int SLn, const float invSL,
+                                             const int kw_base, const int L) {
+    const int count = G * SL;
+    for (int i0 = 0; i0 < count; i0 += 128) {
+        double hi1[4], lo1[4], hi0[4], lo0[4];
+        int sidx[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int i = i0 + 32 * u + lane;
+            const int seg = (int)(((float)i + 0.5f) * invSL);
+            const int o = i - seg * SL;
+            const int kw = kw_base + o;
+            const int kap = seg * L + kw;
+            const bool ok = i < count && o < SLn && kw >= 0 && kw < L && kap < c.nWr;
+            const int s = c.off + kap * c.stp;
+            sidx[u] = ok ? s : -1;
+            hi1[u] = ok ? __ldg(c.s1 + s + c.D) : 0.0;
+            lo1[u] = ok ? __ldg(c.s1 + s) : 0.0;
+            hi0[u] = 1.0; lo0[u] = 0.0;
+            if (!c.uniform) {
+                hi0[u] = ok ? __ldg(c.s0 + s + c.D) : 1.0;
+                lo0[u] = ok ? __ldg(c.s0 + s) : 0.0;
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (sidx[u] >= 0) {
+                const unsigned ta = c.ctab + (unsigned)((i0 + 32 * u + lane) * 8);
+                score_one(c, best, sidx[u], hi1[u], lo1[u], hi0[u], lo0[u], lds64(ta),
+                          c.uniform ? 0.0 : lds64(ta + (unsigned)(c.Kt * 8)));
+            }
+        }
+    }
+}
+
+struct It {                              // one march: 32 lanes = 32 (segment, column) slots
+    bool narrow, direct;                 // narrow path; narrow with stride 1 (no cross-lane sum)
+    int L;                               // windows per segment
+    // wide: item geometry (flat slots f0 .. f0+31)
+    int f0, seg_first, ng, slots, nWt;
+    // narrow: G segments side by side, table slice of SL = KB*MB windows per segment
+    int G, KB, SL, SLn;                  // SL = odd pitch >= SLn = KB*MB valid windows per segment
+    float invSL;
+    unsigned tab;                        // table of the quantity being accumulated (C or G)
+};
+
+__device__ __forceinline__ void tab_add(const unsigned a, const double v) { sts64(a, lds64(a) + v); }
+
+// PF completed window sums per lane sit in part[slot][lane] (windows kwb .. kwb+PF-1 of the lane's
+// segment): sum them over the lanes of each segment in fixed order.
+template <int PF>
+__device__ __forceinline__ void reduce_batch(const Cls& c, const It& it, const int kwb, const int kw_base,
+                                             const int lane) {
     __syncwarp();
-    if (c.ng == 1) {
-        if (lane < MB) {
-            const unsigned pr = c.part + (unsigned)(lane * kPartPitch * 8);
-            double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    if (!it.narrow && it.ng == 1) {
+        // four lanes per slot, eight strided values each, two shuffle steps
+        const int sl = lane >> 2, r = lane & 3;
+        double v = 0.0;
+        if (sl < PF) {
+            const unsigned pr = c.part + (unsigned)((sl * kPartPitch + r) * 8);
+            double a0 = 0.0, a1 = 0.0;
 #pragma unroll
-            for (int q = 0; q < 32; q += 4) {
-                a0 += lds64(pr + 8 * q);
-                a1 += lds64(pr + 8 * q + 8);
-                a2 += lds64(pr + 8 * q + 16);
-                a3 += lds64(pr + 8 * q + 24);
-            }
-            ctab_add(c, c.seg_first, kw0 + lane, (a0 + a1) + (a2 + a3));
+            for (int i = 0; i < 8; i += 2) { a0 += lds64(pr + 32 * i); a1 += lds64(pr + 32 * i + 32); }
+            v = a0 + a1;
         }
-    } else if (c.ng == 2) {
-        if (lane < MB) {
-            const unsigned pr = c.part + (unsigned)(lane * kPartPitch * 8);
-            double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
-#pragma unroll
-            for (int q = 0; q < 32; q += 2) {
-                const double v0 = lds64(pr + 8 * q), v1 = lds64(pr + 8 * q + 8);
-                a0 += q < c.split ? v0 : 0.0;
-                b0 += q < c.split ? 0.0 : v0;
-                a1 += q + 1 < c.split ? v1 : 0.0;
-                b1 += q + 1 < c.split ? 0.0 : v1;
-            }
-            ctab_add(c, c.seg_first, kw0 + lane, a0 + a1);
-            ctab_add(c, c.seg_first + 1, kw0 + lane, b0 + b1);
-        }
-    } else {
-        for (int t = lane; t < c.ng * MB; t += 32) {
-            const int gi = t / MB, sl = t - gi * MB;
-            const int seg = c.seg_first + gi;
-            int lo = seg * c.st - c.f0, hi = lo + c.st;
+        v += __shfl_xor_sync(0xffffffffu, v, 1);
+        v += __shfl_xor_sync(0xffffffffu, v, 2);
+        const int kw = kwb + sl, w = it.seg_first * it.L + kw;
+        if (r == 0 && sl < PF && kw >= 0 && kw < it.L && w < it.nWt) tab_add(it.tab + (unsigned)(w * 8), v);
+    } else if (!it.narrow) {
+        for (int t = lane; t < it.ng * PF; t += 32) {
+            const int gi = t / PF, sl = t - gi * PF;
+            const int seg = it.seg_first + gi;
+            int lo = seg * c.stp - it.f0, hi = lo + c.stp;
             lo = lo < 0 ? 0 : lo;
             hi = hi > 32 ? 32 : hi;
-            hi = hi > c.slots - c.f0 ? c.slots - c.f0 : hi;
+            hi = hi > it.slots - it.f0 ? it.slots - it.f0 : hi;
             const unsigned pr = c.part + (unsigned)(sl * kPartPitch * 8);
-            double s0 = 0.0, s1 = 0.0;
+            double a0 = 0.0, a1 = 0.0;
             int q = lo;
-            for (; q + 1 < hi; q += 2) { s0 += lds64(pr + 8 * q); s1 += lds64(pr + 8 * q + 8); }
-            if (q < hi) s0 += lds64(pr + 8 * q);
-            ctab_add(c, seg, kw0 + sl, s0 + s1);
+            for (; q + 1 < hi; q += 2) { a0 += lds64(pr + 8 * q); a1 += lds64(pr + 8 * q + 8); }
+            if (q < hi) a0 += lds64(pr + 8 * q);
+            const int kw = kwb + sl, w = seg * it.L + kw;
+            if (kw >= 0 && kw < it.L && w < it.nWt) tab_add(it.tab + (unsigned)(w * 8), a0 + a1);
+        }
+    } else {
+        for (int t = lane; t < it.G * PF; t += 32) {
+            const int g = t / PF, sl = t - g * PF;
+            const unsigned pr = c.part + (unsigned)((sl * kPartPitch + g * c.stp) * 8);
+            double a0 = 0.0;
+            for (int q = 0; q < c.stp; ++q) a0 += lds64(pr + 8 * q);
+            sts64(it.tab + (unsigned)((g * it.SL + (kwb + sl - kw_base)) * 8), a0);
         }
     }
     __syncwarp();
 }
 
-// One item: march `nblk` blocks of MB rows.  `xp` points at this lane's X value of the first row;
-// rows >= rows_valid read as 0.  Each lane streams its column through a private FIFO in shared
-// memory filled by 8-byte cp.async copies (kFifoBatches batches of PF rows in flight, so L2 / DRAM
-// latency never reaches the FMAs); after every block of MB rows the MB completed window sums are
-// reduced over the lanes of each segment.
+// One march: `nblk` blocks of MB rows.  `xp` points at this lane's X value of the first row, rows
+// >= rows_valid read as 0 (rows_min = the smallest rows_valid of the warp, so batches below it need
+// no predicate).  Taps T[m] multiply row (window + m).  Narrow path: every KB blocks the table slice
+// is scored and recycled.
 template <int MB>
-__device__ __forceinline__ void march(const double* __restrict__ xp, const double* __restrict__ xsafe,
-                                      const int st, const int rows_valid, const int nblk,
-                                      const double (&T)[MB], const int lane, const EmitCtx& c) {
+__device__ __forceinline__ void march(const Cls& c, const It& it, const double* __restrict__ xp,
+                                      const int rows_valid, const int rows_min, const int nblk,
+                                      const double (&T)[MB], const int lane, Cand& best) {
     constexpr int PF = PfRows<MB>::v;
-    static_assert(MB % PF == 0 && kFifoBatches * PF <= kFifoRows, "FIFO geometry");
+    static_assert(MB % PF == 0 && kFifoBatches * PF <= kFifoRows && PF <= kPartRows, "geometry");
     double acc[MB], xr[PF];
 #pragma unroll
     for (int u = 0; u < MB; ++u) acc[u] = 0.0;
     const unsigned fl = c.fifo + (unsigned)(lane * 8);
+    const long long rstride = (long long)c.stp;
     int row_pf = 0;                                // row index the next copy belongs to
 #pragma unroll
     for (int k = 0; k < kFifoBatches; ++k) {
 #pragma unroll
         for (int u = 0; u < PF; ++u) {
-            const bool ok = row_pf < rows_valid;
-            cp_async8(fl + (unsigned)((k * PF + u) * 256), ok ? xp : xsafe, ok);
-            xp += st;
+            cp_async8(fl + (unsigned)((k * PF + u) * 256), xp, row_pf < rows_valid);
+            xp += rstride;
             ++row_pf;
         }
         cp_async_commit();
     }
     int fb = 0;                                    // FIFO batch holding the rows consumed next
-    const unsigned pl = c.part + (unsigned)(lane * 8);
+    int kw_base = -(MB - 1), bis = 0;              // narrow: first window of the slice, blocks in it
+    const unsigned part_lane = c.part + (unsigned)(lane * 8);
+    const unsigned tab_lane = it.tab + (unsigned)(lane * it.SL * 8);
 #pragma unroll 1
     for (int blk = 0; blk < nblk; ++blk) {
 #pragma unroll
@@ -196,13 +270,14 @@ __device__ __forceinline__ void march(const double* __restrict__ xp, const doubl
                 const unsigned fa = fl + (unsigned)(fb * PF * 256);
 #pragma unroll
                 for (int k = 0; k < PF; ++k) xr[k] = lds64(fa + k * 256);
+                if (row_pf + PF <= rows_min) {
 #pragma unroll
-                for (int k = 0; k < PF; ++k) {
-                    const bool ok = row_pf < rows_valid;
-                    cp_async8(fa + k * 256, ok ? xp : xsafe, ok);
-                    xp += st;
-                    ++row_pf;
+                    for (int k = 0; k < PF; ++k) { cp_async8(fa + k * 256, xp); xp += rstride; }
+                } else {
+#pragma unroll
+                    for (int k = 0; k < PF; ++k) { cp_async8(fa + k * 256, xp, row_pf + k < rows_valid); xp += rstride; }
                 }
+                row_pf += PF;
                 cp_async_commit();
                 fb = fb + 1 == kFifoBatches ? 0 : fb + 1;
             }
@@ -213,11 +288,27 @@ __device__ __forceinline__ void march(const double* __restrict__ xp, const doubl
                 if (m == 0) acc[a] = T[0] * x;                      // window gamma starts at this row
                 else acc[a] = fma(T[m], x, acc[a]);
             }
-            sts64(pl + (unsigned)(u * kPartPitch * 8), acc[(u + 1) % MB]);   // window gamma-(MB-1) complete
+            // window gamma - (MB-1) is complete
+            const unsigned ea = it.direct ? tab_lane + (unsigned)((bis * MB + u) * 8)
+                                          : part_lane + (unsigned)((u % PF) * kPartPitch * 8);
+            sts64(ea, acc[(u + 1) % MB]);
+            if (u % PF == PF - 1 && !it.direct)
+                reduce_batch<PF>(c, it, blk * MB + (u - (PF - 1)) - (MB - 1), kw_base, lane);
         }
-        reduce_block<MB>(c, blk * MB - (MB - 1), lane);
+        if (it.narrow && ++bis == it.KB) {
+            __syncwarp();
+            score_narrow(c, best, lane, it.G, it.SL, it.SLn, it.invSL, kw_base, it.L);
+            __syncwarp();
+            kw_base += it.SLn;
+            bis = 0;
+        }
     }
     cp_async_wait<0>();
+    if (it.narrow && bis > 0) {
+        __syncwarp();
+        score_narrow(c, best, lane, it.G, it.SL, it.SLn, it.invSL, kw_base, it.L);
+        __syncwarp();
+    }
 }
 
 __device__ __forceinline__ double tmpl_lerp(const double* __restrict__ tm, int n_tmpl, int j, double tscale) {
@@ -229,55 +320,117 @@ __device__ __forceinline__ double tmpl_lerp(const double* __restrict__ tm, int n
     return t0 + fr * (tm[k + 1] - t0);
 }
 
-// All items (32 flat (segment, column) slots each) and tap blocks of one window tile, one pass.
+// One march of the lanes' (segment, column) slots: taps, bounds, then the ring.
+//   seg/col: this lane's slot (active == false: an idle lane, zero taps);  row0: first row of seg.
 template <int MB>
-__device__ __forceinline__ void run_tile(const int n, const int n_tmpl, const RGeom& q,
-                                         const double* __restrict__ tm, const double* __restrict__ x,
-                                         const bool square, const int lane, const int nseg, const int L,
-                                         const int nWt, const int k0, const unsigned part,
-                                         const unsigned fifo, const unsigned ctab) {
-    EmitCtx c;
-    c.slots = nseg * q.st; c.st = q.st; c.L = L; c.nWt = nWt;
-    c.ctab = ctab; c.part = part; c.fifo = fifo;
-    const int items = (c.slots + 31) >> 5;
-    const int nblk = (L + MB - 1 + MB - 1) / MB;
-    const long long lim = (long long)n + q.D;          // x entries >= lim are never needed
-    for (int item = 0; item < items; ++item) {
-        c.f0 = item << 5;
-        c.seg_first = c.f0 / q.st;
-        c.ng = min(c.f0 + 31, c.slots - 1) / q.st - c.seg_first + 1;
-        c.split = c.ng == 1 ? 32 : (c.seg_first + 1) * q.st - c.f0;
-        const int f = c.f0 + lane;
-        const bool active = f < c.slots;
-        const int seg = active ? f / q.st : 0;
-        const int col = active ? f - seg * q.st : 0;
-        for (int b = 0; b < q.nmb; ++b) {
-            double T[MB];
+__device__ __forceinline__ void run_march(const Cls& c, const It& it, const int n, const int n_tmpl,
+                                          const double tscale, const double* __restrict__ tm,
+                                          const double* __restrict__ x, const bool square,
+                                          const bool active, const int row0, const int col,
+                                          const int lane, Cand& best) {
+    double T[MB];
 #pragma unroll
-            for (int m = 0; m < MB; ++m) {
-                const long long j = (long long)(b * MB + m) * q.st + col;
-                double g = 0.0;
-                if (active && j < q.D) g = tmpl_lerp(tm, n_tmpl, (int)j, q.tscale);
-                T[m] = square ? g * g : g;
+    for (int m = 0; m < MB; ++m) {
+        const int j = m * c.stp + col;
+        double g = 0.0;
+        if (active && j < c.D) g = tmpl_lerp(tm, n_tmpl, j, tscale);
+        T[m] = square ? g * g : g;
+    }
+    const int nblk = (it.L + MB - 1 + MB - 1) / MB;
+    const int rows_all = nblk * MB + kFifoBatches * PfRows<MB>::v;   // rows ever requested
+    const long long lim = (long long)n + c.D;                        // x entries >= lim are never needed
+    const long long ebase = (long long)c.off + (long long)row0 * c.stp + col;
+    int rows_valid = 0;
+    if (ebase < lim) {
+        const long long rv = (lim - ebase + c.stp - 1) / c.stp;
+        rows_valid = rv > rows_all ? rows_all : (int)rv;
+    }
+    const int rows_min = __reduce_min_sync(0xffffffffu, rows_valid);
+    march<MB>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane, best);
+}
+
+template <int MB, bool NARROW>
+__device__ __forceinline__ void run_class(const Cls& c, const int n, const int n_tmpl, const double tscale,
+                                          const double* __restrict__ tm, const double* __restrict__ x1,
+                                          const double* __restrict__ x0, const int lane, Cand& best) {
+    if (c.nWr <= 0) return;
+    It it;
+    it.tab = c.ctab;
+    if (NARROW) {
+        // ---- narrow: G segments side by side, one march over the whole class -------------------
+        it.narrow = true; it.direct = c.stp == 1;   // (NARROW implies uniform dy and stp <= kChi2NarrowMax)
+        it.G = 32 / c.stp;
+        it.L = (c.nWr + it.G - 1) / it.G;
+        it.KB = (c.Kt - it.G) / (it.G * MB);
+        it.SLn = it.KB * MB;
+        it.SL = it.SLn | 1;
+        it.invSL = 1.0f / (float)it.SL;
+        it.f0 = 0; it.seg_first = 0; it.ng = it.G; it.slots = it.G * c.stp; it.nWt = c.nWr;
+        const bool active = lane < it.slots;
+        const int seg = active ? lane / c.stp : 0;
+        const int col = active ? lane - seg * c.stp : 0;
+        run_march<MB>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best);
+        return;
+    }
+    // ---- wide: window tiles of the table size, flat (segment, column) slots ------------------------
+    it.narrow = false; it.direct = false;
+    it.G = 0; it.KB = 0; it.SL = 0; it.SLn = 0; it.invSL = 0.f;
+    for (int k0 = 0; k0 < c.nWr; k0 += c.Kt) {
+        const int nWt = min(c.Kt, c.nWr - k0);
+        // segment count: minimise items * rows per item (one warp runs them all)
+        int bc = 0x7fffffff, bn = 1;
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+            const int ns = lane + 1 + 32 * r;
+            if (ns <= nWt) {
+                const int L = (nWt + ns - 1) / ns;
+                const int items = (ns * c.stp + 31) >> 5;
+                const int cost = items * (((L + 2 * MB - 2) / MB) * MB + 8);
+                if (cost < bc) { bc = cost; bn = ns; }
             }
-            const long long ebase = ((long long)(k0 + seg * L) + (long long)b * MB) * q.st + col;
-            int rows_valid = 0;
-            if (active && ebase < lim) {
-                const long long rv = (lim - ebase + q.st - 1) / q.st;
-                rows_valid = rv > (long long)nblk * MB ? nblk * MB : (int)rv;
-            }
-            march<MB>(x + (active ? ebase : 0), x, q.st, rows_valid, nblk, T, lane, c);
         }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const int oc = __shfl_xor_sync(0xffffffffu, bc, o), on = __shfl_xor_sync(0xffffffffu, bn, o);
+            if (oc < bc || (oc == bc && on < bn)) { bc = oc; bn = on; }
+        }
+        const int nseg = bn;
+        it.L = (nWt + nseg - 1) / nseg;
+        it.slots = nseg * c.stp;
+        it.nWt = nWt;
+        const int items = (it.slots + 31) >> 5;
+        for (int i = lane; i < (c.uniform ? nWt : c.Kt + nWt); i += 32) sts64(c.ctab + (unsigned)(i * 8), 0.0);
+        __syncwarp();
+        for (int pass = 0; pass < (c.uniform ? 1 : 2); ++pass) {
+            it.tab = c.ctab + (unsigned)(pass * c.Kt * 8);
+            for (int item = 0; item < items; ++item) {
+                it.f0 = item << 5;
+                it.seg_first = it.f0 / c.stp;
+                it.ng = min(it.f0 + 31, it.slots - 1) / c.stp - it.seg_first + 1;
+                const int f = it.f0 + lane;
+                const bool active = f < it.slots;
+                const int seg = active ? f / c.stp : 0;
+                const int col = active ? f - seg * c.stp : 0;
+                run_march<MB>(c, it, n, n_tmpl, tscale, tm, pass == 0 ? x1 : x0, pass == 1, active,
+                              k0 + seg * it.L, col, lane, best);
+            }
+        }
+        __syncwarp();
+        score_wide(c, best, lane, k0, nWt);
+        __syncwarp();
     }
 }
 
-template <bool UNIFORM>
-__global__ void __launch_bounds__(kRT, 3) k_chi2_ring(TileArgs a) {
-    extern __shared__ double dsm[];                 // per warp: [kMBMax][kPartPitch] emit buffer, window table
+template <int MB, bool NARROW, bool UNIFORM>
+__global__ void __launch_bounds__(kRT, 3) k_chi2_ring(TileArgs a, const int* __restrict__ list,
+                                                      const int* __restrict__ count) {
+    extern __shared__ double dsm[];                 // per warp: emit buffer, X FIFO, window table
     __shared__ __align__(16) double s_tmpl[kTmplSmem];
     __shared__ __align__(8) unsigned long long s_mbar;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int n_mine = *count;                      // trials of this variant in the tile
+    if ((int)blockIdx.x * kRW >= n_mine) return;
     // ---- template nodes -> shared memory: one TMA bulk copy when size / alignment allow ------
     const bool tmpl_in_smem = a.n_tmpl <= kTmplSmem;
     const unsigned tbytes = (unsigned)a.n_tmpl * 8u;
@@ -305,134 +458,89 @@ __global__ void __launch_bounds__(kRT, 3) k_chi2_ring(TileArgs a) {
         }
     }
     // ---- from here on every warp works alone on its own trial ------------------------------------
-    const long long trial = (long long)blockIdx.x * kRW + warp;
-    if (trial >= (long long)a.tile * a.n_dur) return;
-    const int pl = (int)(trial / a.n_dur), jd = (int)(trial - (long long)pl * a.n_dur);
+    const int li = (int)blockIdx.x * kRW + warp;
+    if (li >= n_mine) return;
+    const int trial = list[li];
+    const int pl = trial / a.n_dur;
     const DurEntry e = a.durtab[trial];
     Partial* out = a.partial + trial;
-    if (e.skip || e.stride < a.dbg_min_st || e.stride > a.dbg_max_st) {
-        if (lane == 0) { out->valid = 0; out->dchi2 = 0.0; out->depth = 0.0; out->start = 0; }
-        return;
-    }
-    (void)jd;
-    RGeom q;
-    q.D = e.D; q.st = e.stride;
-    q.nW = (a.n + q.st - 1) / q.st;
-    q.M = (q.D + q.st - 1) / q.st;
-    pick_mb(q.M, q.MB, q.nmb);
-    q.Kt = UNIFORM ? kCW : kCW / 2;
-    q.tscale = __ddiv_rn((double)(a.n_tmpl - 1), (double)q.D);
+    const int st = e.stride;
+    const int nW = (a.n + st - 1) / st;
+    const int M = (e.D + st - 1) / st;
+    const int ncls = (M + 20) / 21;                 // window classes: at most 21 taps each
+    Cls c;
+    c.D = e.D; c.stp = ncls * st;
+    c.uniform = UNIFORM;
+    c.gbar = e.gbar;
+    c.G_u = a.w_uniform * e.gg2;
+    c.den_u = ((double)e.D * a.w_uniform) * e.gbar;
+    c.s1 = a.s1 + (long long)pl * a.spitch;
+    c.s0 = a.s0 + (long long)pl * a.spitch;
+    double* const wsm = dsm + warp * kWarpSmem;
+    c.part = (unsigned)__cvta_generic_to_shared(wsm);
+    c.fifo = c.part + (unsigned)(kPartRows * kPartPitch * 8);
+    c.ctab = c.fifo + (unsigned)(kFifoRows * 32 * 8);
+    c.Kt = UNIFORM ? kCW : kCW / 2;
+    const double tscale = __ddiv_rn((double)(a.n_tmpl - 1), (double)e.D);
     const double* __restrict__ tm = tmpl_in_smem ? s_tmpl : a.tmpl;
     const double* __restrict__ x1 = a.x1 + (long long)pl * a.pitch;
     const double* __restrict__ x0 = a.x0 + (long long)pl * a.pitch;
-    const double* __restrict__ s1 = a.s1 + (long long)pl * a.spitch;
-    const double* __restrict__ s0 = a.s0 + (long long)pl * a.spitch;
-    const double G_u = a.w_uniform * e.gg2;
-    const double den_u = ((double)q.D * a.w_uniform) * e.gbar;
-    double* const wsm = dsm + warp * kWarpSmem;
-    const unsigned part = (unsigned)__cvta_generic_to_shared(wsm);
-    const unsigned fifo = part + (unsigned)(kMBMax * kPartPitch * 8);
-    double* const ctab = wsm + kMBMax * kPartPitch + kFifoRows * 32;
-    const unsigned ctab_s = (unsigned)__cvta_generic_to_shared(ctab);
     Cand best; best.has = 0; best.d = 0.0; best.s = 0; best.depth = 0.0;
 
-    for (int k0 = 0; k0 < q.nW; k0 += q.Kt) {
-        const int nWt = min(q.Kt, q.nW - k0);
-        // ---- segment count: minimise items * rows per item (one warp runs them all) -------------------
-        int bc = 0x7fffffff, bn = 1;
-#pragma unroll
-        for (int r = 0; r < 2; ++r) {
-            const int ns = lane + 1 + 32 * r;
-            if (ns <= nWt) {
-                const int L = (nWt + ns - 1) / ns;
-                const int items = (ns * q.st + 31) >> 5;
-                const int cost = items * (((L + 2 * q.MB - 2) / q.MB) * q.MB + 8);
-                if (cost < bc) { bc = cost; bn = ns; }
-            }
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            const int oc = __shfl_xor_sync(0xffffffffu, bc, o), on = __shfl_xor_sync(0xffffffffu, bn, o);
-            if (oc < bc || (oc == bc && on < bn)) { bc = oc; bn = on; }
-        }
-        const int nseg = bn;
-        const int L = (nWt + nseg - 1) / nseg;
-        for (int i = lane; i < (UNIFORM ? nWt : 2 * q.Kt); i += 32) ctab[i] = 0.0;
-        __syncwarp();
-
-        for (int pass = 0; pass < (UNIFORM ? 1 : 2); ++pass) {
-            const double* __restrict__ x = pass == 0 ? x1 : x0;
-            const unsigned ct = ctab_s + (unsigned)(pass * q.Kt * 8);
-            switch (q.MB) {
-                case 21: run_tile<21>(a.n, a.n_tmpl, q, tm, x, pass == 1, lane, nseg, L, nWt, k0, part, fifo, ct); break;
-                case 16: run_tile<16>(a.n, a.n_tmpl, q, tm, x, pass == 1, lane, nseg, L, nWt, k0, part, fifo, ct); break;
-                case 12: run_tile<12>(a.n, a.n_tmpl, q, tm, x, pass == 1, lane, nseg, L, nWt, k0, part, fifo, ct); break;
-                case 8: run_tile<8>(a.n, a.n_tmpl, q, tm, x, pass == 1, lane, nseg, L, nWt, k0, part, fifo, ct); break;
-                default: run_tile<4>(a.n, a.n_tmpl, q, tm, x, pass == 1, lane, nseg, L, nWt, k0, part, fifo, ct); break;
-            }
-        }
-        __syncwarp();
-        // ---- a5 + a8 per window of the tile, four windows per lane in flight ---------------------------
-        for (int w0 = 0; w0 < nWt; w0 += 128) {
-            double hi1[4], lo1[4], hi0[4], lo0[4];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const int w = w0 + 32 * u + lane;
-                const int sidx = (k0 + w) * q.st;
-                const bool ok = w < nWt;
-                hi1[u] = ok ? __ldg(s1 + sidx + q.D) : 0.0;
-                lo1[u] = ok ? __ldg(s1 + sidx) : 0.0;
-                if (!UNIFORM) {
-                    hi0[u] = ok ? __ldg(s0 + sidx + q.D) : 1.0;
-                    lo0[u] = ok ? __ldg(s0 + sidx) : 0.0;
-                }
-            }
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const int w = w0 + 32 * u + lane;
-                if (w < nWt) {
-                    const int sidx = (k0 + w) * q.st;
-                    const double swr = hi1[u] - lo1[u];
-                    const double den = UNIFORM ? den_u : (hi0[u] - lo0[u]) * e.gbar;
-                    // a = max(rbar, 0) / mean(g_D),  rbar = swr / sw   (one division)
-                    const double depth = __ddiv_rn(fmax(swr, 0.0), den);
-                    const double C = ctab[w];
-                    const double Gv = UNIFORM ? G_u : ctab[q.Kt + w];
-                    const double d = -2.0 * depth * C + (depth * depth) * Gv;
-                    cand_offer(best, d, sidx, depth);
-                }
-            }
-        }
-        __syncwarp();
+    for (int r = 0; r < ncls; ++r) {
+        c.off = r * st;
+        c.nWr = nW > r ? (nW - r + ncls - 1) / ncls : 0;
+        run_class<MB, NARROW>(c, a.n, a.n_tmpl, tscale, tm, x1, x0, lane, best);
     }
 
     // warp-wide lexicographic min on (d, s)
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
-        Cand c;
-        c.d = __shfl_xor_sync(0xffffffffu, best.d, o);
-        c.depth = __shfl_xor_sync(0xffffffffu, best.depth, o);
-        c.s = __shfl_xor_sync(0xffffffffu, best.s, o);
-        c.has = __shfl_xor_sync(0xffffffffu, best.has, o);
-        if (c.has) cand_offer(best, c.d, c.s, c.depth);
+        Cand o2;
+        o2.d = __shfl_xor_sync(0xffffffffu, best.d, o);
+        o2.depth = __shfl_xor_sync(0xffffffffu, best.depth, o);
+        o2.s = __shfl_xor_sync(0xffffffffu, best.s, o);
+        o2.has = __shfl_xor_sync(0xffffffffu, best.has, o);
+        if (o2.has) cand_offer(best, o2.d, o2.s, o2.depth);
     }
     if (lane == 0) { out->valid = best.has; out->dchi2 = best.d; out->depth = best.depth; out->start = best.s; }
 }
 
 }  // namespace
 
-void launch_chi2_ring(const TileArgs& a, cudaStream_t st) {
+template <int MB, bool NARROW, bool UNIFORM>
+static void launch_variant(const TileArgs& a, int v, cudaStream_t st) {
     const long long trials = (long long)a.tile * a.n_dur;
-    const unsigned grid = (unsigned)((trials + kRW - 1) / kRW);
+    const unsigned grid = (unsigned)((trials + kRW - 1) / kRW);     // worst case; surplus CTAs exit at once
     const size_t sm = (size_t)(kRW * kWarpSmem) * sizeof(double);
     static bool set = false;
     if (!set) {
-        cudaFuncSetAttribute(k_chi2_ring<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-        cudaFuncSetAttribute(k_chi2_ring<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+        cudaFuncSetAttribute(k_chi2_ring<MB, NARROW, UNIFORM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
         set = true;
     }
-    if (a.uniform) k_chi2_ring<true><<<grid, kRT, sm, st>>>(a);
-    else k_chi2_ring<false><<<grid, kRT, sm, st>>>(a);
+    k_chi2_ring<MB, NARROW, UNIFORM><<<grid, kRT, sm, st>>>(a, a.trial_list + (long long)v * trials, a.trial_count + v);
+}
+
+void launch_chi2_ring(const TileArgs& a, cudaStream_t st) {
+    launch_bin_trials(a, st);
+    if (a.uniform) {
+        launch_variant<21, false, true>(a, 0, st);
+        launch_variant<16, false, true>(a, 1, st);
+        launch_variant<12, false, true>(a, 2, st);
+        launch_variant<8, false, true>(a, 3, st);
+        launch_variant<4, false, true>(a, 4, st);
+        launch_variant<21, true, true>(a, 5, st);
+        launch_variant<16, true, true>(a, 6, st);
+        launch_variant<12, true, true>(a, 7, st);
+        launch_variant<8, true, true>(a, 8, st);
+        launch_variant<4, true, true>(a, 9, st);
+    } else {
+        launch_variant<21, false, false>(a, 0, st);
+        launch_variant<16, false, false>(a, 1, st);
+        launch_variant<12, false, false>(a, 2, st);
+        launch_variant<8, false, false>(a, 3, st);
+        launch_variant<4, false, false>(a, 4, st);
+    }
 }
 
 }  // namespace gtls

@@ -65,7 +65,7 @@ Sizes workspace_sizes(long long n, long long n_per, int n_dur, double q_max, boo
               align_up(sizeof(SdeScratch)) + align_up(2 * sizeof(unsigned long long)) +
               2 * align_up(n_per * sizeof(double)) + align_up(n_per * sizeof(gtls_best)) + 4096;
     s.per_period = 2 * n * sizeof(u64) + 256ull * nt * sizeof(u32) + n_dur * sizeof(DurEntry) +
-                   n_dur * sizeof(Partial) +
+                   n_dur * sizeof(Partial) + (size_t)kChi2Variants * n_dur * sizeof(int) +
                    (uniform ? 1 : 2) * ((size_t)pitch + spitch) * sizeof(double);
     return s;
 }
@@ -275,6 +275,8 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     a.counts = ws.take<u32>((size_t)tile * 256 * nt);
     a.durtab = ws.take<DurEntry>((size_t)tile * n_dur);
     a.partial = ws.take<Partial>((size_t)tile * n_dur);
+    a.trial_list = ws.take<int>((size_t)kChi2Variants * tile * n_dur);
+    a.trial_count = ws.take<int>(kChi2Variants);
     a.x1 = ws.take<double>((size_t)tile * a.pitch);
     a.s1 = ws.take<double>((size_t)tile * a.spitch);
     if (!uniform) {

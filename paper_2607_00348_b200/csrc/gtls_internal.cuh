@@ -40,6 +40,10 @@ struct CurveInfo {
     int32_t pad_;
 };
 
+// chi2 ring kernel variants: ring size index (0..4 = 21, 16, 12, 8, 4 taps) + 5 * narrow
+constexpr int kChi2Variants = 10;
+constexpr int kChi2NarrowMax = 16;   // largest class stride handled by the narrow variants
+
 constexpr int kRadixThreads = 256;
 constexpr int kRadixItems = 8;
 constexpr int kRadixTile = kRadixThreads * kRadixItems;   // 2048 keys per CTA
@@ -114,6 +118,8 @@ struct TileArgs {
     double* x1; double* x0;   // [tile*pitch]
     double* s1; double* s0;   // [tile*spitch]
     Partial* partial;      // [tile*n_dur]
+    int* trial_list;       // [kChi2Variants][tile*n_dur] trial indices binned by chi2 kernel variant
+    int* trial_count;      // [kChi2Variants]
     int dbg_min_st, dbg_max_st;   // timing experiments only (GTLS_DBG_MIN_ST / GTLS_DBG_MAX_ST): skip other trials
 };
 
@@ -122,6 +128,8 @@ void launch_curve_pre(const double* t, const double* y, const double* dy, int n,
 void launch_grid_check(const double* periods, long long n_per, const double* durs,
                        long long n_durs_total, CurveInfo* info, cudaStream_t st);
 void launch_durtab(const TileArgs& a, cudaStream_t st);
+// bins the tile's trials by chi2 kernel variant (order preserved); skipped trials get an invalid Partial
+void launch_bin_trials(const TileArgs& a, cudaStream_t st);
 void launch_fold_keys(const TileArgs& a, double* phase_out, cudaStream_t st);
 // sorts keys_a (in place semantics: result is returned in the pointer the function returns)
 u64* launch_phase_sort(const TileArgs& a, cudaStream_t st, int* n_launches);

@@ -122,6 +122,68 @@ __global__ void __launch_bounds__(256) k_durtab(TileArgs a) {
     }
 }
 
+// chi2 variant of one trial (see chi2_ring.cu): classes of at most 21 taps, ring size, narrow/wide.
+__device__ __forceinline__ int chi2_variant(const DurEntry& e, const TileArgs& a) {
+    if (e.skip || e.stride < a.dbg_min_st || e.stride > a.dbg_max_st) return -1;
+    const int M = (e.D + e.stride - 1) / e.stride;
+    const int ncls = (M + 20) / 21;
+    const int stp = ncls * e.stride;
+    const int Mp = (e.D + stp - 1) / stp;
+    const int mbi = Mp > 16 ? 0 : (Mp > 12 ? 1 : (Mp > 8 ? 2 : (Mp > 4 ? 3 : 4)));
+    const int narrow = (a.uniform && stp <= kChi2NarrowMax) ? 1 : 0;
+    return narrow * 5 + mbi;
+}
+
+// One CTA: every thread owns a contiguous chunk of trials, so the lists keep trial order (the
+// trials of a period stay neighbours and share its x1 in L2).
+__global__ void __launch_bounds__(1024) k_bin_trials(TileArgs a) {
+    __shared__ int s_warp[kChi2Variants][32];
+    const int T = a.tile * a.n_dur;
+    const int chunk = (T + blockDim.x - 1) / blockDim.x;
+    const int t0 = threadIdx.x * chunk, t1 = min(T, t0 + chunk);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int cnt[kChi2Variants];
+#pragma unroll
+    for (int v = 0; v < kChi2Variants; ++v) cnt[v] = 0;
+    for (int t = t0; t < t1; ++t) {
+        const int v = chi2_variant(a.durtab[t], a);
+#pragma unroll
+        for (int k = 0; k < kChi2Variants; ++k) cnt[k] += (v == k) ? 1 : 0;
+        if (v < 0) { Partial p; p.dchi2 = 0.0; p.depth = 0.0; p.start = 0; p.valid = 0; a.partial[t] = p; }
+    }
+    int excl[kChi2Variants];
+#pragma unroll
+    for (int v = 0; v < kChi2Variants; ++v) {
+        int x = cnt[v];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+        excl[v] = x - cnt[v];
+        if (lane == 31) s_warp[v][warp] = x;
+    }
+    __syncthreads();
+    if (warp == 0) {
+#pragma unroll
+        for (int v = 0; v < kChi2Variants; ++v) {
+            const int c = lane < (int)(blockDim.x >> 5) ? s_warp[v][lane] : 0;
+            int x = c;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+            s_warp[v][lane] = x - c;
+            if (lane == 31) a.trial_count[v] = x;
+        }
+    }
+    __syncthreads();
+    int pos[kChi2Variants];
+#pragma unroll
+    for (int v = 0; v < kChi2Variants; ++v) pos[v] = s_warp[v][warp] + excl[v];
+    for (int t = t0; t < t1; ++t) {
+        const int v = chi2_variant(a.durtab[t], a);
+#pragma unroll
+        for (int k = 0; k < kChi2Variants; ++k)
+            if (v == k) { a.trial_list[(long long)k * T + pos[k]] = t; ++pos[k]; }
+    }
+}
+
 }  // namespace
 
 void launch_curve_pre(const double* t, const double* y, const double* dy, int n, double* wr,
@@ -136,6 +198,8 @@ void launch_grid_check(const double* periods, long long n_per, const double* dur
     blocks = blocks < 1 ? 1 : (blocks > 1184 ? 1184 : blocks);
     k_grid_check<<<blocks, 256, 0, st>>>(periods, n_per, durs, n_durs_total, info);
 }
+
+void launch_bin_trials(const TileArgs& a, cudaStream_t st) { k_bin_trials<<<1, 1024, 0, st>>>(a); }
 
 void launch_durtab(const TileArgs& a, cudaStream_t st) {
     const long long warps = (long long)a.tile * a.n_dur;
