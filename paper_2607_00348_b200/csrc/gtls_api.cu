@@ -309,7 +309,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
         tm.mark(5);
         launch_reduce(a, sorted, d_chi2, d_best, d_counters, st);
         tm.mark(6);
-        stats.kernel_launches += launches + 5;
+        stats.kernel_launches += launches + 4 + ((use_v1 || use_rows) ? 1 : 1 + (uniform ? kChi2Variants : kChi2Variants / 2));
         stats.chi2_launches += 1;
         if (o.stats) {
             CU(cudaStreamSynchronize(st));
