@@ -81,7 +81,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 struct Cls {
     int D, stp, off, nWr;                // window length, class stride, element offset, windows
     bool uniform;
-    double G_u, den_u, gbar;             // uniform dy: G and sw*gbar are constants
+    double G_u, inv_den_u, gbar;         // uniform dy: G and 1/(sw*gbar) are constants
     const double* s1; const double* s0;  // prefix sums of this period
     unsigned ctab;                       // shared-space address of the window table
     unsigned part;                       // shared-space address of the [kPartRows][kPartPitch] emit buffer
@@ -90,18 +90,17 @@ struct Cls {
 };
 
 // a5 + a8 for one window kappa of the class (start s = off + kappa*stp): hi/lo are the prefix sums
-// at s+D and s.  a = max(rbar, 0) / mean(g_D) with rbar = swr / sw, taken as ONE division.
+// at s+D and s.  a = max(rbar, 0) / mean(g_D) with rbar = swr / sw.  Uniform dy: sw * mean(g_D) is a
+// constant of the trial, so a = max(swr, 0) * inv_den (one multiply); otherwise one division.
 __device__ __forceinline__ void score_one(const Cls& c, Cand& best, const int s, const double hi1,
                                           const double lo1, const double hi0, const double lo0,
                                           const double C, const double Gt) {
-    const double swr = hi1 - lo1;
-    const double den = c.uniform ? c.den_u : (hi0 - lo0) * c.gbar;
-    const double depth = __ddiv_rn(fmax(swr, 0.0), den);
+    const double swr = fmax(hi1 - lo1, 0.0);
+    const double depth = c.uniform ? swr * c.inv_den_u : __ddiv_rn(swr, (hi0 - lo0) * c.gbar);
     const double Gv = c.uniform ? c.G_u : Gt;
     const double d = -2.0 * depth * C + (depth * depth) * Gv;
-    cand_offer(best, d, s, depth);
+    if (d <= best.d || !best.has) cand_offer(best, d, s, depth);     // rarely taken after the first windows
 }
-
 // Wide path: score the windows [k0, k0 + nWt) of the class from table entries [0, nWt).
 __device__ __forceinline__ void score_wide(const Cls& c, Cand& best, const int lane, const int k0,
                                            const int nWt) {
@@ -473,7 +472,7 @@ __global__ void __launch_bounds__(kRT, 3) k_chi2_ring(TileArgs a, const int* __r
     c.uniform = UNIFORM;
     c.gbar = e.gbar;
     c.G_u = a.w_uniform * e.gg2;
-    c.den_u = ((double)e.D * a.w_uniform) * e.gbar;
+    c.inv_den_u = __ddiv_rn(1.0, ((double)e.D * a.w_uniform) * e.gbar);
     c.s1 = a.s1 + (long long)pl * a.spitch;
     c.s0 = a.s0 + (long long)pl * a.spitch;
     double* const wsm = dsm + warp * kWarpSmem;
