@@ -149,8 +149,7 @@ __global__ void __launch_bounds__(kChiThreads) k_chi2_v1(TileArgs a) {
 }
 
 // a8: per period, first strict minimum over ascending duration index.
-__global__ void __launch_bounds__(128) k_reduce(TileArgs a, const u64* __restrict__ sorted,
-                                                double* __restrict__ out_chi2,
+__global__ void __launch_bounds__(128) k_reduce(TileArgs a, double* __restrict__ out_chi2,
                                                 gtls_best* __restrict__ out_best,
                                                 unsigned long long* __restrict__ counters) {
     const int pl = blockIdx.x * blockDim.x + threadIdx.x;
@@ -172,7 +171,7 @@ __global__ void __launch_bounds__(128) k_reduce(TileArgs a, const u64* __restric
             gtls_best b;
             b.dur_idx = bj; b.start = pp[bj].start; b.depth = pp[bj].depth;
             const int mid = (pp[bj].start + (dd[bj].D - 1) / 2) % a.n;
-            b.t0 = a.t[(u32)sorted[(long long)pl * a.n + mid]];
+            b.t0 = a.t[a.perm[(long long)pl * a.n + mid]];
             out_best[a.p0 + pl] = b;
         }
     }
@@ -232,9 +231,9 @@ void launch_chi2(const TileArgs& a, cudaStream_t st) {
     }
 }
 
-void launch_reduce(const TileArgs& a, const u64* sorted, double* out_chi2, gtls_best* out_best,
+void launch_reduce(const TileArgs& a, double* out_chi2, gtls_best* out_best,
                    unsigned long long* counters, cudaStream_t st) {
-    k_reduce<<<(a.tile + 127) / 128, 128, 0, st>>>(a, sorted, out_chi2, out_best, counters);
+    k_reduce<<<(a.tile + 127) / 128, 128, 0, st>>>(a, out_chi2, out_best, counters);
 }
 
 void launch_window_export(const TileArgs& a, const double* s2, double q, int32_t* out_start,

@@ -222,9 +222,11 @@ __device__ __forceinline__ void reduce_batch(const Cls& c, const It& it, const i
         for (int t = lane; t < it.G * PF; t += 32) {
             const int g = t / PF, sl = t - g * PF;
             const unsigned pr = c.part + (unsigned)((sl * kPartPitch + g * c.stp) * 8);
-            double a0 = 0.0;
-            for (int q = 0; q < c.stp; ++q) a0 += lds64(pr + 8 * q);
-            sts64(it.tab + (unsigned)((g * it.SL + (kwb + sl - kw_base)) * 8), a0);
+            double a0 = 0.0, a1 = 0.0;
+            int q = 0;
+            for (; q + 1 < c.stp; q += 2) { a0 += lds64(pr + 8 * q); a1 += lds64(pr + 8 * q + 8); }
+            if (q < c.stp) a0 += lds64(pr + 8 * q);
+            sts64(it.tab + (unsigned)((g * it.SL + (kwb + sl - kw_base)) * 8), a0 + a1);
         }
     }
     __syncwarp();
@@ -360,7 +362,8 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
         it.narrow = true; it.direct = c.stp == 1;   // (NARROW implies uniform dy and stp <= kChi2NarrowMax)
         it.G = 32 / c.stp;
         it.L = (c.nWr + it.G - 1) / it.G;
-        it.KB = (c.Kt - it.G) / (it.G * MB);
+        it.KB = c.Kt / (it.G * MB);
+        if (it.G * ((it.KB * MB) | 1) > c.Kt) --it.KB;       // odd pitch must still fit (KB >= 1 always)
         it.SLn = it.KB * MB;
         it.SL = it.SLn | 1;
         it.invSL = 1.0f / (float)it.SL;

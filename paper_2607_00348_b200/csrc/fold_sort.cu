@@ -12,6 +12,7 @@ namespace gtls {
 namespace {
 
 __global__ void __launch_bounds__(256) k_fold_keys(TileArgs a, double* __restrict__ phase_out) {
+    if (a.run_if && !*a.run_if) return;
     const long long total = (long long)a.tile * a.n;
     for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < total;
          g += (long long)gridDim.x * blockDim.x) {
@@ -25,8 +26,9 @@ __global__ void __launch_bounds__(256) k_fold_keys(TileArgs a, double* __restric
 // ---- LSD radix pass: per-tile digit histogram ------------------------------------------
 __global__ void __launch_bounds__(kRadixThreads) k_radix_hist(const u64* __restrict__ in,
                                                               u32* __restrict__ counts, int n,
-                                                              int nt, int shift) {
+                                                              int nt, int shift, const int* run_if) {
     __shared__ u32 h[256];
+    if (run_if && !*run_if) return;
     const int tile = blockIdx.x, seg = blockIdx.y;
     h[threadIdx.x] = 0;
     __syncthreads();
@@ -41,7 +43,8 @@ __global__ void __launch_bounds__(kRadixThreads) k_radix_hist(const u64* __restr
 }
 
 // ---- exclusive scan over (digit-major, tile-minor) counts of one segment ------------------
-__global__ void __launch_bounds__(256) k_radix_scan(u32* __restrict__ counts, int nt) {
+__global__ void __launch_bounds__(256) k_radix_scan(u32* __restrict__ counts, int nt, const int* run_if) {
+    if (run_if && !*run_if) return;
     __shared__ u32 s_tot[256];
     const int seg = blockIdx.x, d = threadIdx.x;
     u32* row = counts + ((long long)seg * 256 + d) * nt;
@@ -69,8 +72,9 @@ __global__ void __launch_bounds__(256) k_radix_scan(u32* __restrict__ counts, in
 __global__ void __launch_bounds__(kRadixThreads) k_radix_scatter(const u64* __restrict__ in,
                                                                  u64* __restrict__ out,
                                                                  const u32* __restrict__ counts,
-                                                                 int n, int nt, int shift) {
+                                                                 int n, int nt, int shift, const int* run_if) {
     __shared__ u32 whist[kRadixWarps][256];
+    if (run_if && !*run_if) return;
     const int tile = blockIdx.x, seg = blockIdx.y;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     for (int k = threadIdx.x; k < kRadixWarps * 256; k += kRadixThreads) (&whist[0][0])[k] = 0;
@@ -117,6 +121,7 @@ __global__ void __launch_bounds__(kRadixThreads) k_radix_scatter(const u64* __re
 
 // ---- tie fix-up: order equal-key32 runs by the full fp64 phase (stable) ---------------------
 __global__ void __launch_bounds__(256) k_tie_fixup(TileArgs a, u64* __restrict__ keys) {
+    if (a.run_if && !*a.run_if) return;
     const long long total = (long long)a.tile * a.n;
     for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < total;
          g += (long long)gridDim.x * blockDim.x) {
@@ -140,7 +145,8 @@ __global__ void __launch_bounds__(256) k_tie_fixup(TileArgs a, u64* __restrict__
 }
 
 __global__ void __launch_bounds__(256) k_perm_export(const u64* __restrict__ keys, long long count,
-                                                     int32_t* __restrict__ perm) {
+                                                     int32_t* __restrict__ perm, const int* run_if) {
+    if (run_if && !*run_if) return;
     for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < count;
          g += (long long)gridDim.x * blockDim.x)
         perm[g] = (int32_t)(u32)keys[g];
@@ -166,9 +172,9 @@ u64* launch_phase_sort(const TileArgs& a, cudaStream_t st, int* n_launches) {
     const dim3 grid(nt, a.tile);
     for (int pass = 0; pass < 4; ++pass) {
         const int shift = 32 + 8 * pass;
-        k_radix_hist<<<grid, kRadixThreads, 0, st>>>(src, a.counts, a.n, nt, shift);
-        k_radix_scan<<<a.tile, 256, 0, st>>>(a.counts, nt);
-        k_radix_scatter<<<grid, kRadixThreads, 0, st>>>(src, dst, a.counts, a.n, nt, shift);
+        k_radix_hist<<<grid, kRadixThreads, 0, st>>>(src, a.counts, a.n, nt, shift, a.run_if);
+        k_radix_scan<<<a.tile, 256, 0, st>>>(a.counts, nt, a.run_if);
+        k_radix_scatter<<<grid, kRadixThreads, 0, st>>>(src, dst, a.counts, a.n, nt, shift, a.run_if);
         u64* tmp = src; src = dst; dst = tmp;
     }
     k_tie_fixup<<<grid_for((long long)a.tile * a.n, 256), 256, 0, st>>>(a, src);
@@ -176,8 +182,8 @@ u64* launch_phase_sort(const TileArgs& a, cudaStream_t st, int* n_launches) {
     return src;   // after 4 passes the sorted keys are back in keys_a
 }
 
-void launch_perm_export(const u64* sorted, long long count, int32_t* out_perm, cudaStream_t st) {
-    k_perm_export<<<grid_for(count, 256), 256, 0, st>>>(sorted, count, out_perm);
+void launch_perm_export(const u64* sorted, long long count, int32_t* out_perm, const int* run_if, cudaStream_t st) {
+    k_perm_export<<<grid_for(count, 256), 256, 0, st>>>(sorted, count, out_perm, run_if);
 }
 
 }  // namespace gtls

@@ -66,6 +66,7 @@ Sizes workspace_sizes(long long n, long long n_per, int n_dur, double q_max, boo
               2 * align_up(n_per * sizeof(double)) + align_up(n_per * sizeof(gtls_best)) + 4096;
     s.per_period = 2 * n * sizeof(u64) + 256ull * nt * sizeof(u32) + n_dur * sizeof(DurEntry) +
                    n_dur * sizeof(Partial) + (size_t)kChi2Variants * n_dur * sizeof(int) +
+                   n * sizeof(u32) + (3ull * kMaxBuckets + 1) * sizeof(u32) +
                    (uniform ? 1 : 2) * ((size_t)pitch + spitch) * sizeof(double);
     return s;
 }
@@ -129,6 +130,52 @@ struct CurveDev {
     double *wr = nullptr, *w = nullptr, *wr2 = nullptr;
     CurveInfo* info = nullptr;
 };
+
+
+struct SortScratch { u32* hist; u32* start; u32* cursor; int* fallback; };
+
+bool take_sort_scratch(Arena& ar, size_t tile, int nbk, SortScratch& sc) {
+    sc.hist = ar.take<u32>(tile * nbk);
+    sc.start = ar.take<u32>(tile * (nbk + 1));
+    sc.cursor = ar.take<u32>(tile * nbk);
+    sc.fallback = ar.take<int>(1);
+    return sc.fallback != nullptr;
+}
+
+// Steps a1-a4 for the tile described by `a` (a.perm, a.x1/s1[/x0/s0] are outputs): the bucket fast
+// path, then the LSD radix path, whose kernels return at once unless the fast path raised its
+// fallback flag (a bucket larger than kBucketCap).  sort_only: permutation only.
+void run_fold_sort_scan(TileArgs& a, const SortScratch& sc, double* x2, double* s2, int pad_override,
+                        bool sort_only, double* phase_out, cudaStream_t st, int* launches) {
+    static const bool force_lsd = [] { const char* e = getenv("GTLS_SORT"); return e && strcmp(e, "lsd") == 0; }();
+    BucketArgs b;
+    memset(&b, 0, sizeof(b));
+    b.n = a.n; b.tile = a.tile; b.p0 = a.p0; b.n_dur = a.n_dur; b.pad_override = pad_override;
+    b.nbk = bucket_count_for(a.n);
+    int lg = 0; while ((1 << lg) < b.nbk) ++lg;
+    b.shift = 32 - lg;
+    b.pitch = a.pitch; b.spitch = a.spitch;
+    b.t = a.t; b.wr = a.wr; b.w = a.w; b.wr2 = a.wr2; b.periods = a.periods; b.durtab = a.durtab;
+    b.hist = sc.hist; b.start = sc.start; b.cursor = sc.cursor; b.fallback = sc.fallback;
+    b.force_fallback = force_lsd ? 1 : 0;
+    b.keys = a.keys_b; b.perm = a.perm;
+    b.x1 = a.x1; b.s1 = a.s1; b.x0 = a.x0; b.s0 = a.s0; b.x2 = x2; b.s2 = s2;
+    const bool has2 = s2 != nullptr, has0 = !a.uniform || has2;
+    launch_bucket_sort(b, has0, has2, sort_only, st);
+    if (phase_out) {                       // phases are exported by the fold kernel of the LSD path
+        a.run_if = nullptr;
+        launch_fold_keys(a, phase_out, st);
+        if (launches) *launches += 1;
+    }
+    a.run_if = sc.fallback;
+    launch_fold_keys(a, nullptr, st);
+    int l2 = 0;
+    const u64* sorted = launch_phase_sort(a, st, &l2);
+    if (!sort_only) launch_gather_scan(a, sorted, x2, s2, pad_override, st);
+    launch_perm_export(sorted, (long long)a.tile * a.n, (int32_t*)a.perm, a.run_if, st);
+    a.run_if = nullptr;
+    if (launches) *launches += 6 + 1 + l2 + (sort_only ? 0 : 1) + 1;   // memsets + 4 bucket kernels count as 6
+}
 
 }  // namespace
 
@@ -273,6 +320,9 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     a.keys_a = ws.take<u64>((size_t)tile * n);
     a.keys_b = ws.take<u64>((size_t)tile * n);
     a.counts = ws.take<u32>((size_t)tile * 256 * nt);
+    a.perm = ws.take<u32>((size_t)tile * n);
+    SortScratch ssc;
+    if (!take_sort_scratch(ws, (size_t)tile, bucket_count_for((int)n), ssc)) return GTLS_ENOMEM;
     a.durtab = ws.take<DurEntry>((size_t)tile * n_dur);
     a.partial = ws.take<Partial>((size_t)tile * n_dur);
     a.trial_list = ws.take<int>((size_t)kChi2Variants * tile * n_dur);
@@ -299,17 +349,15 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
         tm.mark(0);
         launch_durtab(a, st);
         tm.mark(1);
-        launch_fold_keys(a, nullptr, st);
         tm.mark(2);
-        const u64* sorted = launch_phase_sort(a, st, &launches);
+        run_fold_sort_scan(a, ssc, nullptr, nullptr, -1, false, nullptr, st, &launches);
         tm.mark(3);
-        launch_gather_scan(a, sorted, nullptr, nullptr, -1, st);
         tm.mark(4);
         if (use_v1) launch_chi2(a, st); else if (use_rows) launch_chi2_rows(a, st); else launch_chi2_ring(a, st);
         tm.mark(5);
-        launch_reduce(a, sorted, d_chi2, d_best, d_counters, st);
+        launch_reduce(a, d_chi2, d_best, d_counters, st);
         tm.mark(6);
-        stats.kernel_launches += launches + 4 + ((use_v1 || use_rows) ? 1 : 1 + (uniform ? kChi2Variants : kChi2Variants / 2));
+        stats.kernel_launches += launches + 2 + ((use_v1 || use_rows) ? 1 : 1 + (uniform ? kChi2Variants : kChi2Variants / 2));
         stats.chi2_launches += 1;
         if (o.stats) {
             CU(cudaStreamSynchronize(st));
@@ -385,14 +433,16 @@ int gtls_fold_sort(const double* t, int64_t n, const double* periods, int64_t n_
     cudaStream_t st = (cudaStream_t)o.stream;
     const bool dev = o.pointers_on_device != 0;
     const int nt = (int)((n + kRadixTile - 1) / kRadixTile);
-    const size_t per_period = 2 * n * sizeof(u64) + 256ull * nt * sizeof(u32) +
+    const int nbk = bucket_count_for((int)n);
+    const size_t per_period = 2 * n * sizeof(u64) + 256ull * nt * sizeof(u32) + n * sizeof(u32) +
+                              (3ull * nbk + 1) * sizeof(u32) +
                               (dev ? 0 : n * (sizeof(double) + sizeof(int32_t))) + 1024;
     long long tile = (long long)((1ull << 30) / per_period);
     if (o.period_tile > 0) tile = o.period_tile;
     if (tile > n_per) tile = n_per;
     if (tile < 1) tile = 1;
     Arena ar;
-    int rc = alloc_arena(ar, align_up(n * 8) + align_up(n_per * 8) + tile * align_up(per_period) + 16 * 256);
+    int rc = alloc_arena(ar, align_up(n * 8) + align_up(n_per * 8) + tile * align_up(per_period) + 32 * 256);
     if (rc) return rc;
     const double *d_t, *d_per;
     if ((rc = stage_in(t, n, dev, ar, st, &d_t))) return rc;
@@ -403,6 +453,8 @@ int gtls_fold_sort(const double* t, int64_t n, const double* periods, int64_t n_
     a.keys_a = ar.take<u64>((size_t)tile * n);
     a.keys_b = ar.take<u64>((size_t)tile * n);
     a.counts = ar.take<u32>((size_t)tile * 256 * nt);
+    SortScratch ssc;
+    if (!take_sort_scratch(ar, (size_t)tile, nbk, ssc)) return GTLS_ENOMEM;
     double* d_phase = dev ? nullptr : (out_phase ? ar.take<double>((size_t)tile * n) : nullptr);
     int32_t* d_perm = dev ? nullptr : ar.take<int32_t>((size_t)tile * n);
     if (!a.counts || (!dev && !d_perm)) return GTLS_ENOMEM;
@@ -412,9 +464,8 @@ int gtls_fold_sort(const double* t, int64_t n, const double* periods, int64_t n_
         const size_t cnt = (size_t)a.tile * n;
         double* ph = dev ? (out_phase ? out_phase + p0 * n : nullptr) : d_phase;
         int32_t* pm = dev ? out_perm + p0 * n : d_perm;
-        launch_fold_keys(a, ph, st);
-        const u64* sorted = launch_phase_sort(a, st, nullptr);
-        launch_perm_export(sorted, (long long)cnt, pm, st);
+        a.perm = (u32*)pm;
+        run_fold_sort_scan(a, ssc, nullptr, nullptr, 0, true, ph, st, nullptr);
         if (!dev) {
             if (out_phase) CU(cudaMemcpyAsync(out_phase + p0 * n, ph, cnt * sizeof(double), cudaMemcpyDeviceToHost, st));
             CU(cudaMemcpyAsync(out_perm + p0 * n, pm, cnt * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
@@ -435,7 +486,7 @@ static int one_period_scan(const double* t, const double* y, const double* dy, i
     const bool dev = o.pointers_on_device != 0;
     const int nt = (int)((n + kRadixTile - 1) / kRadixTile);
     const int pitch = (int)((n + pad + 7) / 8 * 8), spitch = pitch + 8;
-    size_t bytes = 8 * align_up(n * 8) + 2 * align_up(n * sizeof(u64)) + align_up(256ull * nt * 4) +
+    size_t bytes = 9 * align_up(n * 8) + 2 * align_up(n * sizeof(u64)) + align_up(256ull * nt * 4) + 8192 +
                    3 * align_up((size_t)pitch * 8) + 3 * align_up((size_t)spitch * 8) +
                    6 * align_up((size_t)n * 8) + 64 * 256;
     int rc = alloc_arena(ar, bytes);
@@ -461,14 +512,15 @@ static int one_period_scan(const double* t, const double* y, const double* dy, i
     a.periods = d_period; a.chi2_0 = &d_info->chi2_0; a.pitch = pitch; a.spitch = spitch;
     a.dt0 = o.dt0; a.uniform = 0;
     a.keys_a = ar.take<u64>(n); a.keys_b = ar.take<u64>(n); a.counts = ar.take<u32>(256ull * nt);
+    a.perm = ar.take<u32>(n);
+    SortScratch ssc;
+    if (!take_sort_scratch(ar, 1, bucket_count_for((int)n), ssc)) return GTLS_ENOMEM;
     a.x1 = ar.take<double>(pitch); a.x0 = ar.take<double>(pitch);
     double* x2 = ar.take<double>(pitch);
     a.s1 = ar.take<double>(spitch); a.s0 = ar.take<double>(spitch);
     *d_s2 = ar.take<double>(spitch);
     if (!*d_s2) return GTLS_ENOMEM;
-    launch_fold_keys(a, nullptr, st);
-    const u64* sorted = launch_phase_sort(a, st, nullptr);
-    launch_gather_scan(a, sorted, x2, *d_s2, (int)pad, st);
+    run_fold_sort_scan(a, ssc, x2, *d_s2, (int)pad, false, nullptr, st, nullptr);
     return GTLS_OK;
 }
 

@@ -44,6 +44,11 @@ struct CurveInfo {
 constexpr int kChi2Variants = 10;
 constexpr int kChi2NarrowMax = 16;   // largest class stride handled by the narrow variants
 
+// bucket sort (bucket_sort.cu)
+constexpr int kMaxBuckets = 256;      // buckets per period (power of two)
+constexpr int kBucketTarget = 1536;   // aimed-at mean bucket size
+constexpr int kBucketCap = 4096;      // largest bucket the shared-memory sort takes; beyond: LSD fallback
+
 constexpr int kRadixThreads = 256;
 constexpr int kRadixItems = 8;
 constexpr int kRadixTile = kRadixThreads * kRadixItems;   // 2048 keys per CTA
@@ -118,10 +123,33 @@ struct TileArgs {
     double* x1; double* x0;   // [tile*pitch]
     double* s1; double* s0;   // [tile*spitch]
     Partial* partial;      // [tile*n_dur]
+    u32* perm;             // [tile*n]   sorted position -> input index
+    const int* run_if;     // LSD fallback kernels run only when *run_if != 0 (nullptr: always)
     int* trial_list;       // [kChi2Variants][tile*n_dur] trial indices binned by chi2 kernel variant
     int* trial_count;      // [kChi2Variants]
     int dbg_min_st, dbg_max_st;   // timing experiments only (GTLS_DBG_MIN_ST / GTLS_DBG_MAX_ST): skip other trials
 };
+
+// Arguments of the fused fold / bucket sort / gather / scan fast path (bucket_sort.cu).
+struct BucketArgs {
+    int n, tile, nbk, shift;   // points, periods in the tile, buckets per period, 32 - log2(nbk)
+    long long p0;
+    int n_dur, pad_override;   // pad = max D of the period's durtab row unless pad_override >= 0
+    int pitch, spitch;
+    const double* t; const double* wr; const double* w; const double* wr2;
+    const double* periods;
+    const DurEntry* durtab;
+    u32* hist;                 // [tile*nbk]
+    u32* start;                // [tile*(nbk+1)]
+    u32* cursor;               // [tile*nbk]
+    int* fallback;             // device flag: some bucket exceeded kBucketCap
+    int force_fallback;        // GTLS_SORT=lsd: raise the flag regardless (tests of the LSD path)
+    u64* keys;                 // [tile*n] bucketed keys
+    u32* perm;                 // [tile*n]
+    double* x1; double* s1; double* x0; double* s0; double* x2; double* s2;
+};
+int bucket_count_for(int n);
+void launch_bucket_sort(const BucketArgs& b, bool has0, bool has2, bool sort_only, cudaStream_t st);
 
 void launch_curve_pre(const double* t, const double* y, const double* dy, int n, double* wr,
                       double* w, double* wr2, CurveInfo* info, cudaStream_t st);
@@ -139,11 +167,11 @@ void launch_chi2(const TileArgs& a, cudaStream_t st);        // v1: warp per win
 void launch_chi2_rows(const TileArgs& a, cudaStream_t st);   // register-tiled rows kernel (A-B)
 void launch_chi2_ring(const TileArgs& a, cudaStream_t st);   // register-ring correlation kernel (default)
 // counters[0] += windows of all trials, counters[1] += sum of D over evaluated windows
-void launch_reduce(const TileArgs& a, const u64* sorted, double* out_chi2, gtls_best* out_best,
+void launch_reduce(const TileArgs& a, double* out_chi2, gtls_best* out_best,
                    unsigned long long* counters, cudaStream_t st);
 void launch_window_export(const TileArgs& a, const double* s2, double q, int32_t* out_start,
                           double* out_depth, double* out_c_out, double* out_c_in, cudaStream_t st);
-void launch_perm_export(const u64* sorted, long long count, int32_t* out_perm, cudaStream_t st);
+void launch_perm_export(const u64* sorted, long long count, int32_t* out_perm, const int* run_if, cudaStream_t st);
 
 struct SdeScratch {      // device scalars of the epilogue
     double chi2_min, mean_sr, sd_sr, sde_raw_best, sde_max;

@@ -26,6 +26,7 @@ __global__ void __launch_bounds__(kScanThreads) k_gather_scan(TileArgs a, const 
                                                               int pad_override) {
     __shared__ double s_w[3][32];
     __shared__ double s_carry[3];
+    if (a.run_if && !*a.run_if) return;
     const int pl = blockIdx.x;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     int pad = pad_override;
