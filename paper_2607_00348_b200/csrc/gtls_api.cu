@@ -66,7 +66,7 @@ Sizes workspace_sizes(long long n, long long n_per, int n_dur, double q_max, boo
               2 * align_up(n_per * sizeof(double)) + align_up(n_per * sizeof(gtls_best)) + 4096;
     s.per_period = 2 * n * sizeof(u64) + 256ull * nt * sizeof(u32) + n_dur * sizeof(DurEntry) +
                    n_dur * sizeof(Partial) + (size_t)kChi2Variants * n_dur * sizeof(int) +
-                   n * sizeof(u32) + (3ull * kMaxBuckets + 1) * sizeof(u32) +
+                   n * sizeof(u32) + (4ull * kMaxBuckets + 1) * sizeof(u32) + 3ull * kMaxBuckets * sizeof(double) +
                    (uniform ? 1 : 2) * ((size_t)pitch + spitch) * sizeof(double);
     return s;
 }
@@ -132,14 +132,16 @@ struct CurveDev {
 };
 
 
-struct SortScratch { u32* hist; u32* start; u32* cursor; int* fallback; };
+struct SortScratch { u32* hist; u32* start; u32* cursor; int* fallback; double* prefix; int* flag; };
 
 bool take_sort_scratch(Arena& ar, size_t tile, int nbk, SortScratch& sc) {
     sc.hist = ar.take<u32>(tile * nbk);
     sc.start = ar.take<u32>(tile * (nbk + 1));
     sc.cursor = ar.take<u32>(tile * nbk);
     sc.fallback = ar.take<int>(1);
-    return sc.fallback != nullptr;
+    sc.prefix = ar.take<double>(tile * nbk * 3);
+    sc.flag = ar.take<int>(tile * nbk);
+    return sc.flag != nullptr;
 }
 
 // Steps a1-a4 for the tile described by `a` (a.perm, a.x1/s1[/x0/s0] are outputs): the bucket fast
@@ -157,6 +159,7 @@ void run_fold_sort_scan(TileArgs& a, const SortScratch& sc, double* x2, double* 
     b.pitch = a.pitch; b.spitch = a.spitch;
     b.t = a.t; b.wr = a.wr; b.w = a.w; b.wr2 = a.wr2; b.periods = a.periods; b.durtab = a.durtab;
     b.hist = sc.hist; b.start = sc.start; b.cursor = sc.cursor; b.fallback = sc.fallback;
+    b.prefix = sc.prefix; b.flag = sc.flag;
     b.force_fallback = force_lsd ? 1 : 0;
     b.keys = a.keys_b; b.perm = a.perm;
     b.x1 = a.x1; b.s1 = a.s1; b.x0 = a.x0; b.s0 = a.s0; b.x2 = x2; b.s2 = s2;
@@ -174,7 +177,7 @@ void run_fold_sort_scan(TileArgs& a, const SortScratch& sc, double* x2, double* 
     if (!sort_only) launch_gather_scan(a, sorted, x2, s2, pad_override, st);
     launch_perm_export(sorted, (long long)a.tile * a.n, (int32_t*)a.perm, a.run_if, st);
     a.run_if = nullptr;
-    if (launches) *launches += 6 + 1 + l2 + (sort_only ? 0 : 1) + 1;   // memsets + 4 bucket kernels count as 6
+    if (launches) *launches += (sort_only ? 4 : 5) + 1 + l2 + (sort_only ? 0 : 1) + 1;   // kernels only (memsets not counted)
 }
 
 }  // namespace
@@ -435,7 +438,7 @@ int gtls_fold_sort(const double* t, int64_t n, const double* periods, int64_t n_
     const int nt = (int)((n + kRadixTile - 1) / kRadixTile);
     const int nbk = bucket_count_for((int)n);
     const size_t per_period = 2 * n * sizeof(u64) + 256ull * nt * sizeof(u32) + n * sizeof(u32) +
-                              (3ull * nbk + 1) * sizeof(u32) +
+                              (4ull * nbk + 1) * sizeof(u32) + 3ull * nbk * sizeof(double) +
                               (dev ? 0 : n * (sizeof(double) + sizeof(int32_t))) + 1024;
     long long tile = (long long)((1ull << 30) / per_period);
     if (o.period_tile > 0) tile = o.period_tile;
@@ -486,7 +489,7 @@ static int one_period_scan(const double* t, const double* y, const double* dy, i
     const bool dev = o.pointers_on_device != 0;
     const int nt = (int)((n + kRadixTile - 1) / kRadixTile);
     const int pitch = (int)((n + pad + 7) / 8 * 8), spitch = pitch + 8;
-    size_t bytes = 9 * align_up(n * 8) + 2 * align_up(n * sizeof(u64)) + align_up(256ull * nt * 4) + 8192 +
+    size_t bytes = 9 * align_up(n * 8) + 2 * align_up(n * sizeof(u64)) + align_up(256ull * nt * 4) + 32768 +
                    3 * align_up((size_t)pitch * 8) + 3 * align_up((size_t)spitch * 8) +
                    6 * align_up((size_t)n * 8) + 64 * 256;
     int rc = alloc_arena(ar, bytes);

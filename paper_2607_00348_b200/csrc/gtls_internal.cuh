@@ -46,8 +46,8 @@ constexpr int kChi2NarrowMax = 16;   // largest class stride handled by the narr
 
 // bucket sort (bucket_sort.cu)
 constexpr int kMaxBuckets = 256;      // buckets per period (power of two)
-constexpr int kBucketTarget = 1536;   // aimed-at mean bucket size
-constexpr int kBucketCap = 4096;      // largest bucket the shared-memory sort takes; beyond: LSD fallback
+constexpr int kBucketTarget = 1100;   // aimed-at mean bucket size
+constexpr int kBucketCap = 2048;      // largest bucket the shared-memory sort takes; beyond: LSD fallback
 
 constexpr int kRadixThreads = 256;
 constexpr int kRadixItems = 8;
@@ -143,6 +143,8 @@ struct BucketArgs {
     u32* start;                // [tile*(nbk+1)]
     u32* cursor;               // [tile*nbk]
     int* fallback;             // device flag: some bucket exceeded kBucketCap
+    double* prefix;            // [tile*nbk*3] inclusive prefix of (w r, w, w r^2) per bucket (look-back)
+    int* flag;                 // [tile*nbk]   prefix published
     int force_fallback;        // GTLS_SORT=lsd: raise the flag regardless (tests of the LSD path)
     u64* keys;                 // [tile*n] bucketed keys
     u32* perm;                 // [tile*n]
