@@ -77,7 +77,7 @@ __global__ void __launch_bounds__(256) k_bucket_scan(BucketArgs b) {
     if (lane == 0) start[b.nbk] = carry;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) big = max(big, __shfl_xor_sync(0xffffffffu, big, o));
-    if (lane == 0 && (big > (u32)kBucketCap || b.force_fallback)) atomicExch(b.fallback, 1);
+    if (lane == 0 && big > (u32)kBucketCap) atomicExch(b.fallback, 1);
 }
 
 __global__ void __launch_bounds__(kCountThreads) k_bucket_scatter(BucketArgs b) {
@@ -122,11 +122,6 @@ __device__ __forceinline__ bool key_less(const u64 a, const u64 b, const double*
     return (u32)a < (u32)b;
 }
 
-__device__ __forceinline__ int ld_acquire(const int* p) {
-    int v;
-    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
 __device__ __forceinline__ void st_release(int* p, int v) {
     asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
@@ -196,10 +191,12 @@ __global__ void __launch_bounds__(kFinThreads) k_bucket_finish(BucketArgs b) {
         A[r] = k;
     }
     __syncthreads();
-    // 6. the bucket is sorted: permutation
+    // 6. the bucket is sorted: permutation (written below, while warp 0 looks back)
     u32* perm = b.perm + (long long)pl * b.n + bs;
-    for (int i = tid; i < m; i += kFinThreads) perm[i] = (u32)A[i];
-    if (SORT_ONLY) return;
+    if (SORT_ONLY) {
+        for (int i = tid; i < m; i += kFinThreads) perm[i] = (u32)A[i];
+        return;
+    }
 
     // 7. gather + local inclusive scan: thread owns kFinItems consecutive sorted entries
     double v1[kFinItems], v0[kFinItems], v2[kFinItems];
@@ -217,14 +214,9 @@ __global__ void __launch_bounds__(kFinThreads) k_bucket_finish(BucketArgs b) {
     double* x1 = b.x1 + (long long)pl * b.pitch + bs;
     double* x0 = HAS0 ? b.x0 + (long long)pl * b.pitch + bs : nullptr;
     double* x2 = HAS2 ? b.x2 + (long long)pl * b.pitch + bs : nullptr;
+    double r1[kFinItems], r0[kFinItems], r2[kFinItems];          // the gathered values themselves
 #pragma unroll
-    for (int e = 0; e < kFinItems; ++e) {
-        if (first + e < m) {
-            x1[first + e] = v1[e];
-            if (HAS0) x0[first + e] = v0[e];
-            if (HAS2) x2[first + e] = v2[e];
-        }
-    }
+    for (int e = 0; e < kFinItems; ++e) { r1[e] = v1[e]; r0[e] = v0[e]; r2[e] = v2[e]; }
 #pragma unroll
     for (int e = 1; e < kFinItems; ++e) {
         v1[e] += v1[e - 1];
@@ -249,16 +241,31 @@ __global__ void __launch_bounds__(kFinThreads) k_bucket_finish(BucketArgs b) {
         double tot1 = 0.0, tot0 = 0.0, tot2 = 0.0;
 #pragma unroll
         for (int k = 0; k < NW; ++k) { tot1 += s_w[0][k]; tot0 += s_w[1][k]; tot2 += s_w[2][k]; }
-        agg[bk * 3] = tot1; agg[bk * 3 + 1] = tot0; agg[bk * 3 + 2] = tot2;
+        __stcg(agg + bk * 3, tot1); __stcg(agg + bk * 3 + 1, tot0); __stcg(agg + bk * 3 + 2, tot2);
+        __threadfence();
         st_release(flag + bk, 1);
     }
     if (warp == 0) {
+        // poll the earlier buckets' flags with independent relaxed loads, one acquire fence, then the sums
+        for (int j0 = 0; j0 < bk; j0 += 128) {
+            bool ready;
+            do {
+                int f = 1;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const int j = j0 + lane + 32 * q;
+                    if (j < bk) f &= *((volatile const int*)(flag + j));
+                }
+                ready = __all_sync(0xffffffffu, f != 0);
+                if (!ready) __nanosleep(100);
+            } while (!ready);
+        }
+        __threadfence();
         double a1 = 0.0, a0 = 0.0, a2 = 0.0;
         for (int j = lane; j < bk; j += 32) {
-            while (ld_acquire(flag + j) == 0) __nanosleep(40);
-            a1 += agg[j * 3];
-            if (HAS0) a0 += agg[j * 3 + 1];
-            if (HAS2) a2 += agg[j * 3 + 2];
+            a1 += __ldcg(agg + j * 3);
+            if (HAS0) a0 += __ldcg(agg + j * 3 + 1);
+            if (HAS2) a2 += __ldcg(agg + j * 3 + 2);
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
@@ -267,6 +274,17 @@ __global__ void __launch_bounds__(kFinThreads) k_bucket_finish(BucketArgs b) {
             a2 += __shfl_xor_sync(0xffffffffu, a2, o);
         }
         if (lane == 0) { s_base[0] = a1; s_base[1] = a0; s_base[2] = a2; }
+    } else {
+        // meanwhile the other warps write what does not depend on the base
+        for (int i = tid - 32; i < m; i += kFinThreads - 32) perm[i] = (u32)A[i];
+    }
+#pragma unroll
+    for (int e = 0; e < kFinItems; ++e) {
+        if (first + e < m) {
+            x1[first + e] = r1[e];
+            if (HAS0) x0[first + e] = r0[e];
+            if (HAS2) x2[first + e] = r2[e];
+        }
     }
     __syncthreads();
     double w1 = s_base[0], w0 = s_base[1], w2 = s_base[2];     // + totals of the warps before mine
@@ -368,7 +386,6 @@ int bucket_count_for(int n) {
 void launch_bucket_sort(const BucketArgs& b, bool has0, bool has2, bool sort_only, cudaStream_t st) {
     cudaMemsetAsync(b.hist, 0, (size_t)b.tile * b.nbk * sizeof(u32), st);
     cudaMemsetAsync(b.flag, 0, (size_t)b.tile * b.nbk * sizeof(int), st);
-    cudaMemsetAsync(b.fallback, 0, sizeof(int), st);
     const dim3 grid((b.n + kCountThreads * kCountItems - 1) / (kCountThreads * kCountItems), b.tile);
     k_bucket_count<<<grid, kCountThreads, 0, st>>>(b);
     k_bucket_scan<<<(b.tile * 32 + 255) / 256, 256, 0, st>>>(b);

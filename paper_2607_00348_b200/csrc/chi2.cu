@@ -171,7 +171,8 @@ __global__ void __launch_bounds__(128) k_reduce(TileArgs a, double* __restrict__
             gtls_best b;
             b.dur_idx = bj; b.start = pp[bj].start; b.depth = pp[bj].depth;
             const int mid = (pp[bj].start + (dd[bj].D - 1) / 2) % a.n;
-            b.t0 = a.t[a.perm[(long long)pl * a.n + mid]];
+            const u32 src = a.perm[(long long)pl * a.n + mid];
+            b.t0 = a.t[src < (u32)a.n ? src : 0u];      // (a tile whose bucket sort overflowed is recomputed)
             out_best[a.p0 + pl] = b;
         }
     }

@@ -144,40 +144,52 @@ bool take_sort_scratch(Arena& ar, size_t tile, int nbk, SortScratch& sc) {
     return sc.flag != nullptr;
 }
 
-// Steps a1-a4 for the tile described by `a` (a.perm, a.x1/s1[/x0/s0] are outputs): the bucket fast
-// path, then the LSD radix path, whose kernels return at once unless the fast path raised its
-// fallback flag (a bucket larger than kBucketCap).  sort_only: permutation only.
+bool force_lsd_sort() {
+    static const bool f = [] { const char* e = getenv("GTLS_SORT"); return e && strcmp(e, "lsd") == 0; }();
+    return f;
+}
+
+// Steps a1-a4 for the tile described by `a` (a.perm, a.x1/s1[/x0/s0] are outputs).
+//   use_lsd == false: the bucket fast path.  A bucket larger than kBucketCap (clustered phases) raises
+//     the sticky device flag sc.fallback; the caller reads it once at the end and, if set, repeats the
+//     whole call with use_lsd == true.
+//   use_lsd == true: the LSD radix path (fold_sort.cu + scan.cu), any phase distribution.
+// sort_only: permutation only.  phase_out: also export the phases (Eq. 10).
 void run_fold_sort_scan(TileArgs& a, const SortScratch& sc, double* x2, double* s2, int pad_override,
-                        bool sort_only, double* phase_out, cudaStream_t st, int* launches) {
-    static const bool force_lsd = [] { const char* e = getenv("GTLS_SORT"); return e && strcmp(e, "lsd") == 0; }();
-    BucketArgs b;
-    memset(&b, 0, sizeof(b));
-    b.n = a.n; b.tile = a.tile; b.p0 = a.p0; b.n_dur = a.n_dur; b.pad_override = pad_override;
-    b.nbk = bucket_count_for(a.n);
-    int lg = 0; while ((1 << lg) < b.nbk) ++lg;
-    b.shift = 32 - lg;
-    b.pitch = a.pitch; b.spitch = a.spitch;
-    b.t = a.t; b.wr = a.wr; b.w = a.w; b.wr2 = a.wr2; b.periods = a.periods; b.durtab = a.durtab;
-    b.hist = sc.hist; b.start = sc.start; b.cursor = sc.cursor; b.fallback = sc.fallback;
-    b.prefix = sc.prefix; b.flag = sc.flag;
-    b.force_fallback = force_lsd ? 1 : 0;
-    b.keys = a.keys_b; b.perm = a.perm;
-    b.x1 = a.x1; b.s1 = a.s1; b.x0 = a.x0; b.s0 = a.s0; b.x2 = x2; b.s2 = s2;
-    const bool has2 = s2 != nullptr, has0 = !a.uniform || has2;
-    launch_bucket_sort(b, has0, has2, sort_only, st);
-    if (phase_out) {                       // phases are exported by the fold kernel of the LSD path
-        a.run_if = nullptr;
-        launch_fold_keys(a, phase_out, st);
-        if (launches) *launches += 1;
+                        bool sort_only, double* phase_out, bool use_lsd, cudaStream_t st, int* launches) {
+    a.run_if = nullptr;
+    if (!use_lsd) {
+        BucketArgs b;
+        memset(&b, 0, sizeof(b));
+        b.n = a.n; b.tile = a.tile; b.p0 = a.p0; b.n_dur = a.n_dur; b.pad_override = pad_override;
+        b.nbk = bucket_count_for(a.n);
+        int lg = 0; while ((1 << lg) < b.nbk) ++lg;
+        b.shift = 32 - lg;
+        b.pitch = a.pitch; b.spitch = a.spitch;
+        b.t = a.t; b.wr = a.wr; b.w = a.w; b.wr2 = a.wr2; b.periods = a.periods; b.durtab = a.durtab;
+        b.hist = sc.hist; b.start = sc.start; b.cursor = sc.cursor; b.fallback = sc.fallback;
+        b.prefix = sc.prefix; b.flag = sc.flag;
+        b.keys = a.keys_b; b.perm = a.perm;
+        b.x1 = a.x1; b.s1 = a.s1; b.x0 = a.x0; b.s0 = a.s0; b.x2 = x2; b.s2 = s2;
+        const bool has2 = s2 != nullptr, has0 = !a.uniform || has2;
+        launch_bucket_sort(b, has0, has2, sort_only, st);
+        if (phase_out) launch_fold_keys(a, phase_out, st);     // phases come from the LSD path's fold kernel
+        if (launches) *launches += (sort_only ? 4 : 5) + (phase_out ? 1 : 0);
+        return;
     }
-    a.run_if = sc.fallback;
-    launch_fold_keys(a, nullptr, st);
+    launch_fold_keys(a, phase_out, st);
     int l2 = 0;
     const u64* sorted = launch_phase_sort(a, st, &l2);
     if (!sort_only) launch_gather_scan(a, sorted, x2, s2, pad_override, st);
-    launch_perm_export(sorted, (long long)a.tile * a.n, (int32_t*)a.perm, a.run_if, st);
-    a.run_if = nullptr;
-    if (launches) *launches += (sort_only ? 4 : 5) + 1 + l2 + (sort_only ? 0 : 1) + 1;   // kernels only (memsets not counted)
+    launch_perm_export(sorted, (long long)a.tile * a.n, (int32_t*)a.perm, nullptr, st);
+    if (launches) *launches += 1 + l2 + (sort_only ? 0 : 1) + 1;
+}
+
+// reads the sticky fallback flag (synchronises the stream)
+int read_fallback(const SortScratch& sc, cudaStream_t st, int* out) {
+    CU(cudaMemcpyAsync(out, sc.fallback, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return GTLS_OK;
 }
 
 }  // namespace
@@ -344,6 +356,14 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     const bool use_rows = kenv && strcmp(kenv, "rows") == 0;
     a.dbg_min_st = getenv("GTLS_DBG_MIN_ST") ? atoi(getenv("GTLS_DBG_MIN_ST")) : 0;
     a.dbg_max_st = getenv("GTLS_DBG_MAX_ST") ? atoi(getenv("GTLS_DBG_MAX_ST")) : 0x7fffffff;
+    SdeScratch sc;
+    unsigned long long counters[2];
+    const gtls_stats stats0 = stats;
+    for (int attempt = 0; attempt < 2; ++attempt) {
+    const bool use_lsd = force_lsd_sort() || attempt == 1;
+    stats = stats0;
+    CU(cudaMemsetAsync(ssc.fallback, 0, sizeof(int), st));
+    CU(cudaMemsetAsync(d_counters, 0, 2 * sizeof(unsigned long long), st));
     // ---- period tiles ----------------------------------------------------------------------
     for (long long p0 = 0; p0 < n_per; p0 += tile) {
         a.p0 = p0;
@@ -353,7 +373,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
         launch_durtab(a, st);
         tm.mark(1);
         tm.mark(2);
-        run_fold_sort_scan(a, ssc, nullptr, nullptr, -1, false, nullptr, st, &launches);
+        run_fold_sort_scan(a, ssc, nullptr, nullptr, -1, false, nullptr, use_lsd, st, &launches);
         tm.mark(3);
         tm.mark(4);
         if (use_v1) launch_chi2(a, st); else if (use_rows) launch_chi2_rows(a, st); else launch_chi2_ring(a, st);
@@ -376,14 +396,16 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     launch_sde(d_chi2, n_per, o.sde_kernel, d_sde_raw, d_sde, d_sde_sc, st, &launches);
     stats.kernel_launches += launches;
     tm.mark(1);
-    SdeScratch sc;
-    unsigned long long counters[2];
+    int fell_back = 0;
     CU(cudaMemcpyAsync(&sc, d_sde_sc, sizeof(sc), cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(counters, d_counters, sizeof(counters), cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(&fell_back, ssc.fallback, sizeof(int), cudaMemcpyDeviceToHost, st));
     if (o.stats) cudaEventRecord(ev_end, st);
     CU(cudaStreamSynchronize(st));
     CU(cudaGetLastError());
     if (o.stats) stats.ms_epilogue = tm.ms(0, 1);
+    if (use_lsd || !fell_back) break;      // a bucket overflowed: repeat the search on the LSD sort path
+    }
 
     if (out_summary) {
         gtls_best b;
@@ -468,7 +490,13 @@ int gtls_fold_sort(const double* t, int64_t n, const double* periods, int64_t n_
         double* ph = dev ? (out_phase ? out_phase + p0 * n : nullptr) : d_phase;
         int32_t* pm = dev ? out_perm + p0 * n : d_perm;
         a.perm = (u32*)pm;
-        run_fold_sort_scan(a, ssc, nullptr, nullptr, 0, true, ph, st, nullptr);
+        CU(cudaMemsetAsync(ssc.fallback, 0, sizeof(int), st));
+        int fell_back = 0;
+        if (!force_lsd_sort()) {
+            run_fold_sort_scan(a, ssc, nullptr, nullptr, 0, true, ph, false, st, nullptr);
+            if ((rc = read_fallback(ssc, st, &fell_back))) return rc;
+        }
+        if (force_lsd_sort() || fell_back) run_fold_sort_scan(a, ssc, nullptr, nullptr, 0, true, ph, true, st, nullptr);
         if (!dev) {
             if (out_phase) CU(cudaMemcpyAsync(out_phase + p0 * n, ph, cnt * sizeof(double), cudaMemcpyDeviceToHost, st));
             CU(cudaMemcpyAsync(out_perm + p0 * n, pm, cnt * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
@@ -523,7 +551,13 @@ static int one_period_scan(const double* t, const double* y, const double* dy, i
     a.s1 = ar.take<double>(spitch); a.s0 = ar.take<double>(spitch);
     *d_s2 = ar.take<double>(spitch);
     if (!*d_s2) return GTLS_ENOMEM;
-    run_fold_sort_scan(a, ssc, x2, *d_s2, (int)pad, false, nullptr, st, nullptr);
+    CU(cudaMemsetAsync(ssc.fallback, 0, sizeof(int), st));
+    int fell_back = 0, rc2 = 0;
+    if (!force_lsd_sort()) {
+        run_fold_sort_scan(a, ssc, x2, *d_s2, (int)pad, false, nullptr, false, st, nullptr);
+        if ((rc2 = read_fallback(ssc, st, &fell_back))) return rc2;
+    }
+    if (force_lsd_sort() || fell_back) run_fold_sort_scan(a, ssc, x2, *d_s2, (int)pad, false, nullptr, true, st, nullptr);
     return GTLS_OK;
 }
 

@@ -145,7 +145,6 @@ struct BucketArgs {
     int* fallback;             // device flag: some bucket exceeded kBucketCap
     double* prefix;            // [tile*nbk*3] inclusive prefix of (w r, w, w r^2) per bucket (look-back)
     int* flag;                 // [tile*nbk]   prefix published
-    int force_fallback;        // GTLS_SORT=lsd: raise the flag regardless (tests of the LSD path)
     u64* keys;                 // [tile*n] bucketed keys
     u32* perm;                 // [tile*n]
     double* x1; double* s1; double* x0; double* s0; double* x2; double* s2;

@@ -78,6 +78,26 @@ def test_fold_sort_ties_and_tiny_inputs():
         assert np.array_equal(perm, pm_o), n
 
 
+def test_fold_sort_clustered_phases_take_the_lsd_fallback(tmpl512):
+    """More than kBucketCap (2048) points share one phase bucket: the bucket fast path raises its
+    fallback flag and the call is repeated on the LSD radix path; results must not change."""
+    _cuda()
+    rng = np.random.default_rng(11)
+    n = 6000
+    t = np.arange(n) * 0.5 + rng.uniform(0, 1e-4, n)        # phases for P = 0.5 cluster in [0, 2e-4)
+    ph, perm = g.gtls_fold_sort(t, np.array([0.5, 0.37]))
+    ph_o, pm_o = oracle.fold_sort(t, np.array([0.5, 0.37]))
+    assert np.array_equal(perm, pm_o) and np.array_equal(ph.view(np.uint64), ph_o.view(np.uint64))
+    y = 1 + rng.normal(0, 1e-3, n); dy = np.full(n, 1e-3)
+    per = np.array([0.5, 0.37, 1.0]); qs = np.array([0.01, 0.05])
+    ora = oracle.search(t, y, dy, per, qs, tmpl512, dt0=0.05)
+    res = g.gtls_search(t, y, dy, per, qs, tmpl512, dt0=0.05, sde_kernel=3)
+    assert np.allclose(res.chi2, ora.chi2, rtol=CHI2_RTOL, atol=0)
+    b = res.best()
+    assert np.array_equal(b["dur_idx"], ora.best["dur_idx"]) and np.array_equal(b["start"], ora.best["start"])
+    assert np.array_equal(b["t0"], ora.best["t0"])
+
+
 def test_fold_sort_unsorted_and_negative_times():
     _cuda()
     rng = np.random.default_rng(5)
