@@ -256,11 +256,15 @@ def main():
         stages = {k: st_acc[k] / args.steps for k in st_acc if k.startswith("ms_")}
         hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
         pp = float(st_acc["period_points"])
+        # fold + sort + gather + scan are one fused stage (bucket_sort.cu); algorithmic HBM bytes per
+        # period-point: 8 (bucketed key written) + 8 (read back) + 4 (permutation) + 1.15 x 16 (x1, S1 with
+        # the wrap pad) = 38.4 B when dy is uniform, + 18.4 B for x0, S0 otherwise
+        fss_bytes = 38.4 if st_acc["uniform_dy"] else 56.8
+        fss_ms = stages["ms_fold"] + stages["ms_sort"] + stages["ms_scan"]
         stage_roof = {
-            "fold_GBps": pp * 12 / (stages["ms_fold"] * 1e-3) / 1e9 if stages["ms_fold"] else None,
-            "sort_GBps": pp * 16 * 4 / (stages["ms_sort"] * 1e-3) / 1e9 if stages["ms_sort"] else None,
-            "scan_GBps": pp * (8 + 16 * (1 if st_acc["uniform_dy"] else 2)) / (stages["ms_scan"] * 1e-3) / 1e9
-            if stages["ms_scan"] else None,
+            "fold_sort_scan_GBps": pp * fss_bytes / (fss_ms * 1e-3) / 1e9 if fss_ms else None,
+            "fold_sort_scan_bytes_per_period_point": fss_bytes,
+            "fold_sort_scan_frac_of_hbm_peak": (pp * fss_bytes / (fss_ms * 1e-3) / 1e9 / hbm_peak) if fss_ms else None,
             "hbm_peak_GBps": hbm_peak, "peak_source": peak_src,
         }
         out = {

@@ -4,8 +4,8 @@
 // scan.cu, kept as the fallback):
 //
 //   k_bucket_count    fold every point, histogram of the top KBITS bits of floor(phase * 2^32)
-//   k_bucket_scan     per period: bucket starts; a bucket larger than kBucketCap raises the tile's
-//                     fallback flag (clustered phases), and the LSD path redoes the whole tile
+//   k_bucket_scan     per period: bucket starts; a bucket larger than kBucketCap (clustered phases) puts
+//                     the period on the tile's fallback list, which the LSD path processes instead
 //   k_bucket_scatter  fold again (t is L2 resident, the division is cheaper than 16 B of HBM) and
 //                     write (key32 << 32 | index) into its bucket, any order inside the bucket
 //   k_bucket_finish   one CTA per (period, bucket): the bucket (~1000 keys) is sorted entirely in shared
@@ -77,14 +77,18 @@ __global__ void __launch_bounds__(256) k_bucket_scan(BucketArgs b) {
     if (lane == 0) start[b.nbk] = carry;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) big = max(big, __shfl_xor_sync(0xffffffffu, big, o));
-    if (lane == 0 && big > (u32)kBucketCap) atomicExch(b.fallback, 1);
+    if (lane == 0) {
+        const int over = big > (u32)kBucketCap ? 1 : 0;
+        b.fb_flag[pl] = over;
+        if (over) b.fb_list[atomicAdd(b.fb_count, 1)] = pl;
+    }
 }
 
 __global__ void __launch_bounds__(kCountThreads) k_bucket_scatter(BucketArgs b) {
     __shared__ u32 cnt[kMaxBuckets];
     __shared__ u32 basepos[kMaxBuckets];
-    if (*b.fallback) return;
     const int pl = blockIdx.y;
+    if (b.fb_flag[pl]) return;
     for (int k = threadIdx.x; k < b.nbk; k += kCountThreads) cnt[k] = 0;
     __syncthreads();
     const double period = b.periods[b.p0 + pl];
@@ -135,8 +139,8 @@ __global__ void __launch_bounds__(kFinThreads) k_bucket_finish(BucketArgs b) {
     __shared__ double s_w[3][kFinThreads / 32];
     __shared__ double s_base[3];
     __shared__ u32 s_wsum[kFinThreads / 32];
-    if (*b.fallback) return;
     const int bk = blockIdx.x, pl = blockIdx.y;
+    if (b.fb_flag[pl]) return;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NW = kFinThreads / 32;
     const double period = b.periods[b.p0 + pl];
@@ -313,8 +317,8 @@ __global__ void __launch_bounds__(kFinThreads) k_bucket_finish(BucketArgs b) {
 template <bool HAS0, bool HAS2>
 __global__ void __launch_bounds__(kPadThreads) k_pad_scan(BucketArgs b) {
     __shared__ double s_w[3][32];
-    if (*b.fallback) return;
     const int pl = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (b.fb_flag[pl]) return;
     constexpr int NW = kPadThreads / 32;
     int pad = b.pad_override;
     if (pad < 0) {
@@ -386,6 +390,7 @@ int bucket_count_for(int n) {
 void launch_bucket_sort(const BucketArgs& b, bool has0, bool has2, bool sort_only, cudaStream_t st) {
     cudaMemsetAsync(b.hist, 0, (size_t)b.tile * b.nbk * sizeof(u32), st);
     cudaMemsetAsync(b.flag, 0, (size_t)b.tile * b.nbk * sizeof(int), st);
+    cudaMemsetAsync(b.fb_count, 0, sizeof(int), st);
     const dim3 grid((b.n + kCountThreads * kCountItems - 1) / (kCountThreads * kCountItems), b.tile);
     k_bucket_count<<<grid, kCountThreads, 0, st>>>(b);
     k_bucket_scan<<<(b.tile * 32 + 255) / 256, 256, 0, st>>>(b);

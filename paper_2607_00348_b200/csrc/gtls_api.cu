@@ -66,20 +66,20 @@ Sizes workspace_sizes(long long n, long long n_per, int n_dur, double q_max, boo
               2 * align_up(n_per * sizeof(double)) + align_up(n_per * sizeof(gtls_best)) + 4096;
     s.per_period = 2 * n * sizeof(u64) + 256ull * nt * sizeof(u32) + n_dur * sizeof(DurEntry) +
                    n_dur * sizeof(Partial) + (size_t)kChi2Variants * n_dur * sizeof(int) +
-                   n * sizeof(u32) + (4ull * kMaxBuckets + 1) * sizeof(u32) + 3ull * kMaxBuckets * sizeof(double) +
+                   n * sizeof(u32) + (4ull * kMaxBuckets + 3) * sizeof(u32) + 3ull * kMaxBuckets * sizeof(double) +
                    (uniform ? 1 : 2) * ((size_t)pitch + spitch) * sizeof(double);
     return s;
 }
 
 int auto_tile(long long n_per, const Sizes& s, size_t budget) {
     long long t = (long long)(budget / s.per_period);
-    if (t > 4096) t = 4096;
+    if (t > 8192) t = 8192;
     if (t > n_per) t = n_per;
     if (t < 1) t = 1;
     return (int)t;
 }
 
-constexpr size_t kDefaultTileBudget = 3ull << 30;   // bytes of per-tile scratch when automatic
+constexpr size_t kDefaultTileBudget = 12ull << 30;  // bytes of per-tile scratch when automatic
 
 gtls_opts resolve_opts(const gtls_opts* in) {
     gtls_opts o;
@@ -132,13 +132,15 @@ struct CurveDev {
 };
 
 
-struct SortScratch { u32* hist; u32* start; u32* cursor; int* fallback; double* prefix; int* flag; };
+struct SortScratch { u32* hist; u32* start; u32* cursor; int* fb_flag; int* fb_list; int* fb_count; double* prefix; int* flag; };
 
 bool take_sort_scratch(Arena& ar, size_t tile, int nbk, SortScratch& sc) {
     sc.hist = ar.take<u32>(tile * nbk);
     sc.start = ar.take<u32>(tile * (nbk + 1));
     sc.cursor = ar.take<u32>(tile * nbk);
-    sc.fallback = ar.take<int>(1);
+    sc.fb_flag = ar.take<int>(tile);
+    sc.fb_list = ar.take<int>(tile);
+    sc.fb_count = ar.take<int>(1);
     sc.prefix = ar.take<double>(tile * nbk * 3);
     sc.flag = ar.take<int>(tile * nbk);
     return sc.flag != nullptr;
@@ -150,15 +152,16 @@ bool force_lsd_sort() {
 }
 
 // Steps a1-a4 for the tile described by `a` (a.perm, a.x1/s1[/x0/s0] are outputs).
-//   use_lsd == false: the bucket fast path.  A bucket larger than kBucketCap (clustered phases) raises
-//     the sticky device flag sc.fallback; the caller reads it once at the end and, if set, repeats the
-//     whole call with use_lsd == true.
-//   use_lsd == true: the LSD radix path (fold_sort.cu + scan.cu), any phase distribution.
+//   The bucket fast path first; a period with a bucket larger than kBucketCap (clustered phases) is put
+//   on the tile's fallback list on the device and skipped by the fast path; the LSD radix path
+//   (fold_sort.cu + scan.cu) then runs over that list (a handful of CTAs that find it empty, normally).
+//   GTLS_SORT=lsd: the LSD path for every period (A-B runs, tests).
 // sort_only: permutation only.  phase_out: also export the phases (Eq. 10).
 void run_fold_sort_scan(TileArgs& a, const SortScratch& sc, double* x2, double* s2, int pad_override,
-                        bool sort_only, double* phase_out, bool use_lsd, cudaStream_t st, int* launches) {
-    a.run_if = nullptr;
-    if (!use_lsd) {
+                        bool sort_only, double* phase_out, cudaStream_t st, int* launches) {
+    a.seg_list = nullptr; a.seg_count = nullptr;
+    int nl = 0;
+    if (!force_lsd_sort()) {
         BucketArgs b;
         memset(&b, 0, sizeof(b));
         b.n = a.n; b.tile = a.tile; b.p0 = a.p0; b.n_dur = a.n_dur; b.pad_override = pad_override;
@@ -167,29 +170,25 @@ void run_fold_sort_scan(TileArgs& a, const SortScratch& sc, double* x2, double* 
         b.shift = 32 - lg;
         b.pitch = a.pitch; b.spitch = a.spitch;
         b.t = a.t; b.wr = a.wr; b.w = a.w; b.wr2 = a.wr2; b.periods = a.periods; b.durtab = a.durtab;
-        b.hist = sc.hist; b.start = sc.start; b.cursor = sc.cursor; b.fallback = sc.fallback;
+        b.hist = sc.hist; b.start = sc.start; b.cursor = sc.cursor;
+        b.fb_flag = sc.fb_flag; b.fb_list = sc.fb_list; b.fb_count = sc.fb_count;
         b.prefix = sc.prefix; b.flag = sc.flag;
         b.keys = a.keys_b; b.perm = a.perm;
         b.x1 = a.x1; b.s1 = a.s1; b.x0 = a.x0; b.s0 = a.s0; b.x2 = x2; b.s2 = s2;
         const bool has2 = s2 != nullptr, has0 = !a.uniform || has2;
         launch_bucket_sort(b, has0, has2, sort_only, st);
-        if (phase_out) launch_fold_keys(a, phase_out, st);     // phases come from the LSD path's fold kernel
-        if (launches) *launches += (sort_only ? 4 : 5) + (phase_out ? 1 : 0);
-        return;
+        nl += sort_only ? 4 : 5;
+        if (phase_out) { launch_fold_keys(a, phase_out, st); ++nl; }   // phases: the LSD path's fold kernel
+        a.seg_list = sc.fb_list; a.seg_count = sc.fb_count;
+        phase_out = nullptr;
     }
     launch_fold_keys(a, phase_out, st);
     int l2 = 0;
     const u64* sorted = launch_phase_sort(a, st, &l2);
     if (!sort_only) launch_gather_scan(a, sorted, x2, s2, pad_override, st);
-    launch_perm_export(sorted, (long long)a.tile * a.n, (int32_t*)a.perm, nullptr, st);
-    if (launches) *launches += 1 + l2 + (sort_only ? 0 : 1) + 1;
-}
-
-// reads the sticky fallback flag (synchronises the stream)
-int read_fallback(const SortScratch& sc, cudaStream_t st, int* out) {
-    CU(cudaMemcpyAsync(out, sc.fallback, sizeof(int), cudaMemcpyDeviceToHost, st));
-    CU(cudaStreamSynchronize(st));
-    return GTLS_OK;
+    launch_perm_export(a, sorted, (int32_t*)a.perm, st);
+    a.seg_list = nullptr; a.seg_count = nullptr;
+    if (launches) *launches += nl + 1 + l2 + (sort_only ? 0 : 1) + 1;
 }
 
 }  // namespace
@@ -358,12 +357,6 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     a.dbg_max_st = getenv("GTLS_DBG_MAX_ST") ? atoi(getenv("GTLS_DBG_MAX_ST")) : 0x7fffffff;
     SdeScratch sc;
     unsigned long long counters[2];
-    const gtls_stats stats0 = stats;
-    for (int attempt = 0; attempt < 2; ++attempt) {
-    const bool use_lsd = force_lsd_sort() || attempt == 1;
-    stats = stats0;
-    CU(cudaMemsetAsync(ssc.fallback, 0, sizeof(int), st));
-    CU(cudaMemsetAsync(d_counters, 0, 2 * sizeof(unsigned long long), st));
     // ---- period tiles ----------------------------------------------------------------------
     for (long long p0 = 0; p0 < n_per; p0 += tile) {
         a.p0 = p0;
@@ -373,7 +366,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
         launch_durtab(a, st);
         tm.mark(1);
         tm.mark(2);
-        run_fold_sort_scan(a, ssc, nullptr, nullptr, -1, false, nullptr, use_lsd, st, &launches);
+        run_fold_sort_scan(a, ssc, nullptr, nullptr, -1, false, nullptr, st, &launches);
         tm.mark(3);
         tm.mark(4);
         if (use_v1) launch_chi2(a, st); else if (use_rows) launch_chi2_rows(a, st); else launch_chi2_ring(a, st);
@@ -396,16 +389,12 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     launch_sde(d_chi2, n_per, o.sde_kernel, d_sde_raw, d_sde, d_sde_sc, st, &launches);
     stats.kernel_launches += launches;
     tm.mark(1);
-    int fell_back = 0;
     CU(cudaMemcpyAsync(&sc, d_sde_sc, sizeof(sc), cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(counters, d_counters, sizeof(counters), cudaMemcpyDeviceToHost, st));
-    CU(cudaMemcpyAsync(&fell_back, ssc.fallback, sizeof(int), cudaMemcpyDeviceToHost, st));
     if (o.stats) cudaEventRecord(ev_end, st);
     CU(cudaStreamSynchronize(st));
     CU(cudaGetLastError());
     if (o.stats) stats.ms_epilogue = tm.ms(0, 1);
-    if (use_lsd || !fell_back) break;      // a bucket overflowed: repeat the search on the LSD sort path
-    }
 
     if (out_summary) {
         gtls_best b;
@@ -490,13 +479,7 @@ int gtls_fold_sort(const double* t, int64_t n, const double* periods, int64_t n_
         double* ph = dev ? (out_phase ? out_phase + p0 * n : nullptr) : d_phase;
         int32_t* pm = dev ? out_perm + p0 * n : d_perm;
         a.perm = (u32*)pm;
-        CU(cudaMemsetAsync(ssc.fallback, 0, sizeof(int), st));
-        int fell_back = 0;
-        if (!force_lsd_sort()) {
-            run_fold_sort_scan(a, ssc, nullptr, nullptr, 0, true, ph, false, st, nullptr);
-            if ((rc = read_fallback(ssc, st, &fell_back))) return rc;
-        }
-        if (force_lsd_sort() || fell_back) run_fold_sort_scan(a, ssc, nullptr, nullptr, 0, true, ph, true, st, nullptr);
+        run_fold_sort_scan(a, ssc, nullptr, nullptr, 0, true, ph, st, nullptr);
         if (!dev) {
             if (out_phase) CU(cudaMemcpyAsync(out_phase + p0 * n, ph, cnt * sizeof(double), cudaMemcpyDeviceToHost, st));
             CU(cudaMemcpyAsync(out_perm + p0 * n, pm, cnt * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
@@ -551,13 +534,7 @@ static int one_period_scan(const double* t, const double* y, const double* dy, i
     a.s1 = ar.take<double>(spitch); a.s0 = ar.take<double>(spitch);
     *d_s2 = ar.take<double>(spitch);
     if (!*d_s2) return GTLS_ENOMEM;
-    CU(cudaMemsetAsync(ssc.fallback, 0, sizeof(int), st));
-    int fell_back = 0, rc2 = 0;
-    if (!force_lsd_sort()) {
-        run_fold_sort_scan(a, ssc, x2, *d_s2, (int)pad, false, nullptr, false, st, nullptr);
-        if ((rc2 = read_fallback(ssc, st, &fell_back))) return rc2;
-    }
-    if (force_lsd_sort() || fell_back) run_fold_sort_scan(a, ssc, x2, *d_s2, (int)pad, false, nullptr, true, st, nullptr);
+    run_fold_sort_scan(a, ssc, x2, *d_s2, (int)pad, false, nullptr, st, nullptr);
     return GTLS_OK;
 }
 

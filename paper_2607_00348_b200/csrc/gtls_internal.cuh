@@ -95,6 +95,10 @@ __device__ __forceinline__ int t0_stride(int D, double dt0) {
     return s < 1.0 ? 1 : (int)s;
 }
 
+// LSD path: segments (periods of the tile) a kernel has to process
+__device__ __forceinline__ int seg_count(const int* list, const int* count, int tile) { return list ? *count : tile; }
+__device__ __forceinline__ int seg_at(const int* list, int s) { return list ? list[s] : s; }
+
 // ---- host-side launchers (one per kernel family) ----------------------------------------
 struct TileArgs {
     int n;                 // points in the light curve
@@ -124,7 +128,8 @@ struct TileArgs {
     double* s1; double* s0;   // [tile*spitch]
     Partial* partial;      // [tile*n_dur]
     u32* perm;             // [tile*n]   sorted position -> input index
-    const int* run_if;     // LSD fallback kernels run only when *run_if != 0 (nullptr: always)
+    const int* seg_list;   // LSD path: periods (tile-local) to process, or nullptr = all of the tile
+    const int* seg_count;  // number of entries of seg_list (device)
     int* trial_list;       // [kChi2Variants][tile*n_dur] trial indices binned by chi2 kernel variant
     int* trial_count;      // [kChi2Variants]
     int dbg_min_st, dbg_max_st;   // timing experiments only (GTLS_DBG_MIN_ST / GTLS_DBG_MAX_ST): skip other trials
@@ -142,7 +147,9 @@ struct BucketArgs {
     u32* hist;                 // [tile*nbk]
     u32* start;                // [tile*(nbk+1)]
     u32* cursor;               // [tile*nbk]
-    int* fallback;             // device flag: some bucket exceeded kBucketCap
+    int* fb_flag;              // [tile] 1: a bucket of this period exceeded kBucketCap (LSD path takes it)
+    int* fb_list;              // [tile] those periods, any order
+    int* fb_count;             // [1]
     double* prefix;            // [tile*nbk*3] inclusive prefix of (w r, w, w r^2) per bucket (look-back)
     int* flag;                 // [tile*nbk]   prefix published
     u64* keys;                 // [tile*n] bucketed keys
@@ -172,7 +179,7 @@ void launch_reduce(const TileArgs& a, double* out_chi2, gtls_best* out_best,
                    unsigned long long* counters, cudaStream_t st);
 void launch_window_export(const TileArgs& a, const double* s2, double q, int32_t* out_start,
                           double* out_depth, double* out_c_out, double* out_c_in, cudaStream_t st);
-void launch_perm_export(const u64* sorted, long long count, int32_t* out_perm, const int* run_if, cudaStream_t st);
+void launch_perm_export(const TileArgs& a, const u64* sorted, int32_t* out_perm, cudaStream_t st);
 
 struct SdeScratch {      // device scalars of the epilogue
     double chi2_min, mean_sr, sd_sr, sde_raw_best, sde_max;

@@ -26,8 +26,9 @@ __global__ void __launch_bounds__(kScanThreads) k_gather_scan(TileArgs a, const 
                                                               int pad_override) {
     __shared__ double s_w[3][32];
     __shared__ double s_carry[3];
-    if (a.run_if && !*a.run_if) return;
-    const int pl = blockIdx.x;
+    const int nseg = seg_count(a.seg_list, a.seg_count, a.tile);
+    for (int sg = blockIdx.x; sg < nseg; sg += gridDim.x) {      // (body indented one level less)
+    const int pl = seg_at(a.seg_list, sg);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     int pad = pad_override;
     if (pad < 0) {      // D_m of this period = its largest D (reading G3: any D_m >= D is equivalent)
@@ -121,6 +122,8 @@ __global__ void __launch_bounds__(kScanThreads) k_gather_scan(TileArgs a, const 
         }
         __syncthreads();
     }
+    __syncthreads();
+    }
 }
 
 }  // namespace
@@ -128,9 +131,10 @@ __global__ void __launch_bounds__(kScanThreads) k_gather_scan(TileArgs a, const 
 void launch_gather_scan(const TileArgs& a, const u64* sorted, double* x2, double* s2,
                         int pad_override, cudaStream_t st) {
     const bool has0 = !a.uniform || s2 != nullptr;
-    if (s2) k_gather_scan<true, true><<<a.tile, kScanThreads, 0, st>>>(a, sorted, x2, s2, pad_override);
-    else if (has0) k_gather_scan<true, false><<<a.tile, kScanThreads, 0, st>>>(a, sorted, nullptr, nullptr, pad_override);
-    else k_gather_scan<false, false><<<a.tile, kScanThreads, 0, st>>>(a, sorted, nullptr, nullptr, pad_override);
+    const unsigned grid = a.seg_list ? (a.tile < 16 ? a.tile : 16) : a.tile;
+    if (s2) k_gather_scan<true, true><<<grid, kScanThreads, 0, st>>>(a, sorted, x2, s2, pad_override);
+    else if (has0) k_gather_scan<true, false><<<grid, kScanThreads, 0, st>>>(a, sorted, nullptr, nullptr, pad_override);
+    else k_gather_scan<false, false><<<grid, kScanThreads, 0, st>>>(a, sorted, nullptr, nullptr, pad_override);
 }
 
 }  // namespace gtls
