@@ -149,6 +149,17 @@ def run_reference(args, w):
     }
 
 
+def max_over_ranks(x: float, world: int, device="cpu") -> float:
+    """Multi-rank runs (replicas only): the job time is the slowest rank's."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    tt = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
 def workload_desc(w) -> str:
     return (f"{w.name}: {w.lc.n} points, {w.n_per} periods (Ofir grid, OS=3), {w.n_dur} durations/period, "
             f"dt0={w.dt0}, template 512 nodes")
@@ -228,10 +239,7 @@ def main():
     barrier()
     clocks = sampler.stop()
     ms_total = ev0.elapsed_time(ev1)
-    if world > 1:
-        tt = torch.tensor([ms_total], dtype=torch.float64, device=devname)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms_total = float(tt.item())
+    ms_total = max_over_ranks(ms_total, world, devname)
     ms_step = ms_total / args.steps
     value = world * w.trials / (ms_step / 1e3)
 
@@ -300,10 +308,7 @@ def main():
             r2 = g.gtls_search(*h_in, dt0=w.dt0, sde_kernel=151)
         torch.cuda.synchronize()
         dt = (time.perf_counter() - t0) / n_e2e
-        if world > 1:
-            tt = torch.tensor([dt], dtype=torch.float64, device=devname)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            dt = float(tt.item())
+        dt = max_over_ranks(dt, world, devname)
         if rank == 0:
             h2d = int(sum(x.nbytes for x in h_in))
             d2h = int(w.n_per * (8 * 3 + 24))
