@@ -11,9 +11,8 @@
 //   k_bucket_finish   one CTA per (period, bucket): the bucket (~1000 keys) is sorted entirely in shared
 //                     memory -- counting sort on the next 10 key bits, then an exact rank inside every
 //                     run of equal 10-bit codes by (key32, fp64 phase, index) -- gathered and scanned
-//                     locally; the running sums of the earlier buckets of the period arrive through a
-//                     look-back (each CTA publishes its own sums at once and adds the earlier buckets'
-//                     sums in a fixed order; CTAs are scheduled in bucket order), then permutation, x1 = w r (x0 = w), S1 (S0) are written.
+//                     locally: permutation, x1 = w r (x0 = w), bucket-local S1 (S0) and the bucket's sums.
+//   k_prefix_fix      adds the sums of the period's earlier buckets (fixed order) to the local prefixes.
 //   k_pad_scan        wrap padding (Fig. 3): the first D_m sorted entries again, the sums run on.
 //
 // The order inside a bucket before the local sort is irrelevant because the local sort orders by the
@@ -126,10 +125,6 @@ __device__ __forceinline__ bool key_less(const u64 a, const u64 b, const double*
     return (u32)a < (u32)b;
 }
 
-__device__ __forceinline__ void st_release(int* p, int v) {
-    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-
 template <bool HAS0, bool HAS2, bool SORT_ONLY>
 __global__ void __launch_bounds__(kFinThreads) k_bucket_finish(BucketArgs b) {
     __shared__ u64 A[kBucketCap];
@@ -237,51 +232,17 @@ __global__ void __launch_bounds__(kFinThreads) k_bucket_finish(BucketArgs b) {
     }
     if (lane == 31) { s_w[0][warp] = t1; s_w[1][warp] = t0; s_w[2][warp] = t2; }
     __syncthreads();
-    // 8. look-back: publish this bucket's sums at once, then add up the sums of the earlier buckets of the
-    //    period in a fixed order (strided per lane, then a shuffle tree), so the base is deterministic
-    double* agg = b.prefix + (long long)pl * b.nbk * 3;
-    int* flag = b.flag + (long long)pl * b.nbk;
+    // 8. publish this bucket's sums (k_prefix_fix adds the sums of the earlier buckets afterwards: a
+    //    look-back inside this kernel made every CTA wait for the slowest of its period's earlier CTAs)
     if (tid == 0) {
         double tot1 = 0.0, tot0 = 0.0, tot2 = 0.0;
 #pragma unroll
         for (int k = 0; k < NW; ++k) { tot1 += s_w[0][k]; tot0 += s_w[1][k]; tot2 += s_w[2][k]; }
-        __stcg(agg + bk * 3, tot1); __stcg(agg + bk * 3 + 1, tot0); __stcg(agg + bk * 3 + 2, tot2);
-        __threadfence();
-        st_release(flag + bk, 1);
+        double* agg = b.prefix + ((long long)pl * b.nbk + bk) * 3;
+        agg[0] = tot1; agg[1] = tot0; agg[2] = tot2;
+        s_base[0] = 0.0; s_base[1] = 0.0; s_base[2] = 0.0;
     }
-    if (warp == 0) {
-        // poll the earlier buckets' flags with independent relaxed loads, one acquire fence, then the sums
-        for (int j0 = 0; j0 < bk; j0 += 128) {
-            bool ready;
-            do {
-                int f = 1;
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const int j = j0 + lane + 32 * q;
-                    if (j < bk) f &= *((volatile const int*)(flag + j));
-                }
-                ready = __all_sync(0xffffffffu, f != 0);
-                if (!ready) __nanosleep(100);
-            } while (!ready);
-        }
-        __threadfence();
-        double a1 = 0.0, a0 = 0.0, a2 = 0.0;
-        for (int j = lane; j < bk; j += 32) {
-            a1 += __ldcg(agg + j * 3);
-            if (HAS0) a0 += __ldcg(agg + j * 3 + 1);
-            if (HAS2) a2 += __ldcg(agg + j * 3 + 2);
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            a1 += __shfl_xor_sync(0xffffffffu, a1, o);
-            a0 += __shfl_xor_sync(0xffffffffu, a0, o);
-            a2 += __shfl_xor_sync(0xffffffffu, a2, o);
-        }
-        if (lane == 0) { s_base[0] = a1; s_base[1] = a0; s_base[2] = a2; }
-    } else {
-        // meanwhile the other warps write what does not depend on the base
-        for (int i = tid - 32; i < m; i += kFinThreads - 32) perm[i] = (u32)A[i];
-    }
+    for (int i = tid; i < m; i += kFinThreads) perm[i] = (u32)A[i];
 #pragma unroll
     for (int e = 0; e < kFinItems; ++e) {
         if (first + e < m) {
@@ -310,6 +271,44 @@ __global__ void __launch_bounds__(kFinThreads) k_bucket_finish(BucketArgs b) {
             if (HAS0) s0[first + e + 1] = o0 + v0[e];
             if (HAS2) s2[first + e + 1] = o2 + v2[e];
         }
+    }
+}
+
+// Adds to the bucket-local prefix sums the sums of the earlier buckets of the period, taken in a fixed
+// order (strided per lane, then a shuffle tree): deterministic.  One CTA per (period, bucket).
+template <bool HAS0, bool HAS2>
+__global__ void __launch_bounds__(256) k_prefix_fix(BucketArgs b) {
+    __shared__ double s_base[3];
+    const int bk = blockIdx.x, pl = blockIdx.y;
+    if (bk == 0 || b.fb_flag[pl]) return;
+    const int lane = threadIdx.x & 31;
+    if (threadIdx.x < 32) {
+        const double* agg = b.prefix + (long long)pl * b.nbk * 3;
+        double a1 = 0.0, a0 = 0.0, a2 = 0.0;
+        for (int j = lane; j < bk; j += 32) {
+            a1 += agg[j * 3];
+            if (HAS0) a0 += agg[j * 3 + 1];
+            if (HAS2) a2 += agg[j * 3 + 2];
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            a1 += __shfl_xor_sync(0xffffffffu, a1, o);
+            a0 += __shfl_xor_sync(0xffffffffu, a0, o);
+            a2 += __shfl_xor_sync(0xffffffffu, a2, o);
+        }
+        if (lane == 0) { s_base[0] = a1; s_base[1] = a0; s_base[2] = a2; }
+    }
+    __syncthreads();
+    const u32* start = b.start + (long long)pl * (b.nbk + 1);
+    const int bs = (int)start[bk], m = (int)start[bk + 1] - bs;
+    double* s1 = b.s1 + (long long)pl * b.spitch + bs + 1;
+    double* s0 = HAS0 ? b.s0 + (long long)pl * b.spitch + bs + 1 : nullptr;
+    double* s2 = HAS2 ? b.s2 + (long long)pl * b.spitch + bs + 1 : nullptr;
+    const double b1 = s_base[0], b0 = s_base[1], b2 = s_base[2];
+    for (int i = threadIdx.x; i < m; i += blockDim.x) {
+        s1[i] = b1 + s1[i];
+        if (HAS0) s0[i] = b0 + s0[i];
+        if (HAS2) s2[i] = b2 + s2[i];
     }
 }
 
@@ -389,7 +388,6 @@ int bucket_count_for(int n) {
 
 void launch_bucket_sort(const BucketArgs& b, bool has0, bool has2, bool sort_only, cudaStream_t st) {
     cudaMemsetAsync(b.hist, 0, (size_t)b.tile * b.nbk * sizeof(u32), st);
-    cudaMemsetAsync(b.flag, 0, (size_t)b.tile * b.nbk * sizeof(int), st);
     cudaMemsetAsync(b.fb_count, 0, sizeof(int), st);
     const dim3 grid((b.n + kCountThreads * kCountItems - 1) / (kCountThreads * kCountItems), b.tile);
     k_bucket_count<<<grid, kCountThreads, 0, st>>>(b);
@@ -399,12 +397,15 @@ void launch_bucket_sort(const BucketArgs& b, bool has0, bool has2, bool sort_onl
     if (sort_only) { k_bucket_finish<false, false, true><<<fgrid, kFinThreads, 0, st>>>(b); return; }
     if (has2) {
         k_bucket_finish<true, true, false><<<fgrid, kFinThreads, 0, st>>>(b);
+        k_prefix_fix<true, true><<<fgrid, 256, 0, st>>>(b);
         k_pad_scan<true, true><<<b.tile, kPadThreads, 0, st>>>(b);
     } else if (has0) {
         k_bucket_finish<true, false, false><<<fgrid, kFinThreads, 0, st>>>(b);
+        k_prefix_fix<true, false><<<fgrid, 256, 0, st>>>(b);
         k_pad_scan<true, false><<<b.tile, kPadThreads, 0, st>>>(b);
     } else {
         k_bucket_finish<false, false, false><<<fgrid, kFinThreads, 0, st>>>(b);
+        k_prefix_fix<false, false><<<fgrid, 256, 0, st>>>(b);
         k_pad_scan<false, false><<<b.tile, kPadThreads, 0, st>>>(b);
     }
 }

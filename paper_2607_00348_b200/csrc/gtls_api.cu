@@ -177,7 +177,7 @@ void run_fold_sort_scan(TileArgs& a, const SortScratch& sc, double* x2, double* 
         b.x1 = a.x1; b.s1 = a.s1; b.x0 = a.x0; b.s0 = a.s0; b.x2 = x2; b.s2 = s2;
         const bool has2 = s2 != nullptr, has0 = !a.uniform || has2;
         launch_bucket_sort(b, has0, has2, sort_only, st);
-        nl += sort_only ? 4 : 5;
+        nl += sort_only ? 4 : 6;
         if (phase_out) { launch_fold_keys(a, phase_out, st); ++nl; }   // phases: the LSD path's fold kernel
         a.seg_list = sc.fb_list; a.seg_count = sc.fb_count;
         phase_out = nullptr;
