@@ -9,8 +9,8 @@
 //   k_bucket_scatter  fold again (t is L2 resident, the division is cheaper than 16 B of HBM) and
 //                     write (key32 << 32 | index) into its bucket, any order inside the bucket
 //   k_bucket_finish   one CTA per (period, bucket): the bucket (~1000 keys) is sorted entirely in shared
-//                     memory -- counting sort on the next 10 key bits, then an exact rank inside every
-//                     run of equal 10-bit codes by (key32, fp64 phase, index) -- gathered and scanned
+//                     memory -- counting sort on the next 11 key bits, then an exact rank inside every
+//                     run of equal 11-bit codes by (key32, fp64 phase, index) -- gathered and scanned
 //                     locally: permutation, x1 = w r (x0 = w), bucket-local S1 (S0) and the bucket's sums.
 //   k_prefix_fix      adds the sums of the period's earlier buckets (fixed order) to the local prefixes.
 //   k_pad_scan        wrap padding (Fig. 3): the first D_m sorted entries again, the sums run on.
@@ -29,7 +29,7 @@ constexpr int kCountItems = 8;                       // points per thread in cou
 constexpr int kFinThreads = 256;                     // one CTA per bucket
 constexpr int kFinItems = kBucketCap / kFinThreads;  // sorted entries per thread (8)
 constexpr int kPadThreads = 512;
-constexpr int kSubBits = 10;
+constexpr int kSubBits = 11;
 constexpr int kSub = 1 << kSubBits;                  // sub-buckets of the local counting sort
 constexpr int kScanItems = 4;                        // pad scan: entries per thread and round
 
@@ -129,8 +129,7 @@ template <bool HAS0, bool HAS2, bool SORT_ONLY>
 __global__ void __launch_bounds__(kFinThreads) k_bucket_finish(BucketArgs b) {
     __shared__ u64 A[kBucketCap];
     __shared__ u64 B[kBucketCap];
-    __shared__ u32 H[kSub + 1];                                // counts -> starts
-    __shared__ u32 cur[kSub];
+    __shared__ u32 H[kSub + 1];                                // counts -> starts -> (after the scatter) ends
     __shared__ double s_w[3][kFinThreads / 32];
     __shared__ double s_base[3];
     __shared__ u32 s_wsum[kFinThreads / 32];
@@ -146,12 +145,12 @@ __global__ void __launch_bounds__(kFinThreads) k_bucket_finish(BucketArgs b) {
 
     // 1. load the bucket, clear the sub-bucket histogram
     for (int i = tid; i < m; i += kFinThreads) A[i] = keys[i];
-    for (int k = tid; k <= kSub; k += kFinThreads) H[k] = 0;
+    for (int k = tid; k < kSub; k += kFinThreads) H[k] = 0;
     __syncthreads();
-    // 2. histogram of the next 10 key bits
+    // 2. histogram of the next 11 key bits
     for (int i = tid; i < m; i += kFinThreads) atomicAdd(&H[((u32)(A[i] >> 32) >> subshift) & (kSub - 1)], 1u);
     __syncthreads();
-    // 3. exclusive scan of the kSub counts (4 per thread)
+    // 3. exclusive scan of the kSub counts (8 per thread)
     {
         constexpr int PER = kSub / kFinThreads;
         u32 c[PER], sum = 0;
@@ -167,21 +166,20 @@ __global__ void __launch_bounds__(kFinThreads) k_bucket_finish(BucketArgs b) {
         for (int k = 0; k < NW; ++k) wbase += k < warp ? s_wsum[k] : 0u;
         u32 base = wbase + x - sum;
 #pragma unroll
-        for (int e = 0; e < PER; ++e) { H[tid * PER + e] = base; cur[tid * PER + e] = base; base += c[e]; }
-        if (tid == kFinThreads - 1) H[kSub] = base;
+        for (int e = 0; e < PER; ++e) { H[tid * PER + e] = base; base += c[e]; }
     }
     __syncthreads();
     // 4. counting-sort scatter (order inside a sub-bucket is arbitrary)
     for (int i = tid; i < m; i += kFinThreads) {
         const u64 k = A[i];
-        B[atomicAdd(&cur[((u32)(k >> 32) >> subshift) & (kSub - 1)], 1u)] = k;
+        B[atomicAdd(&H[((u32)(k >> 32) >> subshift) & (kSub - 1)], 1u)] = k;
     }
     __syncthreads();
-    // 5. exact rank inside every run of equal 10-bit codes
+    // 5. exact rank inside every run of equal 11-bit codes
     for (int i = tid; i < m; i += kFinThreads) {
         const u64 k = B[i];
         const u32 sb = ((u32)(k >> 32) >> subshift) & (kSub - 1);
-        const int rs = (int)H[sb], re = (int)H[sb + 1];
+        const int rs = sb ? (int)H[sb - 1] : 0, re = (int)H[sb];     // H[sb] is now the end of sub-bucket sb
         int r = i;
         if (re - rs > 1) {
             r = rs;
