@@ -41,10 +41,10 @@ namespace {
 constexpr int kRT = 128;                 // threads per CTA
 constexpr int kRW = kRT / 32;            // warps (= trials) per CTA
 constexpr int kPartPitch = 36;           // doubles per slot row of the per-warp emit buffer
-constexpr int kPartRows = 8;             // >= max PfRows
+constexpr int kPartRows = 16;            // two emit buffers of max PfRows rows (pipelined column sums)
 constexpr int kFifoBatches = 3;          // batches of PfRows rows per lane in the cp.async FIFO
 constexpr int kFifoRows = 24;            // >= kFifoBatches * max PfRows
-constexpr int kCW = 1056;                // window-table doubles per warp (>= 32 * 21)
+constexpr int kCW = 704;                 // window-table doubles per warp (>= 32 * 21)
 constexpr int kTmplSmem = 1024;          // template nodes cached in shared memory
 constexpr int kWarpSmem = kPartRows * kPartPitch + kFifoRows * 32 + kCW;   // doubles per warp
 
@@ -312,6 +312,142 @@ __device__ __forceinline__ void march(const Cls& c, const It& it, const double* 
     }
 }
 
+// Wide path, at most two segments per warp: the same march as a software pipeline.  A warp issues in
+// order, so every load is placed at least one row (MB DFMAs) before its first use:
+//   - the X value of row j+LA is read from the FIFO while row j is multiplied, and its slot is refilled
+//     (cp.async) with row j+LA+MB at once (FIFO depth = MB rows);
+//   - the column sums of a completed batch of PF windows are spread over the rows of the NEXT batch:
+//     A (batch end) 4 loads, B 4 loads + first partial sums, C second partial sums, D/E the two shuffle
+//     steps and the table loads, F the table stores.  Two emit buffers alternate.
+template <int MB>
+__device__ __forceinline__ void march_pipe(const Cls& c, const It& it, const double* __restrict__ xp,
+                                           const int rows_valid, const int nblk, const double (&T)[MB],
+                                           const int lane) {
+    constexpr int PF = PfRows<MB>::v;
+    constexpr int NBAT = MB / PF;                  // copy groups in flight = batches per block
+    constexpr int XQ = (MB % 3 == 0) ? 3 : 4;      // X registers; LA rows of look-ahead
+    constexpr int LA = XQ - 1;
+    static_assert(PF >= 6 && MB % PF == 0 && MB % XQ == 0 && MB <= kFifoRows && 2 * PF <= kPartRows, "geometry");
+    constexpr unsigned kRowB = kPartPitch * 8;     // bytes per emit-buffer row
+    double acc[MB], xq[XQ];
+#pragma unroll
+    for (int u = 0; u < MB; ++u) acc[u] = 0.0;
+    const unsigned fl = c.fifo + (unsigned)(lane * 8);
+    const long long rstride = (long long)c.stp;
+    int row_issue = 0;                             // next row to copy
+#pragma unroll
+    for (int k = 0; k < NBAT; ++k) {
+#pragma unroll
+        for (int u = 0; u < PF; ++u) {
+            cp_async8(fl + (unsigned)((k * PF + u) * 256), xp, row_issue < rows_valid);
+            xp += rstride;
+            ++row_issue;
+        }
+        cp_async_commit();
+    }
+    cp_async_wait<NBAT - 1>();
+#pragma unroll
+    for (int k = 0; k < LA; ++k) {                 // rows 0 .. LA-1: read, refill the slot with row MB + k
+        const unsigned fa = fl + (unsigned)(k * 256);
+        xq[k] = lds64(fa);
+        cp_async8(fa, xp, row_issue < rows_valid);
+        xp += rstride;
+        ++row_issue;
+    }
+
+    // column-sum roles: lane = (window slot sl, quarter r); quarter r adds lanes r, r+4, ..., r+28
+    const int sl = lane >> 2, r = lane & 3;
+    const int slc = sl < PF ? sl : PF - 1;
+    const unsigned rd_off = (unsigned)((slc * kPartPitch + r) * 8);
+    const bool two = it.ng == 2;
+    const int split = two ? (it.seg_first + 1) * c.stp - it.f0 : 32;
+    unsigned pcur = c.part + (unsigned)(lane * 8);            // emit buffer of the running batch (my column)
+    unsigned pother = pcur + (unsigned)(PF * kRowB);
+    unsigned rprev = c.part + rd_off;                         // read base of the batch being summed
+    int kw_prev = 0;
+    bool have_prev = false;
+    double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0, sa = 0.0, sb = 0.0, ta = 0.0, tb = 0.0;
+    int wa = 0, wb = 0;
+    bool oka = false, okb = false;
+
+    auto masked = [&](const double v, const int q, double& a, double& b) {
+        if (q < split) a += v; else b += v;
+    };
+    auto stage_B = [&]() {          // first four values -> sums; load the other four
+        sa = 0.0; sb = 0.0;
+        if (!two) { sa = (v0 + v1) + (v2 + v3); }
+        else { masked(v0, r, sa, sb); masked(v1, r + 4, sa, sb); masked(v2, r + 8, sa, sb); masked(v3, r + 12, sa, sb); }
+        v0 = lds64(rprev + 128); v1 = lds64(rprev + 160); v2 = lds64(rprev + 192); v3 = lds64(rprev + 224);
+    };
+    auto stage_C = [&]() {
+        if (!two) { sa += (v0 + v1) + (v2 + v3); }
+        else { masked(v0, r + 16, sa, sb); masked(v1, r + 20, sa, sb); masked(v2, r + 24, sa, sb); masked(v3, r + 28, sa, sb); }
+    };
+    auto stage_D = [&]() {
+        sa += __shfl_xor_sync(0xffffffffu, sa, 1);
+        if (two) sb += __shfl_xor_sync(0xffffffffu, sb, 1);
+    };
+    auto stage_E = [&]() {
+        sa += __shfl_xor_sync(0xffffffffu, sa, 2);
+        if (two) sb += __shfl_xor_sync(0xffffffffu, sb, 2);
+        const int kw = kw_prev + sl;
+        const bool okk = have_prev && r == 0 && sl < PF && kw >= 0 && kw < it.L;
+        wa = it.seg_first * it.L + kw;
+        wb = wa + it.L;
+        oka = okk && wa < it.nWt;
+        okb = okk && two && wb < it.nWt;
+        ta = oka ? lds64(it.tab + (unsigned)(wa * 8)) : 0.0;
+        tb = okb ? lds64(it.tab + (unsigned)(wb * 8)) : 0.0;
+    };
+    auto stage_F = [&]() {
+        if (oka) sts64(it.tab + (unsigned)(wa * 8), ta + sa);
+        if (okb) sts64(it.tab + (unsigned)(wb * 8), tb + sb);
+    };
+
+#pragma unroll 1
+    for (int blk = 0; blk < nblk; ++blk) {
+#pragma unroll
+        for (int u = 0; u < MB; ++u) {
+            // X of row j+LA: FIFO -> register, slot refilled with row j+LA+MB
+            if ((u + LA) % PF == 0) cp_async_wait<NBAT - 1>();
+            {
+                const unsigned fa = fl + (unsigned)(((u + LA) % MB) * 256);
+                xq[(u + LA) % XQ] = lds64(fa);
+                cp_async8(fa, xp, row_issue < rows_valid);
+                xp += rstride;
+                ++row_issue;
+                if ((u + LA) % PF == PF - 1) cp_async_commit();
+            }
+            const double x = xq[u % XQ];
+#pragma unroll
+            for (int m = 0; m < MB; ++m) {
+                const int a = (u - m + MB) % MB;
+                if (m == 0) acc[a] = T[0] * x;                      // window gamma starts at this row
+                else acc[a] = fma(T[m], x, acc[a]);
+            }
+            sts64(pcur + (unsigned)((u % PF) * kRowB), acc[(u + 1) % MB]);   // window gamma-(MB-1) complete
+            // column sums of the previous batch, one stage per row
+            if (u % PF == 0) stage_B();
+            else if (u % PF == 1) stage_C();
+            else if (u % PF == 2) stage_D();
+            else if (u % PF == 3) stage_E();
+            else if (u % PF == 4) stage_F();
+            if (u % PF == PF - 1) {                                 // batch complete: it becomes "previous"
+                __syncwarp();
+                rprev = (pcur - (unsigned)(lane * 8)) + rd_off;
+                v0 = lds64(rprev); v1 = lds64(rprev + 32); v2 = lds64(rprev + 64); v3 = lds64(rprev + 96);
+                kw_prev = blk * MB + (u - (PF - 1)) - (MB - 1);
+                have_prev = true;
+                const unsigned tmp = pcur; pcur = pother; pother = tmp;
+            }
+        }
+    }
+    // drain: the last batch's sums
+    stage_B(); stage_C(); stage_D(); stage_E(); stage_F();
+    cp_async_wait<0>();
+    __syncwarp();
+}
+
 __device__ __forceinline__ double tmpl_lerp(const double* __restrict__ tm, int n_tmpl, int j, double tscale) {
     const double u = ((double)j + 0.5) * tscale;
     int k = (int)u;                                   // u >= 0: truncation == floor
@@ -323,7 +459,7 @@ __device__ __forceinline__ double tmpl_lerp(const double* __restrict__ tm, int n
 
 // One march of the lanes' (segment, column) slots: taps, bounds, then the ring.
 //   seg/col: this lane's slot (active == false: an idle lane, zero taps);  row0: first row of seg.
-template <int MB>
+template <int MB, bool PIPE>
 __device__ __forceinline__ void run_march(const Cls& c, const It& it, const int n, const int n_tmpl,
                                           const double tscale, const double* __restrict__ tm,
                                           const double* __restrict__ x, const bool square,
@@ -347,7 +483,8 @@ __device__ __forceinline__ void run_march(const Cls& c, const It& it, const int 
         rows_valid = rv > rows_all ? rows_all : (int)rv;
     }
     const int rows_min = __reduce_min_sync(0xffffffffu, rows_valid);
-    march<MB>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane, best);
+    if constexpr (PIPE) march_pipe<MB>(c, it, x + ebase, rows_valid, nblk, T, lane);
+    else march<MB>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane, best);
 }
 
 template <int MB, bool NARROW>
@@ -371,7 +508,7 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
         const bool active = lane < it.slots;
         const int seg = active ? lane / c.stp : 0;
         const int col = active ? lane - seg * c.stp : 0;
-        run_march<MB>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best);
+        run_march<MB, false>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best);
         return;
     }
     // ---- wide: window tiles of the table size, flat (segment, column) slots ------------------------
@@ -413,8 +550,12 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
                 const bool active = f < it.slots;
                 const int seg = active ? f / c.stp : 0;
                 const int col = active ? f - seg * c.stp : 0;
-                run_march<MB>(c, it, n, n_tmpl, tscale, tm, pass == 0 ? x1 : x0, pass == 1, active,
-                              k0 + seg * it.L, col, lane, best);
+                if (PfRows<MB>::v >= 6 && it.ng <= 2)
+                    run_march<MB, (PfRows<MB>::v >= 6)>(c, it, n, n_tmpl, tscale, tm, pass == 0 ? x1 : x0,
+                                                        pass == 1, active, k0 + seg * it.L, col, lane, best);
+                else
+                    run_march<MB, false>(c, it, n, n_tmpl, tscale, tm, pass == 0 ? x1 : x0, pass == 1, active,
+                                         k0 + seg * it.L, col, lane, best);
             }
         }
         __syncwarp();
