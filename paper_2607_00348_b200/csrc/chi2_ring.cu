@@ -312,17 +312,18 @@ __device__ __forceinline__ void march(const Cls& c, const It& it, const double* 
     }
 }
 
-// Wide path, at most two segments per warp: the same march as a software pipeline.  A warp issues in
-// order, so every load is placed at least one row (MB DFMAs) before its first use:
-//   - the X value of row j+LA is read from the FIFO while row j is multiplied, and its slot is refilled
-//     (cp.async) with row j+LA+MB at once (FIFO depth = MB rows);
+// Wide path, one segment per warp: the same march as a software pipeline.  A warp issues in order, so
+// every load is placed at least one row (MB DFMAs) before its first use:
+//   - the X value of row j+LA is read from the FIFO while row j is multiplied; whenever the reads enter a
+//     new group of PF rows, the PF slots of the group just left are refilled (cp.async) with their rows
+//     + MB in one burst (FIFO depth = MB rows);
 //   - the column sums of a completed batch of PF windows are spread over the rows of the NEXT batch:
-//     A (batch end) 4 loads, B 4 loads + first partial sums, C second partial sums, D/E the two shuffle
-//     steps and the table loads, F the table stores.  Two emit buffers alternate.
+//     A (batch end) 4 loads, B 4 loads + first partial sum, C second partial sum, D/E the two shuffle
+//     steps and the table load, F the table store.  Two emit buffers alternate.
 template <int MB>
 __device__ __forceinline__ void march_pipe(const Cls& c, const It& it, const double* __restrict__ xp,
-                                           const int rows_valid, const int nblk, const double (&T)[MB],
-                                           const int lane) {
+                                           const int rows_valid, const int rows_min, const int nblk,
+                                           const double (&T)[MB], const int lane) {
     constexpr int PF = PfRows<MB>::v;
     constexpr int NBAT = MB / PF;                  // copy groups in flight = batches per block
     constexpr int XQ = (MB % 3 == 0) ? 3 : 4;      // X registers; LA rows of look-ahead
@@ -347,77 +348,40 @@ __device__ __forceinline__ void march_pipe(const Cls& c, const It& it, const dou
     }
     cp_async_wait<NBAT - 1>();
 #pragma unroll
-    for (int k = 0; k < LA; ++k) {                 // rows 0 .. LA-1: read, refill the slot with row MB + k
-        const unsigned fa = fl + (unsigned)(k * 256);
-        xq[k] = lds64(fa);
-        cp_async8(fa, xp, row_issue < rows_valid);
-        xp += rstride;
-        ++row_issue;
-    }
+    for (int k = 0; k < LA; ++k) xq[k] = lds64(fl + (unsigned)(k * 256));
 
     // column-sum roles: lane = (window slot sl, quarter r); quarter r adds lanes r, r+4, ..., r+28
     const int sl = lane >> 2, r = lane & 3;
     const int slc = sl < PF ? sl : PF - 1;
     const unsigned rd_off = (unsigned)((slc * kPartPitch + r) * 8);
-    const bool two = it.ng == 2;
-    const int split = two ? (it.seg_first + 1) * c.stp - it.f0 : 32;
+    const bool my_slot = r == 0 && sl < PF;
+    const unsigned tab0 = it.tab + (unsigned)((it.seg_first * it.L + sl) * 8);
     unsigned pcur = c.part + (unsigned)(lane * 8);            // emit buffer of the running batch (my column)
     unsigned pother = pcur + (unsigned)(PF * kRowB);
     unsigned rprev = c.part + rd_off;                         // read base of the batch being summed
-    int kw_prev = 0;
-    bool have_prev = false;
-    double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0, sa = 0.0, sb = 0.0, ta = 0.0, tb = 0.0;
-    int wa = 0, wb = 0;
-    bool oka = false, okb = false;
-
-    auto masked = [&](const double v, const int q, double& a, double& b) {
-        if (q < split) a += v; else b += v;
-    };
-    auto stage_B = [&]() {          // first four values -> sums; load the other four
-        sa = 0.0; sb = 0.0;
-        if (!two) { sa = (v0 + v1) + (v2 + v3); }
-        else { masked(v0, r, sa, sb); masked(v1, r + 4, sa, sb); masked(v2, r + 8, sa, sb); masked(v3, r + 12, sa, sb); }
-        v0 = lds64(rprev + 128); v1 = lds64(rprev + 160); v2 = lds64(rprev + 192); v3 = lds64(rprev + 224);
-    };
-    auto stage_C = [&]() {
-        if (!two) { sa += (v0 + v1) + (v2 + v3); }
-        else { masked(v0, r + 16, sa, sb); masked(v1, r + 20, sa, sb); masked(v2, r + 24, sa, sb); masked(v3, r + 28, sa, sb); }
-    };
-    auto stage_D = [&]() {
-        sa += __shfl_xor_sync(0xffffffffu, sa, 1);
-        if (two) sb += __shfl_xor_sync(0xffffffffu, sb, 1);
-    };
-    auto stage_E = [&]() {
-        sa += __shfl_xor_sync(0xffffffffu, sa, 2);
-        if (two) sb += __shfl_xor_sync(0xffffffffu, sb, 2);
-        const int kw = kw_prev + sl;
-        const bool okk = have_prev && r == 0 && sl < PF && kw >= 0 && kw < it.L;
-        wa = it.seg_first * it.L + kw;
-        wb = wa + it.L;
-        oka = okk && wa < it.nWt;
-        okb = okk && two && wb < it.nWt;
-        ta = oka ? lds64(it.tab + (unsigned)(wa * 8)) : 0.0;
-        tb = okb ? lds64(it.tab + (unsigned)(wb * 8)) : 0.0;
-    };
-    auto stage_F = [&]() {
-        if (oka) sts64(it.tab + (unsigned)(wa * 8), ta + sa);
-        if (okb) sts64(it.tab + (unsigned)(wb * 8), tb + sb);
-    };
+    int kw_prev = -(1 << 30);                                 // no previous batch yet
+    double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0, sa = 0.0, ta = 0.0;
+    bool oka = false;
 
 #pragma unroll 1
     for (int blk = 0; blk < nblk; ++blk) {
 #pragma unroll
         for (int u = 0; u < MB; ++u) {
-            // X of row j+LA: FIFO -> register, slot refilled with row j+LA+MB
-            if ((u + LA) % PF == 0) cp_async_wait<NBAT - 1>();
-            {
-                const unsigned fa = fl + (unsigned)(((u + LA) % MB) * 256);
-                xq[(u + LA) % XQ] = lds64(fa);
-                cp_async8(fa, xp, row_issue < rows_valid);
-                xp += rstride;
-                ++row_issue;
-                if ((u + LA) % PF == PF - 1) cp_async_commit();
+            if ((u + LA) % PF == 0) {
+                // the reads enter a new group: refill the group just left, then make sure the new one landed
+                const int g0 = ((u + LA - PF) % MB + MB) % MB;   // (compile-time after unrolling)
+                if (row_issue + PF <= rows_min) {
+#pragma unroll
+                    for (int k = 0; k < PF; ++k) { cp_async8(fl + (unsigned)((g0 + k) * 256), xp); xp += rstride; }
+                } else {
+#pragma unroll
+                    for (int k = 0; k < PF; ++k) { cp_async8(fl + (unsigned)((g0 + k) * 256), xp, row_issue + k < rows_valid); xp += rstride; }
+                }
+                row_issue += PF;
+                cp_async_commit();
+                cp_async_wait<NBAT - 1>();
             }
+            xq[(u + LA) % XQ] = lds64(fl + (unsigned)(((u + LA) % MB) * 256));
             const double x = xq[u % XQ];
 #pragma unroll
             for (int m = 0; m < MB; ++m) {
@@ -427,23 +391,41 @@ __device__ __forceinline__ void march_pipe(const Cls& c, const It& it, const dou
             }
             sts64(pcur + (unsigned)((u % PF) * kRowB), acc[(u + 1) % MB]);   // window gamma-(MB-1) complete
             // column sums of the previous batch, one stage per row
-            if (u % PF == 0) stage_B();
-            else if (u % PF == 1) stage_C();
-            else if (u % PF == 2) stage_D();
-            else if (u % PF == 3) stage_E();
-            else if (u % PF == 4) stage_F();
+            if (u % PF == 0) {
+                sa = (v0 + v1) + (v2 + v3);
+                v0 = lds64(rprev + 128); v1 = lds64(rprev + 160); v2 = lds64(rprev + 192); v3 = lds64(rprev + 224);
+            } else if (u % PF == 1) {
+                sa += (v0 + v1) + (v2 + v3);
+            } else if (u % PF == 2) {
+                sa += __shfl_xor_sync(0xffffffffu, sa, 1);
+            } else if (u % PF == 3) {
+                sa += __shfl_xor_sync(0xffffffffu, sa, 2);
+                const int kw = kw_prev + sl;
+                oka = my_slot && kw >= 0 && kw < it.L && it.seg_first * it.L + kw < it.nWt;
+                ta = oka ? lds64(tab0 + (unsigned)(kw_prev * 8)) : 0.0;
+            } else if (u % PF == 4) {
+                if (oka) sts64(tab0 + (unsigned)(kw_prev * 8), ta + sa);
+            }
             if (u % PF == PF - 1) {                                 // batch complete: it becomes "previous"
                 __syncwarp();
                 rprev = (pcur - (unsigned)(lane * 8)) + rd_off;
                 v0 = lds64(rprev); v1 = lds64(rprev + 32); v2 = lds64(rprev + 64); v3 = lds64(rprev + 96);
                 kw_prev = blk * MB + (u - (PF - 1)) - (MB - 1);
-                have_prev = true;
                 const unsigned tmp = pcur; pcur = pother; pother = tmp;
             }
         }
     }
     // drain: the last batch's sums
-    stage_B(); stage_C(); stage_D(); stage_E(); stage_F();
+    sa = (v0 + v1) + (v2 + v3);
+    v0 = lds64(rprev + 128); v1 = lds64(rprev + 160); v2 = lds64(rprev + 192); v3 = lds64(rprev + 224);
+    sa += (v0 + v1) + (v2 + v3);
+    sa += __shfl_xor_sync(0xffffffffu, sa, 1);
+    sa += __shfl_xor_sync(0xffffffffu, sa, 2);
+    {
+        const int kw = kw_prev + sl;
+        if (my_slot && kw >= 0 && kw < it.L && it.seg_first * it.L + kw < it.nWt)
+            tab_add(tab0 + (unsigned)(kw_prev * 8), sa);
+    }
     cp_async_wait<0>();
     __syncwarp();
 }
@@ -483,7 +465,7 @@ __device__ __forceinline__ void run_march(const Cls& c, const It& it, const int 
         rows_valid = rv > rows_all ? rows_all : (int)rv;
     }
     const int rows_min = __reduce_min_sync(0xffffffffu, rows_valid);
-    if constexpr (PIPE) march_pipe<MB>(c, it, x + ebase, rows_valid, nblk, T, lane);
+    if constexpr (PIPE) march_pipe<MB>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane);
     else march<MB>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane, best);
 }
 
@@ -550,7 +532,7 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
                 const bool active = f < it.slots;
                 const int seg = active ? f / c.stp : 0;
                 const int col = active ? f - seg * c.stp : 0;
-                if (PfRows<MB>::v >= 6 && it.ng <= 2)
+                if (PfRows<MB>::v >= 6 && it.ng == 1)
                     run_march<MB, (PfRows<MB>::v >= 6)>(c, it, n, n_tmpl, tscale, tm, pass == 0 ? x1 : x0,
                                                         pass == 1, active, k0 + seg * it.L, col, lane, best);
                 else
