@@ -20,7 +20,7 @@
 // ceil(D/(c*st)) <= 21 taps and the array shifted by r*st.
 //
 // ONE WARP OWNS ONE TRIAL (period, duration) from its first row to its argmin: there is no CTA
-// barrier after the template nodes are staged, so the warps of an SM sit in different phases and
+// barrier after the template nodes are staged, so the warps of an SM (6 CTAs x 2 warps) sit in different phases and
 // the scoring of one hides behind the DFMAs of the others.
 //   stride > 16 ("wide"): lanes are assigned from a flat list of (row segment, column) pairs, so
 //     warps are full for every stride; windows are processed in tiles of the table size.
@@ -38,14 +38,14 @@ namespace gtls {
 
 namespace {
 
-constexpr int kRT = 128;                 // threads per CTA
+constexpr int kRT = 64;                  // threads per CTA (two trials: a CTA keeps its slot until both are done)
 constexpr int kRW = kRT / 32;            // warps (= trials) per CTA
 constexpr int kPartPitch = 36;           // doubles per slot row of the per-warp emit buffer
 constexpr int kPartRows = 16;            // two emit buffers of max PfRows rows (pipelined column sums)
 constexpr int kFifoBatches = 3;          // batches of PfRows rows per lane in the cp.async FIFO
 constexpr int kFifoRows = 24;            // >= kFifoBatches * max PfRows
 constexpr int kCW = 704;                 // window-table doubles per warp (>= 32 * 21)
-constexpr int kTmplSmem = 1024;          // template nodes cached in shared memory
+constexpr int kTmplSmem = 512;           // template nodes cached in shared memory
 constexpr int kWarpSmem = kPartRows * kPartPitch + kFifoRows * 32 + kCW;   // doubles per warp
 
 struct Cand { double d; double depth; int s; int has; };
@@ -547,7 +547,7 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
 }
 
 template <int MB, bool NARROW, bool UNIFORM>
-__global__ void __launch_bounds__(kRT, 3) k_chi2_ring(TileArgs a, const int* __restrict__ list,
+__global__ void __launch_bounds__(kRT, 6) k_chi2_ring(TileArgs a, const int* __restrict__ list,
                                                       const int* __restrict__ count) {
     extern __shared__ double dsm[];                 // per warp: emit buffer, X FIFO, window table
     __shared__ __align__(16) double s_tmpl[kTmplSmem];
