@@ -208,6 +208,20 @@ def test_search_shared_duration_grid_and_small_tiles(tmpl512):
         _check_search(w, res, ora, sde_kernel=3, label=f"shared/tile{tile}")
 
 
+@pytest.mark.parametrize("n_tmpl", [2, 7, 513, 1001, 2048])
+def test_search_template_sizes(n_tmpl):
+    """Templates that do not fit the shared-memory cache (> 512 nodes: read from global memory) or that
+    the TMA bulk copy cannot take (odd node count -> size not a multiple of 16 B)."""
+    _cuda()
+    import gtls_inputs as gi2
+    tm = gi2.transit_template(n_tmpl) if n_tmpl > 2 else np.array([1.0, 1.0])
+    w = gi.make_workload(1).subset(97)
+    ora = oracle.search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, tm, dt0=0.05)
+    res = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, tm, dt0=0.05, sde_kernel=5)
+    w2 = gi.Workload(w.name, w.lc, w.periods, w.durations, tm, w.dt0)
+    _check_search(w2, res, ora, sde_kernel=5, label=f"n_tmpl={n_tmpl}")
+
+
 def test_search_device_pointers_and_workspace():
     torch = _cuda()
     w = gi.make_workload(2).subset(301)
