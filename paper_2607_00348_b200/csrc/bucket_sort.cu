@@ -9,8 +9,8 @@
 //   k_bucket_scatter  fold again (t is L2 resident, the division is cheaper than 16 B of HBM) and
 //                     write (key32 << 32 | index) into its bucket, any order inside the bucket
 //   k_bucket_finish   one CTA per (period, bucket): the bucket (~1000 keys) is sorted entirely in shared
-//                     memory -- counting sort on the next 11 key bits, then an exact rank inside every
-//                     run of equal 11-bit codes by (key32, fp64 phase, index) -- gathered and scanned
+//                     memory -- counting sort on the next 10 key bits, then an exact rank inside every
+//                     run of equal 10-bit codes by (key32, fp64 phase, index) -- gathered and scanned
 //                     locally: permutation, x1 = w r (x0 = w), bucket-local S1 (S0) and the bucket's sums.
 //   k_prefix_fix      adds the sums of the period's earlier buckets (fixed order) to the local prefixes.
 //   k_pad_scan        wrap padding (Fig. 3): the first D_m sorted entries again, the sums run on.
@@ -27,9 +27,9 @@ namespace {
 constexpr int kCountThreads = 256;
 constexpr int kCountItems = 8;                       // points per thread in count / scatter
 constexpr int kFinThreads = 256;                     // one CTA per bucket
-constexpr int kFinItems = kBucketCap / kFinThreads;  // sorted entries per thread (8)
+constexpr int kFinItems = kBucketCap / kFinThreads;  // sorted entries per thread (6)
 constexpr int kPadThreads = 512;
-constexpr int kSubBits = 11;
+constexpr int kSubBits = 10;
 constexpr int kSub = 1 << kSubBits;                  // sub-buckets of the local counting sort
 constexpr int kScanItems = 4;                        // pad scan: entries per thread and round
 
@@ -147,10 +147,10 @@ __global__ void __launch_bounds__(kFinThreads) k_bucket_finish(BucketArgs b) {
     for (int i = tid; i < m; i += kFinThreads) A[i] = keys[i];
     for (int k = tid; k < kSub; k += kFinThreads) H[k] = 0;
     __syncthreads();
-    // 2. histogram of the next 11 key bits
+    // 2. histogram of the next 10 key bits
     for (int i = tid; i < m; i += kFinThreads) atomicAdd(&H[((u32)(A[i] >> 32) >> subshift) & (kSub - 1)], 1u);
     __syncthreads();
-    // 3. exclusive scan of the kSub counts (8 per thread)
+    // 3. exclusive scan of the kSub counts (4 per thread)
     {
         constexpr int PER = kSub / kFinThreads;
         u32 c[PER], sum = 0;
@@ -175,7 +175,7 @@ __global__ void __launch_bounds__(kFinThreads) k_bucket_finish(BucketArgs b) {
         B[atomicAdd(&H[((u32)(k >> 32) >> subshift) & (kSub - 1)], 1u)] = k;
     }
     __syncthreads();
-    // 5. exact rank inside every run of equal 11-bit codes
+    // 5. exact rank inside every run of equal 10-bit codes
     for (int i = tid; i < m; i += kFinThreads) {
         const u64 k = B[i];
         const u32 sb = ((u32)(k >> 32) >> subshift) & (kSub - 1);

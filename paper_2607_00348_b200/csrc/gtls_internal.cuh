@@ -47,7 +47,7 @@ constexpr int kChi2NarrowMax = 16;   // largest class stride handled by the narr
 // bucket sort (bucket_sort.cu)
 constexpr int kMaxBuckets = 256;      // buckets per period (power of two)
 constexpr int kBucketTarget = 1100;   // aimed-at mean bucket size
-constexpr int kBucketCap = 2048;      // largest bucket the shared-memory sort takes; beyond: LSD fallback
+constexpr int kBucketCap = 1536;      // largest bucket the shared-memory sort takes; beyond: LSD fallback
 
 constexpr int kRadixThreads = 256;
 constexpr int kRadixItems = 8;

@@ -79,7 +79,7 @@ def test_fold_sort_ties_and_tiny_inputs():
 
 
 def test_fold_sort_clustered_phases_take_the_lsd_fallback(tmpl512):
-    """More than kBucketCap (2048) points share one phase bucket: the bucket fast path raises its
+    """More than kBucketCap (1536) points share one phase bucket: the bucket fast path raises its
     fallback flag and the call is repeated on the LSD radix path; results must not change."""
     _cuda()
     rng = np.random.default_rng(11)
