@@ -493,51 +493,33 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
         run_march<MB, false>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best);
         return;
     }
-    // ---- wide: window tiles of the table size, flat (segment, column) slots ------------------------
+    // ---- wide: window tiles of the table size; the tile's stp columns are cut into nc balanced chunks of
+    // at most 32 lanes, one march per chunk over all rows of the tile (one segment per warp: a few idle
+    // lanes when stp is just above a multiple of 32, but no halo rows between segments and every march
+    // takes the pipelined path).
     it.narrow = false; it.direct = false;
     it.G = 0; it.KB = 0; it.SL = 0; it.SLn = 0; it.invSL = 0.f;
+    constexpr bool kPipe = PfRows<MB>::v >= 6;
+    const int nc = (c.stp + 31) >> 5;
+    const int cw = (c.stp + nc - 1) / nc;
     for (int k0 = 0; k0 < c.nWr; k0 += c.Kt) {
         const int nWt = min(c.Kt, c.nWr - k0);
-        // segment count: minimise items * rows per item (one warp runs them all)
-        int bc = 0x7fffffff, bn = 1;
-#pragma unroll
-        for (int r = 0; r < 2; ++r) {
-            const int ns = lane + 1 + 32 * r;
-            if (ns <= nWt) {
-                const int L = (nWt + ns - 1) / ns;
-                const int items = (ns * c.stp + 31) >> 5;
-                const int cost = items * (((L + 2 * MB - 2) / MB) * MB + 8);
-                if (cost < bc) { bc = cost; bn = ns; }
-            }
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            const int oc = __shfl_xor_sync(0xffffffffu, bc, o), on = __shfl_xor_sync(0xffffffffu, bn, o);
-            if (oc < bc || (oc == bc && on < bn)) { bc = oc; bn = on; }
-        }
-        const int nseg = bn;
-        it.L = (nWt + nseg - 1) / nseg;
-        it.slots = nseg * c.stp;
+        it.L = nWt;
+        it.slots = c.stp;
         it.nWt = nWt;
-        const int items = (it.slots + 31) >> 5;
+        it.seg_first = 0;
+        it.ng = 1;
         for (int i = lane; i < (c.uniform ? nWt : c.Kt + nWt); i += 32) sts64(c.ctab + (unsigned)(i * 8), 0.0);
         __syncwarp();
         for (int pass = 0; pass < (c.uniform ? 1 : 2); ++pass) {
             it.tab = c.ctab + (unsigned)(pass * c.Kt * 8);
-            for (int item = 0; item < items; ++item) {
-                it.f0 = item << 5;
-                it.seg_first = it.f0 / c.stp;
-                it.ng = min(it.f0 + 31, it.slots - 1) / c.stp - it.seg_first + 1;
-                const int f = it.f0 + lane;
-                const bool active = f < it.slots;
-                const int seg = active ? f / c.stp : 0;
-                const int col = active ? f - seg * c.stp : 0;
-                if (PfRows<MB>::v >= 6 && it.ng == 1)
-                    run_march<MB, (PfRows<MB>::v >= 6)>(c, it, n, n_tmpl, tscale, tm, pass == 0 ? x1 : x0,
-                                                        pass == 1, active, k0 + seg * it.L, col, lane, best);
-                else
-                    run_march<MB, false>(c, it, n, n_tmpl, tscale, tm, pass == 0 ? x1 : x0, pass == 1, active,
-                                         k0 + seg * it.L, col, lane, best);
+            for (int ch = 0; ch < nc; ++ch) {
+                const int c0 = ch * cw;
+                it.f0 = c0;
+                const bool active = lane < cw && c0 + lane < c.stp;
+                const int col = active ? c0 + lane : 0;
+                run_march<MB, kPipe>(c, it, n, n_tmpl, tscale, tm, pass == 0 ? x1 : x0, pass == 1, active, k0,
+                                     col, lane, best);
             }
         }
         __syncwarp();

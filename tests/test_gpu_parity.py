@@ -197,6 +197,17 @@ def test_search_large_curves_sampled_periods(cfg, count):
     assert np.array_equal(perm, pm_o)
 
 
+@pytest.mark.parametrize("curve", [0, 1, 2, 7])
+def test_search_survey_curves_c5(curve):
+    """c5 (survey batch): independent 90-day curves with their own noise level, half with an injected
+    transit; per-curve agreement of chi2, indices, SDE and best period on a period subset."""
+    _cuda()
+    w = gi.make_workload(5, curve=curve).subset(53)
+    ora = oracle.search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05)
+    res = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05, sde_kernel=31)
+    _check_search(w, res, ora, sde_kernel=31, label=w.name)
+
+
 def test_search_shared_duration_grid_and_small_tiles(tmpl512):
     _cuda()
     w = gi.make_workload(1).subset(61)
