@@ -488,8 +488,8 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
         it.invSL = 1.0f / (float)it.SL;
         it.f0 = 0; it.seg_first = 0; it.ng = it.G; it.slots = it.G * c.stp; it.nWt = c.nWr;
         const bool active = lane < it.slots;
-        const int seg = active ? lane / c.stp : 0;
-        const int col = active ? lane - seg * c.stp : 0;
+        const int seg = min(lane / c.stp, it.G - 1);
+        const int col = lane - seg * c.stp;      // idle lanes read on behind the last segment (zero taps)
         run_march<MB, false>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best);
         return;
     }
@@ -517,7 +517,8 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
                 const int c0 = ch * cw;
                 it.f0 = c0;
                 const bool active = lane < cw && c0 + lane < c.stp;
-                const int col = active ? c0 + lane : 0;
+                const int col = c0 + lane;     // idle lanes read on behind the chunk (zero taps): the warp's
+                                               // copies stay one contiguous, conflict-free 256-byte row
                 run_march<MB, kPipe>(c, it, n, n_tmpl, tscale, tm, pass == 0 ? x1 : x0, pass == 1, active, k0,
                                      col, lane, best);
             }
