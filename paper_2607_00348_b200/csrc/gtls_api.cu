@@ -277,7 +277,13 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
         if (((uintptr_t)ws.base & 255) != 0) return GTLS_EINVAL;
         if (ws.size < worst.fixed + align_up(worst.per_period)) return GTLS_ENOMEM;
     } else {
-        const size_t need = gtls_workspace_bytes(n, n_per, n_dur, &o);
+        // own scratch: the automatic tile, shrunk so that it takes at most half of the free device memory
+        size_t need = gtls_workspace_bytes(n, n_per, n_dur, &o);
+        size_t free_b = 0, total_b = 0;
+        if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && need > free_b / 2) {
+            const size_t floor_b = worst.fixed + align_up(worst.per_period) + 64 * 256;
+            need = free_b / 2 > floor_b ? free_b / 2 : floor_b;
+        }
         if ((rc = alloc_arena(ws, need))) return rc;
     }
     double* d_wr = ws.take<double>(n);

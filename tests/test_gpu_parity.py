@@ -208,6 +208,28 @@ def test_search_survey_curves_c5(curve):
     _check_search(w, res, ora, sde_kernel=31, label=w.name)
 
 
+@pytest.mark.parametrize("dt0", [0.2, 0.5, 1.0, 3.0])
+def test_search_large_skip_fractions(dt0):
+    """Large dt0: few taps per window (ring sizes 8 and 4, generic march), stride up to and beyond D."""
+    _cuda()
+    w = gi.make_workload(2).subset(307)
+    ora = oracle.search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=dt0)
+    res = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=dt0, sde_kernel=5)
+    _check_search(w, res, ora, sde_kernel=5, label=f"dt0={dt0}")
+
+
+def test_fold_sort_very_long_curve_uses_lsd_path():
+    """n beyond 256 buckets x 1536 keys: every period overflows its buckets and goes through the LSD path."""
+    _cuda()
+    rng = np.random.default_rng(21)
+    n = 420_000
+    t = np.sort(rng.uniform(0, 3000, n))
+    periods = np.array([1.2345, 77.7])
+    _, perm = g.gtls_fold_sort(t, periods, want_phase=False)
+    _, pm_o = oracle.fold_sort(t, periods, want_phase=False)
+    assert np.array_equal(perm, pm_o)
+
+
 def test_search_shared_duration_grid_and_small_tiles(tmpl512):
     _cuda()
     w = gi.make_workload(1).subset(61)
