@@ -100,9 +100,9 @@ class ClockSampler:
                 "power_w_max": float(max(pw)), "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def build_workload(name: str, curve: int = 0, every: int = 1):
+def build_workload(name: str, curve: int = 0, every: int = 1, dt0=None):
     cfg = int(name[1])
-    w = gi.make_workload(cfg, curve=curve)
+    w = gi.make_workload(cfg, curve=curve) if dt0 is None else gi.make_workload(cfg, curve=curve, dt0=float(dt0))
     return w.subset(every) if every > 1 else w
 
 
@@ -176,6 +176,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--period-tile", type=int, default=0)
+    ap.add_argument("--dt0", type=float, default=None,
+                    help="T0 skip fraction of Eq. 18 (default: the workload's 0.05); the paper's sweep is 0.1 .. 0.01")
     ap.add_argument("--every", type=int, default=1,
                     help="profiling aid: search only every k-th period of the workload (default 1 = the "
                          "full workload; any other value is named in config.workload)")
@@ -188,7 +190,7 @@ def main():
     if args.impl == "reference":
         if rank != 0:
             return 0
-        w = build_workload(args.workload, every=args.every)
+        w = build_workload(args.workload, every=args.every, dt0=args.dt0)
         print(json.dumps(run_reference(args, w)), flush=True)
         return 0
 
@@ -205,7 +207,7 @@ def main():
     g.load_library()
 
     # every rank searches its own curve of the same shape (independent problems)
-    w = build_workload(args.workload, curve=rank, every=args.every)
+    w = build_workload(args.workload, curve=rank, every=args.every, dt0=args.dt0)
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(devname)
     d_in = [dev(x) for x in (w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl)]
     ws = torch.empty(g.gtls_workspace_bytes(w.lc.n, w.n_per, w.n_dur, args.period_tile), dtype=torch.uint8,
