@@ -148,6 +148,25 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
                 double* out_sde_raw, double* out_sde,
                 gtls_summary* out_summary);
 
+/* Two-stage hierarchical search (section 2.5).
+ *   Stage 1: gtls_search over all periods with opts->dt0 (the coarse T0 skip of Eq. 18).
+ *   Stage 2: the n_refine trial periods of highest SDE after stage 1 (ties -> lower index; the paper uses
+ *            ~200) are searched again with stride 1 (every trial T0, "without skipping");
+ *            their chi2 / best records replace the stage-1 values, then SR, SDE_raw, SDE and the summary
+ *            are recomputed over the whole grid (a9).
+ * Arguments as gtls_search.  out_best is required here.  out_refined [min(n_refine, n_per)] (int64
+ * indices into period_grid in selection order; host or device like the other arrays) may be NULL.
+ * n_refine <= 0 is GTLS_EINVAL.  A degenerate stage-1 spectrum returns GTLS_EDEGENERATE without stage 2.
+ * The SNR statistic the paper mentions for stage 2 is not defined in the paper and is not computed. */
+int gtls_search_two_stage(const double* t, const double* y, const double* dy, int64_t n,
+                          const double* period_grid, int64_t n_per,
+                          const double* duration_grid, int32_t n_dur,
+                          const double* tmpl, int32_t n_tmpl,
+                          const gtls_opts* opts, int32_t n_refine,
+                          double* out_chi2, gtls_best* out_best,
+                          double* out_sde_raw, double* out_sde,
+                          int64_t* out_refined, gtls_summary* out_summary);
+
 /* Parity / debug export of steps a1-a2: phases (Eq. 10) and the stable phase-sort permutation
  * for each period.  out_phase [n_per*n] may be NULL; out_perm [n_per*n] (int32) is required.
  * out_phase[ip*n + i] is the phase of input point i; out_perm[ip*n + s] is the input index at

@@ -167,3 +167,35 @@ def sde(chi2, kernel: int = 151) -> SdeResult:
     rc = lib().oracle_sde(cp, n, int(kernel), sr.ctypes.data_as(_dp), raw.ctypes.data_as(_dp),
                           out.ctypes.data_as(_dp), C.byref(ib), C.byref(im))
     return SdeResult(sr, raw, out, int(ib.value), int(im.value), bool(rc))
+
+
+@dataclass
+class TwoStageResult:
+    chi2: np.ndarray
+    best: np.ndarray
+    sde: SdeResult
+    refined: np.ndarray        # indices of the refined periods, in selection order
+    coarse_sde: np.ndarray     # SDE after stage 1 (what the selection ranked)
+    windows: int
+
+
+def search_two_stage(t, y, dy, periods, durations, tmpl, dt0: float = 0.05, n_refine: int = 200,
+                     sde_kernel: int = 151) -> TwoStageResult:
+    """Two-stage hierarchical search, PAPER.md:293-295 (section 2.5), step by step:
+    stage 1 = the search with the T0 skip of Eq. 18 over all periods; stage 2 = the n_refine periods of
+    highest SDE (ties: lower index) searched again without skipping (stride 1); their chi2 / best replace
+    the stage-1 values; SR / SDE are then recomputed over the whole grid."""
+    periods = np.ascontiguousarray(np.atleast_1d(periods), dtype=np.float64)
+    durations = np.ascontiguousarray(durations, dtype=np.float64)
+    r1 = search(t, y, dy, periods, durations, tmpl, dt0=dt0)
+    s1 = sde(r1.chi2, sde_kernel)
+    k = min(int(n_refine), periods.size)
+    order = np.argsort(-s1.sde, kind="stable")[:k]        # highest SDE first, ties keep the lower index
+    dur2 = durations[order] if durations.ndim == 2 else np.tile(durations, (k, 1))
+    r2 = search(t, y, dy, periods[order], dur2, tmpl, dt0=0.0)
+    chi2 = r1.chi2.copy()
+    best = r1.best.copy()
+    chi2[order] = r2.chi2
+    best[order] = r2.best
+    return TwoStageResult(chi2, best, sde(chi2, sde_kernel), order.astype(np.int64), s1.sde,
+                          r1.windows + r2.windows)

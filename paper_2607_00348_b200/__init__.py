@@ -20,7 +20,7 @@ from typing import Any, Optional
 
 import numpy as np
 
-__all__ = ["gtls_search", "gtls_fold_sort", "gtls_fold_scan", "gtls_window_chi2", "gtls_sde",
+__all__ = ["gtls_search", "gtls_search_two_stage", "gtls_fold_sort", "gtls_fold_scan", "gtls_window_chi2", "gtls_sde",
            "gtls_workspace_bytes", "gtls_strerror", "gtls_version", "GtlsError", "SearchResult",
            "BEST_DTYPE", "lib_path", "load_library"]
 
@@ -98,6 +98,10 @@ def load_library():
     lib.gtls_search.argtypes = [dp, dp, dp, C.c_int64, dp, C.c_int64, dp, C.c_int32, dp, C.c_int32,
                                 C.POINTER(GtlsOpts), dp, vp, dp, dp, C.POINTER(GtlsSummary)]
     lib.gtls_search.restype = C.c_int
+    lib.gtls_search_two_stage.argtypes = [dp, dp, dp, C.c_int64, dp, C.c_int64, dp, C.c_int32, dp, C.c_int32,
+                                          C.POINTER(GtlsOpts), C.c_int32, dp, vp, dp, dp, vp,
+                                          C.POINTER(GtlsSummary)]
+    lib.gtls_search_two_stage.restype = C.c_int
     lib.gtls_fold_sort.argtypes = [dp, C.c_int64, dp, C.c_int64, C.POINTER(GtlsOpts), dp, ip]
     lib.gtls_fold_sort.restype = C.c_int
     lib.gtls_fold_scan.argtypes = [dp, dp, dp, C.c_int64, C.c_double, C.c_int64, C.POINTER(GtlsOpts),
@@ -243,6 +247,48 @@ def gtls_search(t, y, dy, period_grid, duration_grid, tmpl, *, dt0: float = 0.05
         raise GtlsError(rc, "gtls_search")
     return SearchResult(chi2, sde_raw, sde, best, summ.as_dict(), rc,
                         st.as_dict() if stats else None, [kt, ky, kd, kp, kq, km])
+
+
+def gtls_search_two_stage(t, y, dy, period_grid, duration_grid, tmpl, *, dt0: float = 0.05,
+                          n_refine: int = 200, sde_kernel: int = 151, period_tile: int = 0, workspace=None,
+                          stream=None):
+    """Two-stage hierarchical search (``gtls_search_two_stage`` in include/gtls.h): returns
+    (SearchResult, refined) with ``refined`` the int64 indices of the refined periods."""
+    lib = load_library()
+    kt, pt, dev = _prep(t)
+    ky, py, d2 = _prep(y)
+    kd, pd, d3 = _prep(dy)
+    kp, pp, d4 = _prep(period_grid)
+    kq, pq, d5 = _prep(duration_grid)
+    km, pm, d6 = _prep(tmpl)
+    if len({dev, d2, d3, d4, d5, d6}) != 1:
+        raise ValueError("all arrays must be either CUDA tensors or host arrays")
+    n, n_per, n_tmpl = int(kt.shape[0]), int(kp.shape[0]), int(km.shape[0])
+    per_period = 1 if kq.ndim == 2 else 0
+    n_dur = int(kq.shape[-1])
+    o = _opts(dev, kt, stream, dt0=float(dt0), sde_kernel=int(sde_kernel), dur_per_period=per_period,
+              period_tile=int(period_tile))
+    if workspace is not None:
+        o.workspace = workspace.data_ptr()
+        o.workspace_bytes = workspace.numel() * workspace.element_size()
+    chi2 = _empty((n_per,), kt)
+    sde_raw = _empty((n_per,), kt)
+    sde = _empty((n_per,), kt)
+    best = _empty((n_per, BEST_DTYPE.itemsize), kt, np.uint8)
+    k = min(int(n_refine), n_per)
+    if _is_torch(kt):
+        import torch
+        refined = torch.empty((max(k, 1),), dtype=torch.int64, device=kt.device)
+    else:
+        refined = np.empty((max(k, 1),), dtype=np.int64)
+    summ = GtlsSummary()
+    rc = lib.gtls_search_two_stage(pt, py, pd, n, pp, n_per, pq, n_dur, pm, n_tmpl, C.byref(o), int(n_refine),
+                                   _ptr(chi2), _ptr(best), _ptr(sde_raw), _ptr(sde), _ptr(refined),
+                                   C.byref(summ))
+    if rc not in (GTLS_OK, GTLS_EDEGENERATE):
+        raise GtlsError(rc, "gtls_search_two_stage")
+    res = SearchResult(chi2, sde_raw, sde, best, summ.as_dict(), rc, None, [kt, ky, kd, kp, kq, km])
+    return res, refined[:k]
 
 
 def gtls_fold_sort(t, periods, *, want_phase: bool = True, period_tile: int = 0, stream=None):

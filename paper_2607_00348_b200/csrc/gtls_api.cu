@@ -648,4 +648,106 @@ int gtls_sde(const double* chi2, int64_t n_per, const gtls_opts* opts, double* o
     return sc.degenerate ? GTLS_EDEGENERATE : GTLS_OK;
 }
 
+int gtls_search_two_stage(const double* t, const double* y, const double* dy, int64_t n,
+                          const double* period_grid, int64_t n_per, const double* duration_grid,
+                          int32_t n_dur, const double* tmpl, int32_t n_tmpl, const gtls_opts* opts,
+                          int32_t n_refine, double* out_chi2, gtls_best* out_best, double* out_sde_raw,
+                          double* out_sde, int64_t* out_refined, gtls_summary* out_summary) {
+    g_cuda_err[0] = 0;
+    const gtls_opts o = resolve_opts(opts);
+    if (!t || !y || !dy || !period_grid || !duration_grid || !tmpl || !out_chi2 || !out_best) return GTLS_EINVAL;
+    if (n < 3 || n_per < 1 || n_dur < 1 || n_tmpl < 2 || n_refine <= 0) return GTLS_EINVAL;
+    CU(cudaSetDevice(o.device));
+    cudaStream_t st = (cudaStream_t)o.stream;
+    const bool dev = o.pointers_on_device != 0;
+    const long long n_durs_total = o.dur_per_period ? n_per * (long long)n_dur : n_dur;
+    const int K = (int)(n_refine < n_per ? n_refine : n_per);
+
+    // device copies of everything (host mode), and the stage-2 scratch
+    Arena ar;
+    size_t bytes = align_up(n_per) + align_up((size_t)K * 8) * 3 + align_up((size_t)K * n_dur * 8) +
+                   align_up((size_t)K * sizeof(gtls_best)) + 2 * align_up(n_per * 8) + 32 * 256;
+    if (!dev)
+        bytes += 3 * align_up(n * 8) + align_up(n_per * 8) + align_up(n_durs_total * 8) + align_up(n_tmpl * 8) +
+                 align_up(n_per * 8) + align_up(n_per * sizeof(gtls_best));
+    int rc = alloc_arena(ar, bytes);
+    if (rc) return rc;
+    const double *d_t, *d_y, *d_dy, *d_per, *d_dur, *d_tmpl;
+    if ((rc = stage_in(t, n, dev, ar, st, &d_t))) return rc;
+    if ((rc = stage_in(y, n, dev, ar, st, &d_y))) return rc;
+    if ((rc = stage_in(dy, n, dev, ar, st, &d_dy))) return rc;
+    if ((rc = stage_in(period_grid, n_per, dev, ar, st, &d_per))) return rc;
+    if ((rc = stage_in(duration_grid, n_durs_total, dev, ar, st, &d_dur))) return rc;
+    if ((rc = stage_in(tmpl, n_tmpl, dev, ar, st, &d_tmpl))) return rc;
+    double* d_chi2 = dev ? out_chi2 : ar.take<double>(n_per);
+    gtls_best* d_best = dev ? out_best : ar.take<gtls_best>(n_per);
+    double* d_sde_raw = (dev && out_sde_raw) ? out_sde_raw : ar.take<double>(n_per);
+    double* d_sde = (dev && out_sde) ? out_sde : ar.take<double>(n_per);
+    unsigned char* d_mark = ar.take<unsigned char>(n_per);
+    long long* d_sel = ar.take<long long>(K);
+    double* d_per2 = ar.take<double>(K);
+    double* d_dur2 = ar.take<double>((size_t)K * n_dur);
+    double* d_chi2b = ar.take<double>(K);
+    gtls_best* d_bestb = ar.take<gtls_best>(K);
+    if (!d_bestb) return GTLS_ENOMEM;
+
+    // ---- stage 1: coarse search over all periods ---------------------------------------------------
+    gtls_opts o1 = o;
+    o1.pointers_on_device = 1;
+    o1.stats = nullptr;
+    gtls_summary s1, s2, s3;
+    memset(&s1, 0, sizeof(s1)); memset(&s2, 0, sizeof(s2)); memset(&s3, 0, sizeof(s3));
+    rc = gtls_search(d_t, d_y, d_dy, n, d_per, n_per, d_dur, n_dur, d_tmpl, n_tmpl, &o1, d_chi2, d_best,
+                     d_sde_raw, d_sde, &s1);
+    int rc_final = rc;
+    const bool refined = rc == GTLS_OK;
+    if (refined) {
+        // ---- stage 2: the K periods of highest SDE, every trial T0 -------------------------------------
+        launch_topk_sde(d_sde, n_per, K, d_mark, d_sel, st);
+        launch_gather_refine(d_per, d_dur, o.dur_per_period, n_dur, d_sel, K, d_per2, d_dur2, st);
+        gtls_opts o2 = o1;
+        o2.dt0 = 0.0;
+        o2.dur_per_period = 1;
+        o2.sde_kernel = 0;
+        rc = gtls_search(d_t, d_y, d_dy, n, d_per2, K, d_dur2, n_dur, d_tmpl, n_tmpl, &o2, d_chi2b, d_bestb,
+                         nullptr, nullptr, &s2);
+        if (rc != GTLS_OK && rc != GTLS_EDEGENERATE) return rc;
+        launch_merge_refined(d_sel, K, d_chi2b, d_bestb, d_chi2, d_best, st);
+        rc_final = gtls_sde(d_chi2, n_per, &o1, d_sde_raw, d_sde, &s3);
+        if (rc_final != GTLS_OK && rc_final != GTLS_EDEGENERATE) return rc_final;
+    } else if (rc != GTLS_EDEGENERATE) {
+        return rc;
+    }
+    if (out_summary) {
+        *out_summary = s1;
+        if (refined) {
+            out_summary->best_period_idx = s3.best_period_idx;
+            out_summary->chi2_min = s3.chi2_min;
+            out_summary->sde_raw_max = s3.sde_raw_max;
+            out_summary->sde_max = s3.sde_max;
+            out_summary->sde_argmax = s3.sde_argmax;
+            gtls_best b;
+            double period = 0.0;
+            CU(cudaMemcpyAsync(&b, d_best + s3.best_period_idx, sizeof(b), cudaMemcpyDeviceToHost, st));
+            CU(cudaMemcpyAsync(&period, d_per + s3.best_period_idx, sizeof(double), cudaMemcpyDeviceToHost, st));
+            CU(cudaStreamSynchronize(st));
+            out_summary->best_dur_idx = b.dur_idx; out_summary->best_start = b.start;
+            out_summary->best_period = period; out_summary->best_t0 = b.t0; out_summary->best_depth = b.depth;
+        }
+        out_summary->windows_evaluated = s1.windows_evaluated + s2.windows_evaluated;
+    }
+    const cudaMemcpyKind d2x = dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    if (out_refined && refined)
+        CU(cudaMemcpyAsync(out_refined, d_sel, (size_t)K * sizeof(long long), d2x, st));
+    if (!dev) {
+        CU(cudaMemcpyAsync(out_chi2, d_chi2, n_per * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(out_best, d_best, n_per * sizeof(gtls_best), cudaMemcpyDeviceToHost, st));
+        if (out_sde_raw) CU(cudaMemcpyAsync(out_sde_raw, d_sde_raw, n_per * sizeof(double), cudaMemcpyDeviceToHost, st));
+        if (out_sde) CU(cudaMemcpyAsync(out_sde, d_sde, n_per * sizeof(double), cudaMemcpyDeviceToHost, st));
+    }
+    CU(cudaStreamSynchronize(st));
+    CU(cudaGetLastError());
+    return rc_final;
+}
+
 }  // extern "C"

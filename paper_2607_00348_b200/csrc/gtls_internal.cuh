@@ -181,6 +181,12 @@ void launch_window_export(const TileArgs& a, const double* s2, double q, int32_t
                           double* out_depth, double* out_c_out, double* out_c_in, cudaStream_t st);
 void launch_perm_export(const TileArgs& a, const u64* sorted, int32_t* out_perm, cudaStream_t st);
 
+void launch_topk_sde(const double* sde, long long n, int K, unsigned char* mark, long long* sel, cudaStream_t st);
+void launch_gather_refine(const double* periods, const double* durs, int dur_per_period, int n_dur,
+                          const long long* sel, int K, double* per2, double* dur2, cudaStream_t st);
+void launch_merge_refined(const long long* sel, int K, const double* chi2b, const gtls_best* bestb, double* chi2,
+                          gtls_best* best, cudaStream_t st);
+
 struct SdeScratch {      // device scalars of the epilogue
     double chi2_min, mean_sr, sd_sr, sde_raw_best, sde_max;
     long long argmin, sde_argmax;

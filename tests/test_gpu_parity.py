@@ -269,6 +269,44 @@ def test_search_device_pointers_and_workspace():
     assert res.summary == host.summary
 
 
+@pytest.mark.parametrize("cfg,every,n_refine", [(1, 5, 40), (2, 37, 25), (1, 61, 500)])
+def test_two_stage_search_matches_oracle(cfg, every, n_refine):
+    """Section 2.5: coarse pass with skipped T0, stride-1 refinement of the n_refine
+    periods of highest SDE, merged spectrum.  The selection is compared as a set; periods whose coarse SDE
+    lies within 1e-9 of the selection threshold may swap (SDE differs by rounding between the two sides)."""
+    _cuda()
+    w = gi.make_workload(cfg).subset(every)
+    ora = oracle.search_two_stage(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.1,
+                                  n_refine=n_refine, sde_kernel=31)
+    res, refined = g.gtls_search_two_stage(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.1,
+                                           n_refine=n_refine, sde_kernel=31)
+    k = min(n_refine, w.n_per)
+    assert refined.shape == (k,) and len(set(refined.tolist())) == k
+    diff = set(refined.tolist()) ^ set(ora.refined.tolist())
+    if k < w.n_per:
+        thr = np.sort(ora.coarse_sde)[::-1][k - 1]
+        assert all(abs(ora.coarse_sde[i] - thr) < 1e-9 for i in diff), diff
+    else:
+        assert not diff
+    same = np.ones(w.n_per, dtype=bool)
+    same[list(diff)] = False
+    chi2 = np.asarray(res.chi2)
+    rel = np.abs(chi2 - ora.chi2)[same] / ora.chi2[same]
+    assert rel.max() <= CHI2_RTOL
+    b = res.best()
+    assert np.array_equal(b["dur_idx"][same], ora.best["dur_idx"][same])
+    assert np.array_equal(b["start"][same], ora.best["start"][same])
+    assert np.array_equal(b["t0"][same], ora.best["t0"][same])
+    if not diff:
+        assert np.abs(np.asarray(res.sde) - ora.sde.sde).max() <= SDE_ATOL
+        assert res.summary["best_period_idx"] == ora.sde.best_period_idx
+        assert res.summary["windows_evaluated"] == ora.windows
+    # refinement can only lower chi2 (the stride-1 starts contain the strided ones)
+    coarse = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.1, sde_kernel=31)
+    assert np.all(chi2 <= np.asarray(coarse.chi2) * (1 + 1e-12))
+    assert np.all(chi2[np.setdiff1d(np.arange(w.n_per), refined)] == np.asarray(coarse.chi2)[np.setdiff1d(np.arange(w.n_per), refined)])
+
+
 def test_tiny_and_degenerate_inputs(tmpl512):
     _cuda()
     rng = np.random.default_rng(3)

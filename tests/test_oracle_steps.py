@@ -128,3 +128,23 @@ def test_sde_degenerate():
     assert s.degenerate and np.all(s.sde == 0)
     s = oracle.sde(np.full(10, 3.0), 5)
     assert s.degenerate and np.all(s.sde_raw == 0)
+
+
+def test_two_stage_refinement_properties(tmpl512):
+    """Section 2.5 (PAPER.md:293-295) on the oracle: n_refine >= n_per equals the stride-1 search;
+    refinement never raises chi2 and leaves unselected periods untouched; selection = highest SDE."""
+    import gtls_inputs as gi
+    w = gi.make_workload(1).subset(127)
+    full = oracle.search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, tmpl512, dt0=0.0)
+    coarse = oracle.search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, tmpl512, dt0=0.1)
+    ts_all = oracle.search_two_stage(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, tmpl512, dt0=0.1,
+                                     n_refine=10 ** 6, sde_kernel=5)
+    assert np.array_equal(ts_all.chi2, full.chi2) and np.array_equal(ts_all.best, full.best)
+    ts = oracle.search_two_stage(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, tmpl512, dt0=0.1,
+                                 n_refine=5, sde_kernel=5)
+    assert ts.refined.size == 5
+    assert np.all(ts.chi2 <= coarse.chi2)
+    rest = np.setdiff1d(np.arange(w.n_per), ts.refined)
+    assert np.array_equal(ts.chi2[rest], coarse.chi2[rest])
+    assert np.array_equal(ts.chi2[ts.refined], full.chi2[ts.refined])
+    assert ts.coarse_sde[ts.refined].min() >= np.delete(ts.coarse_sde, ts.refined).max()
