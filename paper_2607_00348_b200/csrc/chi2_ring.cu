@@ -22,8 +22,9 @@
 // ONE WARP OWNS ONE TRIAL (period, duration) from its first row to its argmin: there is no CTA
 // barrier after the template nodes are staged, so the warps of an SM (6 CTAs x 2 warps) sit in different phases and
 // the scoring of one hides behind the DFMAs of the others.
-//   stride > 16 ("wide"): lanes are assigned from a flat list of (row segment, column) pairs, so
-//     warps are full for every stride; windows are processed in tiles of the table size.
+//   stride > 16 ("wide"): the columns are cut into ceil(stride/32) balanced chunks; the warp marches
+//     one chunk at a time down the rows of a window tile (software-pipelined, march_pipe) and adds
+//     its per-window sums into the table; windows are processed in tiles of the table size.
 //   stride <= 16 ("narrow", short durations, very many windows): floor(32/stride) segments sit
 //     side by side in the warp, the whole class is ONE march of ~n/32 rows, and the table is a
 //     time slice that is scored and recycled every few blocks.
