@@ -33,6 +33,8 @@
 // S2 window term of Eq. 15 cancels against the same term of Eq. 16) and the lexicographic
 // (dchi2, start) argmin (a8) run from the table.
 // The template nodes are staged in shared memory with one TMA bulk copy (cp.async.bulk).
+#include <cstdlib>
+
 #include "gtls_internal.cuh"
 
 namespace gtls {
@@ -56,7 +58,7 @@ __device__ __forceinline__ void cand_offer(Cand& b, double d, int s, double dept
 }
 
 // rows per FIFO batch = completed windows reduced at once (divides MB)
-template <int MB> struct PfRows { static constexpr int v = (MB % 7 == 0) ? 7 : (MB >= 8 ? MB / 2 : MB); };
+template <int MB> struct PfRows { static constexpr int v = (MB % 7 == 0) ? 7 : (MB >= 16 ? 8 : (MB >= 8 ? MB / 2 : MB)); };
 
 __device__ __forceinline__ double lds64(const unsigned addr) {
     double v;
@@ -576,7 +578,7 @@ __global__ void __launch_bounds__(kRT, 6) k_chi2_ring(TileArgs a, const int* __r
     const int st = e.stride;
     const int nW = (a.n + st - 1) / st;
     const int M = (e.D + st - 1) / st;
-    const int ncls = (M + 20) / 21;                 // window classes: at most 21 taps each
+    const int ncls = chi2_classes(M, st);           // window classes: at most MB taps each
     Cls c;
     c.D = e.D; c.stp = ncls * st;
     c.uniform = UNIFORM;
@@ -630,25 +632,57 @@ static void launch_variant(const TileArgs& a, int v, cudaStream_t st) {
     k_chi2_ring<MB, NARROW, UNIFORM><<<grid, kRT, sm, st>>>(a, a.trial_list + (long long)v * trials, a.trial_count + v);
 }
 
+// The variants other than the dominant one (21-ring, wide) often hold few, long trials: alone on the
+// device they leave most warp slots empty.  They are launched on a side stream of higher priority between
+// two events, so their CTAs take slots first and the dominant kernel fills the rest of the device.
+struct SideStream {
+    cudaStream_t s = nullptr;
+    cudaEvent_t fork = nullptr, join = nullptr;
+    bool ok = false;
+    SideStream() {
+        int lo = 0, hi = 0;
+        if (cudaDeviceGetStreamPriorityRange(&lo, &hi) != cudaSuccess) return;
+        if (cudaStreamCreateWithPriority(&s, cudaStreamNonBlocking, hi) != cudaSuccess) return;
+        if (cudaEventCreateWithFlags(&fork, cudaEventDisableTiming) != cudaSuccess) return;
+        if (cudaEventCreateWithFlags(&join, cudaEventDisableTiming) != cudaSuccess) return;
+        ok = true;
+    }
+};
+
 void launch_chi2_ring(const TileArgs& a, cudaStream_t st) {
     launch_bin_trials(a, st);
+    static SideStream side;                     // (one device per process)
+    static const bool overlap = !(getenv("GTLS_CHI2_STREAMS") && atoi(getenv("GTLS_CHI2_STREAMS")) == 0);
+    cudaStream_t ss = st;
+    if (overlap && side.ok) {
+        cudaEventRecord(side.fork, st);
+        cudaStreamWaitEvent(side.s, side.fork, 0);
+        ss = side.s;
+    }
     if (a.uniform) {
-        launch_variant<21, false, true>(a, 0, st);
-        launch_variant<16, false, true>(a, 1, st);
-        launch_variant<12, false, true>(a, 2, st);
-        launch_variant<8, false, true>(a, 3, st);
-        launch_variant<4, false, true>(a, 4, st);
-        launch_variant<21, true, true>(a, 5, st);
-        launch_variant<16, true, true>(a, 6, st);
-        launch_variant<12, true, true>(a, 7, st);
-        launch_variant<8, true, true>(a, 8, st);
-        launch_variant<4, true, true>(a, 9, st);
+        launch_variant<12, true, true>(a, 9, ss);
+        launch_variant<16, true, true>(a, 8, ss);
+        launch_variant<8, true, true>(a, 10, ss);
+        launch_variant<4, true, true>(a, 11, ss);
+        launch_variant<24, true, true>(a, 6, ss);
+        launch_variant<21, true, true>(a, 7, ss);
+        launch_variant<24, false, true>(a, 0, ss);
+        launch_variant<16, false, true>(a, 2, ss);
+        launch_variant<12, false, true>(a, 3, ss);
+        launch_variant<8, false, true>(a, 4, ss);
+        launch_variant<4, false, true>(a, 5, ss);
+        launch_variant<21, false, true>(a, 1, st);
     } else {
-        launch_variant<21, false, false>(a, 0, st);
-        launch_variant<16, false, false>(a, 1, st);
-        launch_variant<12, false, false>(a, 2, st);
-        launch_variant<8, false, false>(a, 3, st);
-        launch_variant<4, false, false>(a, 4, st);
+        launch_variant<24, false, false>(a, 0, ss);
+        launch_variant<16, false, false>(a, 2, ss);
+        launch_variant<12, false, false>(a, 3, ss);
+        launch_variant<8, false, false>(a, 4, ss);
+        launch_variant<4, false, false>(a, 5, ss);
+        launch_variant<21, false, false>(a, 1, st);
+    }
+    if (ss != st) {
+        cudaEventRecord(side.join, ss);
+        cudaStreamWaitEvent(st, side.join, 0);
     }
 }
 

@@ -40,9 +40,19 @@ struct CurveInfo {
     int32_t pad_;
 };
 
-// chi2 ring kernel variants: ring size index (0..4 = 21, 16, 12, 8, 4 taps) + 5 * narrow
-constexpr int kChi2Variants = 10;
+// chi2 ring kernel variants: ring size index (0..5 = 24, 21, 16, 12, 8, 4 taps) + 6 * narrow
+constexpr int kChi2Rings = 6;
+constexpr int kChi2Variants = 2 * kChi2Rings;
 constexpr int kChi2NarrowMax = 16;   // largest class stride handled by the narrow variants
+// Window classes of a trial with M = ceil(D/stride) taps: the smallest count that leaves at most 24 taps
+// per class (21 when the stride is 1: 32 side-by-side segments of a 24-ring do not fit the window table).
+// (A 28-ring was measured: its unrolled body outgrows the instruction cache and spills; 2 classes win.)
+__host__ __device__ __forceinline__ int chi2_classes(int M, int stride) {
+    return stride == 1 ? (M + 20) / 21 : (M + 23) / 24;
+}
+__host__ __device__ __forceinline__ int chi2_ring_index(int taps) {
+    return taps > 21 ? 0 : (taps > 16 ? 1 : (taps > 12 ? 2 : (taps > 8 ? 3 : (taps > 4 ? 4 : 5))));
+}
 
 // bucket sort (bucket_sort.cu)
 constexpr int kMaxBuckets = 256;      // buckets per period (power of two)

@@ -126,12 +126,11 @@ __global__ void __launch_bounds__(256) k_durtab(TileArgs a) {
 __device__ __forceinline__ int chi2_variant(const DurEntry& e, const TileArgs& a) {
     if (e.skip || e.stride < a.dbg_min_st || e.stride > a.dbg_max_st) return -1;
     const int M = (e.D + e.stride - 1) / e.stride;
-    const int ncls = (M + 20) / 21;
+    const int ncls = chi2_classes(M, e.stride);
     const int stp = ncls * e.stride;
-    const int Mp = (e.D + stp - 1) / stp;
-    const int mbi = Mp > 16 ? 0 : (Mp > 12 ? 1 : (Mp > 8 ? 2 : (Mp > 4 ? 3 : 4)));
+    const int mbi = chi2_ring_index((e.D + stp - 1) / stp);
     const int narrow = (a.uniform && stp <= kChi2NarrowMax) ? 1 : 0;
-    return narrow * 5 + mbi;
+    return narrow * kChi2Rings + mbi;
 }
 
 // One CTA: every thread owns a contiguous chunk of trials, so the lists keep trial order (the
