@@ -171,11 +171,10 @@ __device__ __forceinline__ void score_narrow(const Cls& c, Cand& best, const int
     }
 }
 
-struct It {                              // one march: 32 lanes = 32 (segment, column) slots
-    bool narrow, direct;                 // narrow path; narrow with stride 1 (no cross-lane sum)
-    int L;                               // windows per segment
-    // wide: item geometry (flat slots f0 .. f0+31)
-    int f0, seg_first, ng, slots, nWt;
+struct It {                              // one march
+    bool direct;                         // narrow with stride 1: no cross-lane sum
+    int L;                               // windows per segment (wide: one segment = the window tile)
+    int nWt;                             // wide: windows in the tile
     // narrow: G segments side by side, table slice of SL = KB*MB windows per segment
     int G, KB, SL, SLn;                  // SL = odd pitch >= SLn = KB*MB valid windows per segment
     float invSL;
@@ -186,12 +185,12 @@ __device__ __forceinline__ void tab_add(const unsigned a, const double v) { sts6
 
 // PF completed window sums per lane sit in part[slot][lane] (windows kwb .. kwb+PF-1 of the lane's
 // segment): sum them over the lanes of each segment in fixed order.
-template <int PF>
+template <int PF, bool NARROW>
 __device__ __forceinline__ void reduce_batch(const Cls& c, const It& it, const int kwb, const int kw_base,
                                              const int lane) {
     __syncwarp();
-    if (!it.narrow && it.ng == 1) {
-        // four lanes per slot, eight strided values each, two shuffle steps
+    if constexpr (!NARROW) {
+        // wide: the warp holds one segment; four lanes per slot, eight strided values each, two shuffle steps
         const int sl = lane >> 2, r = lane & 3;
         double v = 0.0;
         if (sl < PF) {
@@ -203,24 +202,8 @@ __device__ __forceinline__ void reduce_batch(const Cls& c, const It& it, const i
         }
         v += __shfl_xor_sync(0xffffffffu, v, 1);
         v += __shfl_xor_sync(0xffffffffu, v, 2);
-        const int kw = kwb + sl, w = it.seg_first * it.L + kw;
-        if (r == 0 && sl < PF && kw >= 0 && kw < it.L && w < it.nWt) tab_add(it.tab + (unsigned)(w * 8), v);
-    } else if (!it.narrow) {
-        for (int t = lane; t < it.ng * PF; t += 32) {
-            const int gi = t / PF, sl = t - gi * PF;
-            const int seg = it.seg_first + gi;
-            int lo = seg * c.stp - it.f0, hi = lo + c.stp;
-            lo = lo < 0 ? 0 : lo;
-            hi = hi > 32 ? 32 : hi;
-            hi = hi > it.slots - it.f0 ? it.slots - it.f0 : hi;
-            const unsigned pr = c.part + (unsigned)(sl * kPartPitch * 8);
-            double a0 = 0.0, a1 = 0.0;
-            int q = lo;
-            for (; q + 1 < hi; q += 2) { a0 += lds64(pr + 8 * q); a1 += lds64(pr + 8 * q + 8); }
-            if (q < hi) a0 += lds64(pr + 8 * q);
-            const int kw = kwb + sl, w = seg * it.L + kw;
-            if (kw >= 0 && kw < it.L && w < it.nWt) tab_add(it.tab + (unsigned)(w * 8), a0 + a1);
-        }
+        const int kw = kwb + sl;
+        if (r == 0 && sl < PF && kw >= 0 && kw < it.L && kw < it.nWt) tab_add(it.tab + (unsigned)(kw * 8), v);
     } else {
         for (int t = lane; t < it.G * PF; t += 32) {
             const int g = t / PF, sl = t - g * PF;
@@ -239,7 +222,7 @@ __device__ __forceinline__ void reduce_batch(const Cls& c, const It& it, const i
 // >= rows_valid read as 0 (rows_min = the smallest rows_valid of the warp, so batches below it need
 // no predicate).  Taps T[m] multiply row (window + m).  Narrow path: every KB blocks the table slice
 // is scored and recycled.
-template <int MB>
+template <int MB, bool NARROW>
 __device__ __forceinline__ void march(const Cls& c, const It& it, const double* __restrict__ xp,
                                       const int rows_valid, const int rows_min, const int nblk,
                                       const double (&T)[MB], const int lane, Cand& best) {
@@ -293,13 +276,13 @@ __device__ __forceinline__ void march(const Cls& c, const It& it, const double* 
                 else acc[a] = fma(T[m], x, acc[a]);
             }
             // window gamma - (MB-1) is complete
-            const unsigned ea = it.direct ? tab_lane + (unsigned)((bis * MB + u) * 8)
+            const unsigned ea = (NARROW && it.direct) ? tab_lane + (unsigned)((bis * MB + u) * 8)
                                           : part_lane + (unsigned)((u % PF) * kPartPitch * 8);
             sts64(ea, acc[(u + 1) % MB]);
-            if (u % PF == PF - 1 && !it.direct)
-                reduce_batch<PF>(c, it, blk * MB + (u - (PF - 1)) - (MB - 1), kw_base, lane);
+            if (u % PF == PF - 1 && !(NARROW && it.direct))
+                reduce_batch<PF, NARROW>(c, it, blk * MB + (u - (PF - 1)) - (MB - 1), kw_base, lane);
         }
-        if (it.narrow && ++bis == it.KB) {
+        if (NARROW && ++bis == it.KB) {
             __syncwarp();
             score_narrow(c, best, lane, it.G, it.SL, it.SLn, it.invSL, kw_base, it.L);
             __syncwarp();
@@ -308,7 +291,7 @@ __device__ __forceinline__ void march(const Cls& c, const It& it, const double* 
         }
     }
     cp_async_wait<0>();
-    if (it.narrow && bis > 0) {
+    if (NARROW && bis > 0) {
         __syncwarp();
         score_narrow(c, best, lane, it.G, it.SL, it.SLn, it.invSL, kw_base, it.L);
         __syncwarp();
@@ -358,7 +341,7 @@ __device__ __forceinline__ void march_pipe(const Cls& c, const It& it, const dou
     const int slc = sl < PF ? sl : PF - 1;
     const unsigned rd_off = (unsigned)((slc * kPartPitch + r) * 8);
     const bool my_slot = r == 0 && sl < PF;
-    const unsigned tab0 = it.tab + (unsigned)((it.seg_first * it.L + sl) * 8);
+    const unsigned tab0 = it.tab + (unsigned)(sl * 8);
     unsigned pcur = c.part + (unsigned)(lane * 8);            // emit buffer of the running batch (my column)
     unsigned pother = pcur + (unsigned)(PF * kRowB);
     unsigned rprev = c.part + rd_off;                         // read base of the batch being summed
@@ -404,7 +387,7 @@ __device__ __forceinline__ void march_pipe(const Cls& c, const It& it, const dou
             } else if (u % PF == 3) {
                 sa += __shfl_xor_sync(0xffffffffu, sa, 2);
                 const int kw = kw_prev + sl;
-                oka = my_slot && kw >= 0 && kw < it.L && it.seg_first * it.L + kw < it.nWt;
+                oka = my_slot && kw >= 0 && kw < it.L && kw < it.nWt;
                 ta = oka ? lds64(tab0 + (unsigned)(kw_prev * 8)) : 0.0;
             } else if (u % PF == 4) {
                 if (oka) sts64(tab0 + (unsigned)(kw_prev * 8), ta + sa);
@@ -426,7 +409,7 @@ __device__ __forceinline__ void march_pipe(const Cls& c, const It& it, const dou
     sa += __shfl_xor_sync(0xffffffffu, sa, 2);
     {
         const int kw = kw_prev + sl;
-        if (my_slot && kw >= 0 && kw < it.L && it.seg_first * it.L + kw < it.nWt)
+        if (my_slot && kw >= 0 && kw < it.L && kw < it.nWt)
             tab_add(tab0 + (unsigned)(kw_prev * 8), sa);
     }
     cp_async_wait<0>();
@@ -444,7 +427,7 @@ __device__ __forceinline__ double tmpl_lerp(const double* __restrict__ tm, int n
 
 // One march of the lanes' (segment, column) slots: taps, bounds, then the ring.
 //   seg/col: this lane's slot (active == false: an idle lane, zero taps);  row0: first row of seg.
-template <int MB, bool PIPE>
+template <int MB, bool PIPE, bool NARROW>
 __device__ __forceinline__ void run_march(const Cls& c, const It& it, const int n, const int n_tmpl,
                                           const double tscale, const double* __restrict__ tm,
                                           const double* __restrict__ x, const bool square,
@@ -469,7 +452,7 @@ __device__ __forceinline__ void run_march(const Cls& c, const It& it, const int 
     }
     const int rows_min = __reduce_min_sync(0xffffffffu, rows_valid);
     if constexpr (PIPE) march_pipe<MB>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane);
-    else march<MB>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane, best);
+    else march<MB, NARROW>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane, best);
 }
 
 template <int MB, bool NARROW>
@@ -481,7 +464,7 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
     it.tab = c.ctab;
     if (NARROW) {
         // ---- narrow: G segments side by side, one march over the whole class -------------------
-        it.narrow = true; it.direct = c.stp == 1;   // (NARROW implies uniform dy and stp <= kChi2NarrowMax)
+        it.direct = c.stp == 1;   // (NARROW implies uniform dy and stp <= kChi2NarrowMax)
         it.G = 32 / c.stp;
         it.L = (c.nWr + it.G - 1) / it.G;
         it.KB = c.Kt / (it.G * MB);
@@ -489,18 +472,18 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
         it.SLn = it.KB * MB;
         it.SL = it.SLn | 1;
         it.invSL = 1.0f / (float)it.SL;
-        it.f0 = 0; it.seg_first = 0; it.ng = it.G; it.slots = it.G * c.stp; it.nWt = c.nWr;
-        const bool active = lane < it.slots;
+        it.nWt = c.nWr;
+        const bool active = lane < it.G * c.stp;
         const int seg = min(lane / c.stp, it.G - 1);
         const int col = lane - seg * c.stp;      // idle lanes read on behind the last segment (zero taps)
-        run_march<MB, false>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best);
+        run_march<MB, false, true>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best);
         return;
     }
     // ---- wide: window tiles of the table size; the tile's stp columns are cut into nc balanced chunks of
     // at most 32 lanes, one march per chunk over all rows of the tile (one segment per warp: a few idle
     // lanes when stp is just above a multiple of 32, but no halo rows between segments and every march
     // takes the pipelined path).
-    it.narrow = false; it.direct = false;
+    it.direct = false;
     it.G = 0; it.KB = 0; it.SL = 0; it.SLn = 0; it.invSL = 0.f;
     constexpr bool kPipe = PfRows<MB>::v >= 6;
     const int nc = (c.stp + 31) >> 5;
@@ -508,21 +491,17 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
     for (int k0 = 0; k0 < c.nWr; k0 += c.Kt) {
         const int nWt = min(c.Kt, c.nWr - k0);
         it.L = nWt;
-        it.slots = c.stp;
         it.nWt = nWt;
-        it.seg_first = 0;
-        it.ng = 1;
         for (int i = lane; i < (c.uniform ? nWt : c.Kt + nWt); i += 32) sts64(c.ctab + (unsigned)(i * 8), 0.0);
         __syncwarp();
         for (int pass = 0; pass < (c.uniform ? 1 : 2); ++pass) {
             it.tab = c.ctab + (unsigned)(pass * c.Kt * 8);
             for (int ch = 0; ch < nc; ++ch) {
                 const int c0 = ch * cw;
-                it.f0 = c0;
                 const bool active = lane < cw && c0 + lane < c.stp;
                 const int col = c0 + lane;     // idle lanes read on behind the chunk (zero taps): the warp's
                                                // copies stay one contiguous, conflict-free 256-byte row
-                run_march<MB, kPipe>(c, it, n, n_tmpl, tscale, tm, pass == 0 ? x1 : x0, pass == 1, active, k0,
+                run_march<MB, kPipe, false>(c, it, n, n_tmpl, tscale, tm, pass == 0 ? x1 : x0, pass == 1, active, k0,
                                      col, lane, best);
             }
         }
@@ -639,8 +618,10 @@ struct SideStream {
     cudaStream_t s = nullptr;
     cudaEvent_t fork = nullptr, join = nullptr;
     bool ok = false;
+    int dev = -1;
     SideStream() {
         int lo = 0, hi = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return;
         if (cudaDeviceGetStreamPriorityRange(&lo, &hi) != cudaSuccess) return;
         if (cudaStreamCreateWithPriority(&s, cudaStreamNonBlocking, hi) != cudaSuccess) return;
         if (cudaEventCreateWithFlags(&fork, cudaEventDisableTiming) != cudaSuccess) return;
@@ -651,10 +632,12 @@ struct SideStream {
 
 void launch_chi2_ring(const TileArgs& a, cudaStream_t st) {
     launch_bin_trials(a, st);
-    static SideStream side;                     // (one device per process)
+    static thread_local SideStream side;        // per host thread; bound to the device of its first call
+    int dev = -1;
+    cudaGetDevice(&dev);
     static const bool overlap = !(getenv("GTLS_CHI2_STREAMS") && atoi(getenv("GTLS_CHI2_STREAMS")) == 0);
     cudaStream_t ss = st;
-    if (overlap && side.ok) {
+    if (overlap && side.ok && dev == side.dev) {
         cudaEventRecord(side.fork, st);
         cudaStreamWaitEvent(side.s, side.fork, 0);
         ss = side.s;
