@@ -8,11 +8,11 @@
 //                     the period on the tile's fallback list, which the LSD path processes instead
 //   k_bucket_scatter  fold again (t is L2 resident, the division is cheaper than 16 B of HBM) and
 //                     write (key32 << 32 | index) into its bucket, any order inside the bucket
-//   k_bucket_finish   one CTA per (period, bucket): the bucket (~1000 keys) is sorted entirely in shared
-//                     memory -- counting sort on the next 10 key bits, then an exact rank inside every
-//                     run of equal 10-bit codes by (key32, fp64 phase, index) -- gathered and scanned
-//                     locally: permutation, x1 = w r (x0 = w), bucket-local S1 (S0) and the bucket's sums.
-//   k_prefix_fix      adds the sums of the period's earlier buckets (fixed order) to the local prefixes.
+//   k_bucket_finish   one CTA per period walks through its buckets in order: a bucket (~1000 keys) is
+//                     sorted entirely in shared memory -- counting sort on the next 10 key bits, then an
+//                     exact rank inside every run of equal 10-bit codes by (key32, fp64 phase, index) --
+//                     gathered and scanned with the running sums carried from bucket to bucket:
+//                     permutation, x1 = w r (x0 = w) and the final S1 (S0) in one pass.
 //   k_pad_scan        wrap padding (Fig. 3): the first D_m sorted entries again, the sums run on.
 //
 // The order inside a bucket before the local sort is irrelevant because the local sort orders by the
@@ -26,10 +26,20 @@ namespace {
 
 constexpr int kCountThreads = 256;
 constexpr int kCountItems = 8;                       // points per thread in count / scatter
-constexpr int kFinThreads = 256;                     // one CTA per bucket
+#ifndef GTLS_FIN_CTAS
+#define GTLS_FIN_CTAS 4
+#endif
+constexpr int kFinCtas = GTLS_FIN_CTAS;              // resident CTAs per SM the finish kernel is compiled for
+#ifndef GTLS_FIN_THREADS
+#define GTLS_FIN_THREADS 256
+#endif
+constexpr int kFinThreads = GTLS_FIN_THREADS;                     // one CTA per period
 constexpr int kFinItems = kBucketCap / kFinThreads;  // sorted entries per thread (6)
 constexpr int kPadThreads = 512;
-constexpr int kSubBits = 10;
+#ifndef GTLS_SUB_BITS
+#define GTLS_SUB_BITS 10
+#endif
+constexpr int kSubBits = GTLS_SUB_BITS;
 constexpr int kSub = 1 << kSubBits;                  // sub-buckets of the local counting sort
 constexpr int kScanItems = 4;                        // pad scan: entries per thread and round
 
@@ -125,188 +135,174 @@ __device__ __forceinline__ bool key_less(const u64 a, const u64 b, const double*
     return (u32)a < (u32)b;
 }
 
+// One CTA per PERIOD walks through the period's buckets in order, so the running prefix sums are carried
+// in registers from bucket to bucket (no look-back between CTAs, no second pass over S1), the next
+// bucket's keys are already on their way while the current bucket is sorted, and the per-CTA set-up is
+// paid once per period.
 template <bool HAS0, bool HAS2, bool SORT_ONLY>
-__global__ void __launch_bounds__(kFinThreads) k_bucket_finish(BucketArgs b) {
-    __shared__ u64 A[kBucketCap];
-    __shared__ u64 B[kBucketCap];
-    __shared__ u32 H[kSub + 1];                                // counts -> starts -> (after the scatter) ends
+__global__ void __launch_bounds__(kFinThreads, kFinCtas) k_bucket_finish(BucketArgs b) {
+    extern __shared__ __align__(16) unsigned char fin_smem[];
+    u64* const A = reinterpret_cast<u64*>(fin_smem);           // [kBucketCap]
+    u64* const B = A + kBucketCap;                             // [kBucketCap]
+    u32* const H = reinterpret_cast<u32*>(B + kBucketCap);     // [kSub + 1] counts -> starts -> (after the scatter) ends
     __shared__ double s_w[3][kFinThreads / 32];
-    __shared__ double s_base[3];
     __shared__ u32 s_wsum[kFinThreads / 32];
-    const int bk = blockIdx.x, pl = blockIdx.y;
+    const int pl = blockIdx.x;
     if (b.fb_flag[pl]) return;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NW = kFinThreads / 32;
     const double period = b.periods[b.p0 + pl];
     const u32* start = b.start + (long long)pl * (b.nbk + 1);
-    const int bs = (int)start[bk], m = (int)start[bk + 1] - bs;
-    const u64* keys = b.keys + (long long)pl * b.n + bs;
+    const u64* keys = b.keys + (long long)pl * b.n;
     const int subshift = b.shift - kSubBits;                   // sub-bucket = next kSubBits key bits
+    u32* perm = b.perm + (long long)pl * b.n;
+    double* x1 = b.x1 + (long long)pl * b.pitch;
+    double* x0 = HAS0 ? b.x0 + (long long)pl * b.pitch : nullptr;
+    double* x2 = HAS2 ? b.x2 + (long long)pl * b.pitch : nullptr;
+    double* s1 = b.s1 + (long long)pl * b.spitch;
+    double* s0 = HAS0 ? b.s0 + (long long)pl * b.spitch : nullptr;
+    double* s2 = HAS2 ? b.s2 + (long long)pl * b.spitch : nullptr;
+    if (!SORT_ONLY && tid == 0) { s1[0] = 0.0; if (HAS0) s0[0] = 0.0; if (HAS2) s2[0] = 0.0; }
+    double carry1 = 0.0, carry0 = 0.0, carry2 = 0.0;           // sums of the buckets before the current one
 
-    // 1. load the bucket, clear the sub-bucket histogram
-    for (int i = tid; i < m; i += kFinThreads) A[i] = keys[i];
-    for (int k = tid; k < kSub; k += kFinThreads) H[k] = 0;
-    __syncthreads();
-    // 2. histogram of the next 10 key bits
-    for (int i = tid; i < m; i += kFinThreads) atomicAdd(&H[((u32)(A[i] >> 32) >> subshift) & (kSub - 1)], 1u);
-    __syncthreads();
-    // 3. exclusive scan of the kSub counts (4 per thread)
-    {
-        constexpr int PER = kSub / kFinThreads;
-        u32 c[PER], sum = 0;
+    // keys of the first bucket
+    u64 nk[kFinItems];
+    int bs = (int)start[0], be = (int)start[1];
 #pragma unroll
-        for (int e = 0; e < PER; ++e) { c[e] = H[tid * PER + e]; sum += c[e]; }
-        u32 x = sum;
+    for (int e = 0; e < kFinItems; ++e) {
+        const int i = e * kFinThreads + tid;
+        nk[e] = bs + i < be ? keys[bs + i] : 0ull;
+    }
+    for (int bk = 0; bk < b.nbk; ++bk) {
+        const int m = be - bs;
+        // 1. the prefetched keys go to shared memory; the next bucket's keys are requested
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { const u32 y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
-        if (lane == 31) s_wsum[warp] = x;
+        for (int e = 0; e < kFinItems; ++e) {
+            const int i = e * kFinThreads + tid;
+            if (i < m) A[i] = nk[e];
+        }
+        for (int k = tid; k < kSub; k += kFinThreads) H[k] = 0;
+        const int nbs = be, nbe = bk + 1 < b.nbk ? (int)start[bk + 2] : be;
+#pragma unroll
+        for (int e = 0; e < kFinItems; ++e) {
+            const int i = e * kFinThreads + tid;
+            nk[e] = nbs + i < nbe ? keys[nbs + i] : 0ull;
+        }
         __syncthreads();
-        u32 wbase = 0;
+        // 2. histogram of the next 10 key bits
+        for (int i = tid; i < m; i += kFinThreads) atomicAdd(&H[((u32)(A[i] >> 32) >> subshift) & (kSub - 1)], 1u);
+        __syncthreads();
+        // 3. exclusive scan of the kSub counts (4 per thread)
+        {
+            constexpr int PER = kSub / kFinThreads;
+            u32 c[PER], sum = 0;
 #pragma unroll
-        for (int k = 0; k < NW; ++k) wbase += k < warp ? s_wsum[k] : 0u;
-        u32 base = wbase + x - sum;
+            for (int e = 0; e < PER; ++e) { c[e] = H[tid * PER + e]; sum += c[e]; }
+            u32 x = sum;
 #pragma unroll
-        for (int e = 0; e < PER; ++e) { H[tid * PER + e] = base; base += c[e]; }
-    }
-    __syncthreads();
-    // 4. counting-sort scatter (order inside a sub-bucket is arbitrary)
-    for (int i = tid; i < m; i += kFinThreads) {
-        const u64 k = A[i];
-        B[atomicAdd(&H[((u32)(k >> 32) >> subshift) & (kSub - 1)], 1u)] = k;
-    }
-    __syncthreads();
-    // 5. exact rank inside every run of equal 10-bit codes
-    for (int i = tid; i < m; i += kFinThreads) {
-        const u64 k = B[i];
-        const u32 sb = ((u32)(k >> 32) >> subshift) & (kSub - 1);
-        const int rs = sb ? (int)H[sb - 1] : 0, re = (int)H[sb];     // H[sb] is now the end of sub-bucket sb
-        int r = i;
-        if (re - rs > 1) {
-            r = rs;
-            for (int j = rs; j < re; ++j) r += (j != i && key_less(B[j], k, b.t, period)) ? 1 : 0;
+            for (int o = 1; o < 32; o <<= 1) { const u32 y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+            if (lane == 31) s_wsum[warp] = x;
+            __syncthreads();
+            u32 wbase = 0;
+#pragma unroll
+            for (int k = 0; k < NW; ++k) wbase += k < warp ? s_wsum[k] : 0u;
+            u32 base = wbase + x - sum;
+#pragma unroll
+            for (int e = 0; e < PER; ++e) { H[tid * PER + e] = base; base += c[e]; }
         }
-        A[r] = k;
-    }
-    __syncthreads();
-    // 6. the bucket is sorted: permutation (written below, while warp 0 looks back)
-    u32* perm = b.perm + (long long)pl * b.n + bs;
-    if (SORT_ONLY) {
-        for (int i = tid; i < m; i += kFinThreads) perm[i] = (u32)A[i];
-        return;
-    }
-
-    // 7. gather + local inclusive scan: thread owns kFinItems consecutive sorted entries
-    double v1[kFinItems], v0[kFinItems], v2[kFinItems];
-    const int first = tid * kFinItems;
-#pragma unroll
-    for (int e = 0; e < kFinItems; ++e) {
-        v1[e] = 0.0; v0[e] = 0.0; v2[e] = 0.0;
-        if (first + e < m) {
-            const u32 idx = (u32)A[first + e];
-            v1[e] = b.wr[idx];
-            if (HAS0) v0[e] = b.w[idx];
-            if (HAS2) v2[e] = b.wr2[idx];
+        __syncthreads();
+        // 4. counting-sort scatter (order inside a sub-bucket is arbitrary)
+        for (int i = tid; i < m; i += kFinThreads) {
+            const u64 k = A[i];
+            B[atomicAdd(&H[((u32)(k >> 32) >> subshift) & (kSub - 1)], 1u)] = k;
         }
-    }
-    double* x1 = b.x1 + (long long)pl * b.pitch + bs;
-    double* x0 = HAS0 ? b.x0 + (long long)pl * b.pitch + bs : nullptr;
-    double* x2 = HAS2 ? b.x2 + (long long)pl * b.pitch + bs : nullptr;
-    double r1[kFinItems], r0[kFinItems], r2[kFinItems];          // the gathered values themselves
-#pragma unroll
-    for (int e = 0; e < kFinItems; ++e) { r1[e] = v1[e]; r0[e] = v0[e]; r2[e] = v2[e]; }
-#pragma unroll
-    for (int e = 1; e < kFinItems; ++e) {
-        v1[e] += v1[e - 1];
-        if (HAS0) v0[e] += v0[e - 1];
-        if (HAS2) v2[e] += v2[e - 1];
-    }
-    double t1 = v1[kFinItems - 1], t0 = v0[kFinItems - 1], t2 = v2[kFinItems - 1];
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const double u1 = __shfl_up_sync(0xffffffffu, t1, o);
-        const double u0 = HAS0 ? __shfl_up_sync(0xffffffffu, t0, o) : 0.0;
-        const double u2 = HAS2 ? __shfl_up_sync(0xffffffffu, t2, o) : 0.0;
-        if (lane >= o) { t1 += u1; t0 += u0; t2 += u2; }
-    }
-    if (lane == 31) { s_w[0][warp] = t1; s_w[1][warp] = t0; s_w[2][warp] = t2; }
-    __syncthreads();
-    // 8. publish this bucket's sums (k_prefix_fix adds the sums of the earlier buckets afterwards: a
-    //    look-back inside this kernel made every CTA wait for the slowest of its period's earlier CTAs)
-    if (tid == 0) {
-        double tot1 = 0.0, tot0 = 0.0, tot2 = 0.0;
-#pragma unroll
-        for (int k = 0; k < NW; ++k) { tot1 += s_w[0][k]; tot0 += s_w[1][k]; tot2 += s_w[2][k]; }
-        double* agg = b.prefix + ((long long)pl * b.nbk + bk) * 3;
-        agg[0] = tot1; agg[1] = tot0; agg[2] = tot2;
-        s_base[0] = 0.0; s_base[1] = 0.0; s_base[2] = 0.0;
-    }
-    for (int i = tid; i < m; i += kFinThreads) perm[i] = (u32)A[i];
-#pragma unroll
-    for (int e = 0; e < kFinItems; ++e) {
-        if (first + e < m) {
-            x1[first + e] = r1[e];
-            if (HAS0) x0[first + e] = r0[e];
-            if (HAS2) x2[first + e] = r2[e];
+        __syncthreads();
+        // 5. exact rank inside every run of equal 10-bit codes
+        for (int i = tid; i < m; i += kFinThreads) {
+            const u64 k = B[i];
+            const u32 sb = ((u32)(k >> 32) >> subshift) & (kSub - 1);
+            const int rs = sb ? (int)H[sb - 1] : 0, re = (int)H[sb];     // H[sb] is now the end of sub-bucket sb
+            int r = i;
+            if (re - rs > 1) {
+                // (key32, index) orders the run unless two of its 32-bit keys are equal: then (rare) the
+                // fp64 phases decide
+                r = rs;
+                bool tie = false;
+                for (int j = rs; j < re; ++j) {
+                    const u64 o = B[j];
+                    r += o < k ? 1 : 0;
+                    tie |= j != i && (u32)(o >> 32) == (u32)(k >> 32);
+                }
+                if (tie) {
+                    r = rs;
+                    for (int j = rs; j < re; ++j) r += (j != i && key_less(B[j], k, b.t, period)) ? 1 : 0;
+                }
+            }
+            A[r] = k;
         }
-    }
-    __syncthreads();
-    double w1 = s_base[0], w0 = s_base[1], w2 = s_base[2];     // + totals of the warps before mine
+        __syncthreads();
+        // 6. the bucket is sorted: permutation
+        for (int i = tid; i < m; i += kFinThreads) perm[bs + i] = (u32)A[i];
+        if (!SORT_ONLY) {
+            // 7. gather + inclusive scan: thread owns kFinItems consecutive sorted entries
+            double v1[kFinItems], v0[kFinItems], v2[kFinItems];
+            const int first = tid * kFinItems;
 #pragma unroll
-    for (int k = 0; k < NW; ++k) {
-        if (k < warp) { w1 += s_w[0][k]; w0 += s_w[1][k]; w2 += s_w[2][k]; }
-    }
-    const double o1 = w1 + (t1 - v1[kFinItems - 1]);
-    const double o0 = w0 + (t0 - v0[kFinItems - 1]);
-    const double o2 = w2 + (t2 - v2[kFinItems - 1]);
-    double* s1 = b.s1 + (long long)pl * b.spitch + bs;
-    double* s0 = HAS0 ? b.s0 + (long long)pl * b.spitch + bs : nullptr;
-    double* s2 = HAS2 ? b.s2 + (long long)pl * b.spitch + bs : nullptr;
-    if (bk == 0 && tid == 0) { s1[0] = 0.0; if (HAS0) s0[0] = 0.0; if (HAS2) s2[0] = 0.0; }
+            for (int e = 0; e < kFinItems; ++e) {
+                v1[e] = 0.0; v0[e] = 0.0; v2[e] = 0.0;
+                if (first + e < m) {
+                    const u32 idx = (u32)A[first + e];
+                    v1[e] = b.wr[idx];
+                    if (HAS0) v0[e] = b.w[idx];
+                    if (HAS2) v2[e] = b.wr2[idx];
+                }
+            }
 #pragma unroll
-    for (int e = 0; e < kFinItems; ++e) {
-        if (first + e < m) {
-            s1[first + e + 1] = o1 + v1[e];
-            if (HAS0) s0[first + e + 1] = o0 + v0[e];
-            if (HAS2) s2[first + e + 1] = o2 + v2[e];
-        }
-    }
-}
-
-// Adds to the bucket-local prefix sums the sums of the earlier buckets of the period, taken in a fixed
-// order (strided per lane, then a shuffle tree): deterministic.  One CTA per (period, bucket).
-template <bool HAS0, bool HAS2>
-__global__ void __launch_bounds__(256) k_prefix_fix(BucketArgs b) {
-    __shared__ double s_base[3];
-    const int bk = blockIdx.x, pl = blockIdx.y;
-    if (bk == 0 || b.fb_flag[pl]) return;
-    const int lane = threadIdx.x & 31;
-    if (threadIdx.x < 32) {
-        const double* agg = b.prefix + (long long)pl * b.nbk * 3;
-        double a1 = 0.0, a0 = 0.0, a2 = 0.0;
-        for (int j = lane; j < bk; j += 32) {
-            a1 += agg[j * 3];
-            if (HAS0) a0 += agg[j * 3 + 1];
-            if (HAS2) a2 += agg[j * 3 + 2];
-        }
+            for (int e = 0; e < kFinItems; ++e) {
+                if (first + e < m) {
+                    x1[bs + first + e] = v1[e];
+                    if (HAS0) x0[bs + first + e] = v0[e];
+                    if (HAS2) x2[bs + first + e] = v2[e];
+                }
+            }
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            a1 += __shfl_xor_sync(0xffffffffu, a1, o);
-            a0 += __shfl_xor_sync(0xffffffffu, a0, o);
-            a2 += __shfl_xor_sync(0xffffffffu, a2, o);
+            for (int e = 1; e < kFinItems; ++e) {
+                v1[e] += v1[e - 1];
+                if (HAS0) v0[e] += v0[e - 1];
+                if (HAS2) v2[e] += v2[e - 1];
+            }
+            double t1 = v1[kFinItems - 1], t0 = v0[kFinItems - 1], t2 = v2[kFinItems - 1];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const double u1 = __shfl_up_sync(0xffffffffu, t1, o);
+                const double u0 = HAS0 ? __shfl_up_sync(0xffffffffu, t0, o) : 0.0;
+                const double u2 = HAS2 ? __shfl_up_sync(0xffffffffu, t2, o) : 0.0;
+                if (lane >= o) { t1 += u1; t0 += u0; t2 += u2; }
+            }
+            if (lane == 31) { s_w[0][warp] = t1; s_w[1][warp] = t0; s_w[2][warp] = t2; }
+            __syncthreads();
+            // carry + totals of the warps before mine (every thread adds in the same fixed order)
+            double w1 = carry1, w0 = carry0, w2 = carry2, a1 = carry1, a0 = carry0, a2 = carry2;
+#pragma unroll
+            for (int k = 0; k < NW; ++k) {
+                if (k < warp) { w1 += s_w[0][k]; w0 += s_w[1][k]; w2 += s_w[2][k]; }
+                a1 += s_w[0][k]; a0 += s_w[1][k]; a2 += s_w[2][k];
+            }
+            const double o1 = w1 + (t1 - v1[kFinItems - 1]);
+            const double o0 = w0 + (t0 - v0[kFinItems - 1]);
+            const double o2 = w2 + (t2 - v2[kFinItems - 1]);
+#pragma unroll
+            for (int e = 0; e < kFinItems; ++e) {
+                if (first + e < m) {
+                    s1[bs + first + e + 1] = o1 + v1[e];
+                    if (HAS0) s0[bs + first + e + 1] = o0 + v0[e];
+                    if (HAS2) s2[bs + first + e + 1] = o2 + v2[e];
+                }
+            }
+            carry1 = a1; carry0 = a0; carry2 = a2;
         }
-        if (lane == 0) { s_base[0] = a1; s_base[1] = a0; s_base[2] = a2; }
-    }
-    __syncthreads();
-    const u32* start = b.start + (long long)pl * (b.nbk + 1);
-    const int bs = (int)start[bk], m = (int)start[bk + 1] - bs;
-    double* s1 = b.s1 + (long long)pl * b.spitch + bs + 1;
-    double* s0 = HAS0 ? b.s0 + (long long)pl * b.spitch + bs + 1 : nullptr;
-    double* s2 = HAS2 ? b.s2 + (long long)pl * b.spitch + bs + 1 : nullptr;
-    const double b1 = s_base[0], b0 = s_base[1], b2 = s_base[2];
-    for (int i = threadIdx.x; i < m; i += blockDim.x) {
-        s1[i] = b1 + s1[i];
-        if (HAS0) s0[i] = b0 + s0[i];
-        if (HAS2) s2[i] = b2 + s2[i];
+        bs = nbs; be = nbe;
+        __syncthreads();                                           // A, H, s_w are reused by the next bucket
     }
 }
 
@@ -384,26 +380,39 @@ int bucket_count_for(int n) {
     return nbk;
 }
 
-void launch_bucket_sort(const BucketArgs& b, bool has0, bool has2, bool sort_only, cudaStream_t st) {
+constexpr size_t kFinSmem = 2 * (size_t)kBucketCap * sizeof(u64) + (kSub + 1) * sizeof(u32);
+
+static dim3 count_grid(const BucketArgs& b) {
+    return dim3((b.n + kCountThreads * kCountItems - 1) / (kCountThreads * kCountItems), b.tile);
+}
+
+void launch_bucket_sort_head(const BucketArgs& b, cudaStream_t st) {
     cudaMemsetAsync(b.hist, 0, (size_t)b.tile * b.nbk * sizeof(u32), st);
     cudaMemsetAsync(b.fb_count, 0, sizeof(int), st);
-    const dim3 grid((b.n + kCountThreads * kCountItems - 1) / (kCountThreads * kCountItems), b.tile);
-    k_bucket_count<<<grid, kCountThreads, 0, st>>>(b);
+    k_bucket_count<<<count_grid(b), kCountThreads, 0, st>>>(b);
     k_bucket_scan<<<(b.tile * 32 + 255) / 256, 256, 0, st>>>(b);
-    k_bucket_scatter<<<grid, kCountThreads, 0, st>>>(b);
-    const dim3 fgrid(b.nbk, b.tile);
-    if (sort_only) { k_bucket_finish<false, false, true><<<fgrid, kFinThreads, 0, st>>>(b); return; }
+}
+
+void launch_bucket_sort_tail(const BucketArgs& b, bool has0, bool has2, bool sort_only, cudaStream_t st) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(k_bucket_finish<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFinSmem);
+        cudaFuncSetAttribute(k_bucket_finish<true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFinSmem);
+        cudaFuncSetAttribute(k_bucket_finish<true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFinSmem);
+        cudaFuncSetAttribute(k_bucket_finish<false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFinSmem);
+        attr_set = true;
+    }
+    k_bucket_scatter<<<count_grid(b), kCountThreads, 0, st>>>(b);
+    const dim3 fgrid(b.tile);
+    if (sort_only) { k_bucket_finish<false, false, true><<<fgrid, kFinThreads, kFinSmem, st>>>(b); return; }
     if (has2) {
-        k_bucket_finish<true, true, false><<<fgrid, kFinThreads, 0, st>>>(b);
-        k_prefix_fix<true, true><<<fgrid, 256, 0, st>>>(b);
+        k_bucket_finish<true, true, false><<<fgrid, kFinThreads, kFinSmem, st>>>(b);
         k_pad_scan<true, true><<<b.tile, kPadThreads, 0, st>>>(b);
     } else if (has0) {
-        k_bucket_finish<true, false, false><<<fgrid, kFinThreads, 0, st>>>(b);
-        k_prefix_fix<true, false><<<fgrid, 256, 0, st>>>(b);
+        k_bucket_finish<true, false, false><<<fgrid, kFinThreads, kFinSmem, st>>>(b);
         k_pad_scan<true, false><<<b.tile, kPadThreads, 0, st>>>(b);
     } else {
-        k_bucket_finish<false, false, false><<<fgrid, kFinThreads, 0, st>>>(b);
-        k_prefix_fix<false, false><<<fgrid, 256, 0, st>>>(b);
+        k_bucket_finish<false, false, false><<<fgrid, kFinThreads, kFinSmem, st>>>(b);
         k_pad_scan<false, false><<<b.tile, kPadThreads, 0, st>>>(b);
     }
 }

@@ -614,33 +614,14 @@ static void launch_variant(const TileArgs& a, int v, cudaStream_t st) {
 // The variants other than the dominant one (21-ring, wide) often hold few, long trials: alone on the
 // device they leave most warp slots empty.  They are launched on a side stream of higher priority between
 // two events, so their CTAs take slots first and the dominant kernel fills the rest of the device.
-struct SideStream {
-    cudaStream_t s = nullptr;
-    cudaEvent_t fork = nullptr, join = nullptr;
-    bool ok = false;
-    int dev = -1;
-    SideStream() {
-        int lo = 0, hi = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess) return;
-        if (cudaDeviceGetStreamPriorityRange(&lo, &hi) != cudaSuccess) return;
-        if (cudaStreamCreateWithPriority(&s, cudaStreamNonBlocking, hi) != cudaSuccess) return;
-        if (cudaEventCreateWithFlags(&fork, cudaEventDisableTiming) != cudaSuccess) return;
-        if (cudaEventCreateWithFlags(&join, cudaEventDisableTiming) != cudaSuccess) return;
-        ok = true;
-    }
-};
-
 void launch_chi2_ring(const TileArgs& a, cudaStream_t st) {
     launch_bin_trials(a, st);
-    static thread_local SideStream side;        // per host thread; bound to the device of its first call
-    int dev = -1;
-    cudaGetDevice(&dev);
-    static const bool overlap = !(getenv("GTLS_CHI2_STREAMS") && atoi(getenv("GTLS_CHI2_STREAMS")) == 0);
     cudaStream_t ss = st;
-    if (overlap && side.ok && dev == side.dev) {
-        cudaEventRecord(side.fork, st);
-        cudaStreamWaitEvent(side.s, side.fork, 0);
-        ss = side.s;
+    SideStream* side = side_stream(0);
+    if (side) {
+        cudaEventRecord(side->fork, st);
+        cudaStreamWaitEvent(side->s, side->fork, 0);
+        ss = side->s;
     }
     if (a.uniform) {
         launch_variant<12, true, true>(a, 9, ss);
@@ -663,9 +644,9 @@ void launch_chi2_ring(const TileArgs& a, cudaStream_t st) {
         launch_variant<4, false, false>(a, 5, ss);
         launch_variant<21, false, false>(a, 1, st);
     }
-    if (ss != st) {
-        cudaEventRecord(side.join, ss);
-        cudaStreamWaitEvent(st, side.join, 0);
+    if (side) {
+        cudaEventRecord(side->join, ss);
+        cudaStreamWaitEvent(st, side->join, 0);
     }
 }
 

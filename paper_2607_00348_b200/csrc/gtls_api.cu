@@ -71,9 +71,17 @@ Sizes workspace_sizes(long long n, long long n_per, int n_dur, double q_max, boo
     return s;
 }
 
+#ifndef GTLS_FIN_SLOTS
+#define GTLS_FIN_SLOTS (148 * 4)
+#endif
+constexpr long long kFinishSlots = GTLS_FIN_SLOTS;
+
 int auto_tile(long long n_per, const Sizes& s, size_t budget) {
     long long t = (long long)(budget / s.per_period);
     if (t > 8192) t = 8192;
+    // k_bucket_finish runs one CTA per period, kFinishSlots of them at a time (148 SMs x 5 CTAs): a tile
+    // that is a multiple of that leaves no partly filled last round
+    if (t >= kFinishSlots && t < n_per) t -= t % kFinishSlots;
     if (t > n_per) t = n_per;
     if (t < 1) t = 1;
     return (int)t;
@@ -151,6 +159,34 @@ bool force_lsd_sort() {
     return f;
 }
 
+}  // namespace
+
+SideStream* gtls::side_stream(int which) {
+    struct Slot {
+        SideStream ss{};
+        bool ok = false;
+        int dev = -1;
+        Slot() {
+            int lo = 0, hi = 0;
+            if (cudaGetDevice(&dev) != cudaSuccess) return;
+            if (cudaDeviceGetStreamPriorityRange(&lo, &hi) != cudaSuccess) return;
+            if (cudaStreamCreateWithPriority(&ss.s, cudaStreamNonBlocking, hi) != cudaSuccess) return;
+            if (cudaEventCreateWithFlags(&ss.fork, cudaEventDisableTiming) != cudaSuccess) return;
+            if (cudaEventCreateWithFlags(&ss.join, cudaEventDisableTiming) != cudaSuccess) return;
+            ok = true;
+        }
+    };
+    static const bool enabled = [] { const char* e = getenv("GTLS_STREAMS"); return !(e && atoi(e) == 0); }();
+    if (!enabled || which < 0 || which > 1) return nullptr;
+    static thread_local Slot slots[2];
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return nullptr;
+    Slot& sl = slots[which];
+    return (sl.ok && sl.dev == dev) ? &sl.ss : nullptr;
+}
+
+namespace {
+
 // Steps a1-a4 for the tile described by `a` (a.perm, a.x1/s1[/x0/s0] are outputs).
 //   The bucket fast path first; a period with a bucket larger than kBucketCap (clustered phases) is put
 //   on the tile's fallback list on the device and skipped by the fast path; the LSD radix path
@@ -176,18 +212,41 @@ void run_fold_sort_scan(TileArgs& a, const SortScratch& sc, double* x2, double* 
         b.keys = a.keys_b; b.perm = a.perm;
         b.x1 = a.x1; b.s1 = a.s1; b.x0 = a.x0; b.s0 = a.s0; b.x2 = x2; b.s2 = s2;
         const bool has2 = s2 != nullptr, has0 = !a.uniform || has2;
-        launch_bucket_sort(b, has0, has2, sort_only, st);
-        nl += sort_only ? 4 : 6;
-        if (phase_out) { launch_fold_keys(a, phase_out, st); ++nl; }   // phases: the LSD path's fold kernel
+        launch_bucket_sort_head(b, st);
+        // the fallback list is known: the LSD path over it (a handful of CTAs, a few hundred microseconds
+        // of latency when a period is on the list) runs beside the fast path on a side stream
+        cudaStream_t ls = st;
+        SideStream* side = side_stream(1);
+        if (side) {
+            cudaEventRecord(side->fork, st);
+            cudaStreamWaitEvent(side->s, side->fork, 0);
+            ls = side->s;
+        }
+        launch_bucket_sort_tail(b, has0, has2, sort_only, st);
+        nl += sort_only ? 4 : 5;
         a.seg_list = sc.fb_list; a.seg_count = sc.fb_count;
-        phase_out = nullptr;
+        launch_fold_keys(a, nullptr, ls);
+        int l2 = 0;
+        const u64* sorted = launch_phase_sort(a, ls, &l2);
+        if (!sort_only) launch_gather_scan(a, sorted, x2, s2, pad_override, ls);
+        launch_perm_export(a, sorted, (int32_t*)a.perm, ls);
+        if (side) {
+            cudaEventRecord(side->join, ls);
+            cudaStreamWaitEvent(st, side->join, 0);
+        }
+        if (phase_out) {                          // phases of every period: the LSD path's fold kernel, dense
+            a.seg_list = nullptr; a.seg_count = nullptr;
+            launch_fold_keys(a, phase_out, st); ++nl;
+        }
+        a.seg_list = nullptr; a.seg_count = nullptr;
+        if (launches) *launches += nl + 1 + l2 + (sort_only ? 0 : 1) + 1;
+        return;
     }
     launch_fold_keys(a, phase_out, st);
     int l2 = 0;
     const u64* sorted = launch_phase_sort(a, st, &l2);
     if (!sort_only) launch_gather_scan(a, sorted, x2, s2, pad_override, st);
     launch_perm_export(a, sorted, (int32_t*)a.perm, st);
-    a.seg_list = nullptr; a.seg_count = nullptr;
     if (launches) *launches += nl + 1 + l2 + (sort_only ? 0 : 1) + 1;
 }
 

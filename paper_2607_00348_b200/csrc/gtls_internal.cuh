@@ -56,8 +56,12 @@ __host__ __device__ __forceinline__ int chi2_ring_index(int taps) {
 
 // bucket sort (bucket_sort.cu)
 constexpr int kMaxBuckets = 256;      // buckets per period (power of two)
-constexpr int kBucketTarget = 1100;   // aimed-at mean bucket size
-constexpr int kBucketCap = 1536;      // largest bucket the shared-memory sort takes; beyond: LSD fallback
+#ifndef GTLS_BUCKET_TARGET
+#define GTLS_BUCKET_TARGET 1100
+#define GTLS_BUCKET_CAP 1536
+#endif
+constexpr int kBucketTarget = GTLS_BUCKET_TARGET;   // aimed-at mean bucket size
+constexpr int kBucketCap = GTLS_BUCKET_CAP;      // largest bucket the shared-memory sort takes; beyond: LSD fallback
 
 constexpr int kRadixThreads = 256;
 constexpr int kRadixItems = 8;
@@ -167,7 +171,16 @@ struct BucketArgs {
     double* x1; double* s1; double* x0; double* s0; double* x2; double* s2;
 };
 int bucket_count_for(int n);
-void launch_bucket_sort(const BucketArgs& b, bool has0, bool has2, bool sort_only, cudaStream_t st);
+// count + bucket starts + fallback list; then (after the caller forked the fallback path) scatter + finish + pad
+void launch_bucket_sort_head(const BucketArgs& b, cudaStream_t st);
+void launch_bucket_sort_tail(const BucketArgs& b, bool has0, bool has2, bool sort_only, cudaStream_t st);
+
+// A high-priority side stream with a fork and a join event, per host thread, bound to the device of the
+// thread's first call.  which: 0 = chi2 variants, 1 = LSD fallback of the sort.  nullptr when streams
+// are switched off (GTLS_STREAMS=0), creation failed, or the current device is another one: the caller then
+// launches everything on its own stream.
+struct SideStream { cudaStream_t s; cudaEvent_t fork, join; };
+SideStream* side_stream(int which);
 
 void launch_curve_pre(const double* t, const double* y, const double* dy, int n, double* wr,
                       double* w, double* wr2, CurveInfo* info, cudaStream_t st);
