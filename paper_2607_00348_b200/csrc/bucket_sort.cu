@@ -175,12 +175,11 @@ __global__ void __launch_bounds__(kFinThreads, kFinCtas) k_bucket_finish(BucketA
     }
     for (int bk = 0; bk < b.nbk; ++bk) {
         const int m = be - bs;
-        // 1. the prefetched keys go to shared memory; the next bucket's keys are requested
+        // 1. the prefetched keys stay in registers (thread owns entries e*kFinThreads + tid); the next
+        //    bucket's keys are requested
+        u64 kc[kFinItems];
 #pragma unroll
-        for (int e = 0; e < kFinItems; ++e) {
-            const int i = e * kFinThreads + tid;
-            if (i < m) A[i] = nk[e];
-        }
+        for (int e = 0; e < kFinItems; ++e) kc[e] = nk[e];
         for (int k = tid; k < kSub; k += kFinThreads) H[k] = 0;
         const int nbs = be, nbe = bk + 1 < b.nbk ? (int)start[bk + 2] : be;
 #pragma unroll
@@ -190,7 +189,9 @@ __global__ void __launch_bounds__(kFinThreads, kFinCtas) k_bucket_finish(BucketA
         }
         __syncthreads();
         // 2. histogram of the next 10 key bits
-        for (int i = tid; i < m; i += kFinThreads) atomicAdd(&H[((u32)(A[i] >> 32) >> subshift) & (kSub - 1)], 1u);
+#pragma unroll
+        for (int e = 0; e < kFinItems; ++e)
+            if (e * kFinThreads + tid < m) atomicAdd(&H[((u32)(kc[e] >> 32) >> subshift) & (kSub - 1)], 1u);
         __syncthreads();
         // 3. exclusive scan of the kSub counts (4 per thread)
         {
@@ -212,9 +213,15 @@ __global__ void __launch_bounds__(kFinThreads, kFinCtas) k_bucket_finish(BucketA
         }
         __syncthreads();
         // 4. counting-sort scatter (order inside a sub-bucket is arbitrary)
-        for (int i = tid; i < m; i += kFinThreads) {
-            const u64 k = A[i];
-            B[atomicAdd(&H[((u32)(k >> 32) >> subshift) & (kSub - 1)], 1u)] = k;
+        {
+            u32 pos[kFinItems];
+#pragma unroll
+            for (int e = 0; e < kFinItems; ++e)
+                pos[e] = e * kFinThreads + tid < m
+                             ? atomicAdd(&H[((u32)(kc[e] >> 32) >> subshift) & (kSub - 1)], 1u) : 0u;
+#pragma unroll
+            for (int e = 0; e < kFinItems; ++e)
+                if (e * kFinThreads + tid < m) B[pos[e]] = kc[e];
         }
         __syncthreads();
         // 5. exact rank inside every run of equal 10-bit codes

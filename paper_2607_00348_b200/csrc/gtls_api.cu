@@ -140,7 +140,7 @@ struct CurveDev {
 };
 
 
-struct SortScratch { u32* hist; u32* start; u32* cursor; int* fb_flag; int* fb_list; int* fb_count; double* prefix; int* flag; };
+struct SortScratch { u32* hist; u32* start; u32* cursor; int* fb_flag; int* fb_list; int* fb_count; };
 
 bool take_sort_scratch(Arena& ar, size_t tile, int nbk, SortScratch& sc) {
     sc.hist = ar.take<u32>(tile * nbk);
@@ -149,9 +149,7 @@ bool take_sort_scratch(Arena& ar, size_t tile, int nbk, SortScratch& sc) {
     sc.fb_flag = ar.take<int>(tile);
     sc.fb_list = ar.take<int>(tile);
     sc.fb_count = ar.take<int>(1);
-    sc.prefix = ar.take<double>(tile * nbk * 3);
-    sc.flag = ar.take<int>(tile * nbk);
-    return sc.flag != nullptr;
+    return sc.fb_count != nullptr;
 }
 
 bool force_lsd_sort() {
@@ -208,7 +206,6 @@ void run_fold_sort_scan(TileArgs& a, const SortScratch& sc, double* x2, double* 
         b.t = a.t; b.wr = a.wr; b.w = a.w; b.wr2 = a.wr2; b.periods = a.periods; b.durtab = a.durtab;
         b.hist = sc.hist; b.start = sc.start; b.cursor = sc.cursor;
         b.fb_flag = sc.fb_flag; b.fb_list = sc.fb_list; b.fb_count = sc.fb_count;
-        b.prefix = sc.prefix; b.flag = sc.flag;
         b.keys = a.keys_b; b.perm = a.perm;
         b.x1 = a.x1; b.s1 = a.s1; b.x0 = a.x0; b.s0 = a.s0; b.x2 = x2; b.s2 = s2;
         const bool has2 = s2 != nullptr, has0 = !a.uniform || has2;

@@ -164,8 +164,6 @@ struct BucketArgs {
     int* fb_flag;              // [tile] 1: a bucket of this period exceeded kBucketCap (LSD path takes it)
     int* fb_list;              // [tile] those periods, any order
     int* fb_count;             // [1]
-    double* prefix;            // [tile*nbk*3] inclusive prefix of (w r, w, w r^2) per bucket (look-back)
-    int* flag;                 // [tile*nbk]   prefix published
     u64* keys;                 // [tile*n] bucketed keys
     u32* perm;                 // [tile*n]
     double* x1; double* s1; double* x0; double* s0; double* x2; double* s2;
