@@ -63,7 +63,8 @@ Sizes workspace_sizes(long long n, long long n_per, int n_dur, double q_max, boo
     const int nt = (int)((n + kRadixTile - 1) / kRadixTile);
     s.fixed = 3 * align_up(n * sizeof(double)) + align_up(sizeof(CurveInfo)) +
               align_up(sizeof(SdeScratch)) + align_up(2 * sizeof(unsigned long long)) +
-              2 * align_up(n_per * sizeof(double)) + align_up(n_per * sizeof(gtls_best)) + 4096;
+              2 * align_up(n_per * sizeof(double)) + align_up(n_per * sizeof(gtls_best)) + 4096 +
+              align_up(2 * (size_t)(pitch - n + 2) * sizeof(double));       // gtab: D <= pitch - n
     s.per_period = 2 * n * sizeof(u64) + 256ull * nt * sizeof(u32) + n_dur * sizeof(DurEntry) +
                    n_dur * sizeof(Partial) + (size_t)kChi2Variants * n_dur * sizeof(int) +
                    n * sizeof(u32) + (4ull * kMaxBuckets + 3) * sizeof(u32) + 3ull * kMaxBuckets * sizeof(double) +
@@ -377,6 +378,18 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     if (o.stats) { CU(cudaStreamSynchronize(st)); stats.ms_pre += tm.ms(0, 1); }
     const bool uniform = info.w_min == info.w_max;
 
+    const double* gtab_dev = nullptr;
+    int gtab_max = 0;
+    {   // template sums per D, once per search (every D the grid can ask for: D <= floor(q_max * n) <= pitch - n)
+        long long dmax = (long long)(info.q_max * (double)n);
+        dmax = dmax < 1 ? 1 : (dmax > n - 1 ? n - 1 : dmax);
+        double* gtab = ws.take<double>(2 * (size_t)(dmax + 1));
+        if (!gtab) return GTLS_ENOMEM;
+        launch_gtab(d_tmpl, n_tmpl, (int)dmax, gtab, st);
+        stats.kernel_launches += 1;
+        gtab_dev = gtab; gtab_max = (int)dmax;
+    }
+
     // ---- tile geometry -------------------------------------------------------------------
     const Sizes sz = workspace_sizes(n, n_per, n_dur, info.q_max, uniform);
     const size_t avail = ws.size - align_up(ws.off) - 32 * 256;
@@ -400,6 +413,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     SortScratch ssc;
     if (!take_sort_scratch(ws, (size_t)tile, bucket_count_for((int)n), ssc)) return GTLS_ENOMEM;
     a.durtab = ws.take<DurEntry>((size_t)tile * n_dur);
+    a.gtab = gtab_dev; a.gtab_max = gtab_max;
     a.partial = ws.take<Partial>((size_t)tile * n_dur);
     a.trial_list = ws.take<int>((size_t)kChi2Variants * tile * n_dur);
     a.trial_count = ws.take<int>(kChi2Variants);

@@ -146,6 +146,8 @@ struct TileArgs {
     const int* seg_count;  // number of entries of seg_list (device)
     int* trial_list;       // [kChi2Variants][tile*n_dur] trial indices binned by chi2 kernel variant
     int* trial_count;      // [kChi2Variants]
+    const double* gtab;    // [2*(gtab_max+1)] sum g_D, sum g_D^2 for D = 1 .. gtab_max (k_gtab)
+    int gtab_max;
     int dbg_min_st, dbg_max_st;   // timing experiments only (GTLS_DBG_MIN_ST / GTLS_DBG_MAX_ST): skip other trials
 };
 
@@ -184,6 +186,7 @@ void launch_curve_pre(const double* t, const double* y, const double* dy, int n,
                       double* w, double* wr2, CurveInfo* info, cudaStream_t st);
 void launch_grid_check(const double* periods, long long n_per, const double* durs,
                        long long n_durs_total, CurveInfo* info, cudaStream_t st);
+void launch_gtab(const double* tmpl, int n_tmpl, int gtab_max, double* gtab, cudaStream_t st);
 void launch_durtab(const TileArgs& a, cudaStream_t st);
 // bins the tile's trials by chi2 kernel variant (order preserved); skipped trials get an invalid Partial
 void launch_bin_trials(const TileArgs& a, cudaStream_t st);

@@ -96,30 +96,49 @@ __global__ void __launch_bounds__(256) k_grid_check(const double* __restrict__ p
     }
 }
 
-// One warp per (period, duration): D, stride, mean(g_D), sum g_D^2, duplicate-D flag.
-__global__ void __launch_bounds__(256) k_durtab(TileArgs a) {
-    const int warp_global = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+// sum g_D and sum g_D^2 depend on D alone: one warp per D = 1 .. gtab_max, once per search
+// (lane-strided sums + shuffle tree: the order every later use relies on).
+__global__ void __launch_bounds__(256) k_gtab(const double* __restrict__ tmpl, int n_tmpl, int gtab_max,
+                                              double* __restrict__ gtab) {
+    const int D = ((blockIdx.x * blockDim.x + threadIdx.x) >> 5) + 1;
     const int lane = threadIdx.x & 31;
-    if (warp_global >= a.tile * a.n_dur) return;
-    const int pl = warp_global / a.n_dur, jd = warp_global % a.n_dur;
+    if (D > gtab_max) return;
+    double sg = 0.0, sg2 = 0.0;
+    for (int j = lane; j < D; j += 32) {
+        const double g = tmpl_at(tmpl, n_tmpl, j, D);
+        sg += g; sg2 += g * g;
+    }
+    sg = warp_sum(sg); sg2 = warp_sum(sg2);
+    if (lane == 0) { gtab[2 * D] = sg; gtab[2 * D + 1] = sg2; }
+}
+
+// One thread per (period, duration): D, stride, mean(g_D), sum g_D^2 (table look-up), duplicate-D flag.
+__global__ void __launch_bounds__(256) k_durtab(TileArgs a) {
+    const int tr = blockIdx.x * blockDim.x + threadIdx.x;
+    if (tr >= a.tile * a.n_dur) return;
+    const int pl = tr / a.n_dur, jd = tr % a.n_dur;
     const double* qrow = a.dur_per_period ? a.durs + (a.p0 + pl) * (long long)a.n_dur : a.durs;
     const int D = points_in_duration(qrow[jd], a.n);
     int skip = 0;
     for (int k = 0; k < jd; ++k) skip |= (points_in_duration(qrow[k], a.n) == D);
     double sg = 0.0, sg2 = 0.0;
     if (!skip) {
-        for (int j = lane; j < D; j += 32) {
-            const double g = tmpl_at(a.tmpl, a.n_tmpl, j, D);
-            sg += g; sg2 += g * g;
+        if (D <= a.gtab_max) { sg = a.gtab[2 * D]; sg2 = a.gtab[2 * D + 1]; }
+        else {                       // beyond the table (not reached: it covers q_max): the same sums, serially
+            double p[32], p2[32];
+            for (int l = 0; l < 32; ++l) {
+                p[l] = 0.0; p2[l] = 0.0;
+                for (int j = l; j < D; j += 32) { const double g = tmpl_at(a.tmpl, a.n_tmpl, j, D); p[l] += g; p2[l] += g * g; }
+            }
+            for (int o = 16; o > 0; o >>= 1)             // the butterfly of warp_sum, lane by lane
+                for (int l = 0; l < o; ++l) { p[l] += p[l ^ o]; p2[l] += p2[l ^ o]; }
+            sg = p[0]; sg2 = p2[0];
         }
-        sg = warp_sum(sg); sg2 = warp_sum(sg2);
     }
-    if (lane == 0) {
-        DurEntry e;
-        e.D = D; e.stride = t0_stride(D, a.dt0);
-        e.gbar = __ddiv_rn(sg, (double)D); e.gg2 = sg2; e.skip = skip; e.pad_ = 0;
-        a.durtab[(long long)pl * a.n_dur + jd] = e;
-    }
+    DurEntry e;
+    e.D = D; e.stride = t0_stride(D, a.dt0);
+    e.gbar = __ddiv_rn(sg, (double)D); e.gg2 = sg2; e.skip = skip; e.pad_ = 0;
+    a.durtab[tr] = e;
 }
 
 // chi2 variant of one trial (see chi2_ring.cu): classes of at most 21 taps, ring size, narrow/wide.
@@ -200,10 +219,14 @@ void launch_grid_check(const double* periods, long long n_per, const double* dur
 
 void launch_bin_trials(const TileArgs& a, cudaStream_t st) { k_bin_trials<<<1, 1024, 0, st>>>(a); }
 
+void launch_gtab(const double* tmpl, int n_tmpl, int gtab_max, double* gtab, cudaStream_t st) {
+    const int blocks = (int)(((long long)gtab_max * 32 + 255) / 256);
+    k_gtab<<<blocks, 256, 0, st>>>(tmpl, n_tmpl, gtab_max, gtab);
+}
+
 void launch_durtab(const TileArgs& a, cudaStream_t st) {
-    const long long warps = (long long)a.tile * a.n_dur;
-    const int blocks = (int)((warps * 32 + 255) / 256);
-    k_durtab<<<blocks, 256, 0, st>>>(a);
+    const long long trials = (long long)a.tile * a.n_dur;
+    k_durtab<<<(int)((trials + 255) / 256), 256, 0, st>>>(a);
 }
 
 }  // namespace gtls
