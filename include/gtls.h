@@ -91,7 +91,10 @@ typedef struct {
                                     1: duration_grid[n_per][n_dur] (row per period, reading G12)   */
     int32_t  sde_kernel;         /* odd window of the moving-median detrend (PAPER.md:279,
                                     reading G17); 0 or 1 => SDE = SDE_raw                          */
-    int32_t  chi2_fp32;          /* 0 = fp64.  1 (fp32 in-transit variant) => GTLS_EUNSUPPORTED     */
+    int32_t  chi2_fp32;          /* 0 = fp64.  1 = fp32 in-transit variant: template taps, X and the
+                                    window accumulators of the chi2 kernels in fp32 (<= 24 products
+                                    per sum); column sums, prefix sums, depth and scoring stay fp64.
+                                    chi2 within 1e-6 relative of the fp64 result (north_star: 1e-4)  */
     int32_t  pointers_on_device; /* see Conventions                                               */
     int32_t  device;             /* CUDA device ordinal                                           */
     void*    stream;             /* cudaStream_t                                                  */

@@ -222,15 +222,15 @@ __device__ __forceinline__ void reduce_batch(const Cls& c, const It& it, const i
 // >= rows_valid read as 0 (rows_min = the smallest rows_valid of the warp, so batches below it need
 // no predicate).  Taps T[m] multiply row (window + m).  Narrow path: every KB blocks the table slice
 // is scored and recycled.
-template <int MB, bool NARROW>
+template <int MB, bool NARROW, typename F>
 __device__ __forceinline__ void march(const Cls& c, const It& it, const double* __restrict__ xp,
                                       const int rows_valid, const int rows_min, const int nblk,
-                                      const double (&T)[MB], const int lane, Cand& best) {
+                                      const F (&T)[MB], const int lane, Cand& best) {
     constexpr int PF = PfRows<MB>::v;
     static_assert(MB % PF == 0 && kFifoBatches * PF <= kFifoRows && PF <= kPartRows, "geometry");
-    double acc[MB], xr[PF];
+    F acc[MB], xr[PF];
 #pragma unroll
-    for (int u = 0; u < MB; ++u) acc[u] = 0.0;
+    for (int u = 0; u < MB; ++u) acc[u] = (F)0;
     const unsigned fl = c.fifo + (unsigned)(lane * 8);
     const long long rstride = (long long)c.stp;
     int row_pf = 0;                                // row index the next copy belongs to
@@ -256,7 +256,7 @@ __device__ __forceinline__ void march(const Cls& c, const It& it, const double* 
                 cp_async_wait<kFifoBatches - 1>();
                 const unsigned fa = fl + (unsigned)(fb * PF * 256);
 #pragma unroll
-                for (int k = 0; k < PF; ++k) xr[k] = lds64(fa + k * 256);
+                for (int k = 0; k < PF; ++k) xr[k] = (F)lds64(fa + k * 256);
                 if (row_pf + PF <= rows_min) {
 #pragma unroll
                     for (int k = 0; k < PF; ++k) { cp_async8(fa + k * 256, xp); xp += rstride; }
@@ -268,7 +268,7 @@ __device__ __forceinline__ void march(const Cls& c, const It& it, const double* 
                 cp_async_commit();
                 fb = fb + 1 == kFifoBatches ? 0 : fb + 1;
             }
-            const double x = xr[u % PF];
+            const F x = xr[u % PF];
 #pragma unroll
             for (int m = 0; m < MB; ++m) {
                 const int a = (u - m + MB) % MB;
@@ -278,7 +278,7 @@ __device__ __forceinline__ void march(const Cls& c, const It& it, const double* 
             // window gamma - (MB-1) is complete
             const unsigned ea = (NARROW && it.direct) ? tab_lane + (unsigned)((bis * MB + u) * 8)
                                           : part_lane + (unsigned)((u % PF) * kPartPitch * 8);
-            sts64(ea, acc[(u + 1) % MB]);
+            sts64(ea, (double)acc[(u + 1) % MB]);
             if (u % PF == PF - 1 && !(NARROW && it.direct))
                 reduce_batch<PF, NARROW>(c, it, blk * MB + (u - (PF - 1)) - (MB - 1), kw_base, lane);
         }
@@ -306,19 +306,19 @@ __device__ __forceinline__ void march(const Cls& c, const It& it, const double* 
 //   - the column sums of a completed batch of PF windows are spread over the rows of the NEXT batch:
 //     A (batch end) 4 loads, B 4 loads + first partial sum, C second partial sum, D/E the two shuffle
 //     steps and the table load, F the table store.  Two emit buffers alternate.
-template <int MB>
+template <int MB, typename F>
 __device__ __forceinline__ void march_pipe(const Cls& c, const It& it, const double* __restrict__ xp,
                                            const int rows_valid, const int rows_min, const int nblk,
-                                           const double (&T)[MB], const int lane) {
+                                           const F (&T)[MB], const int lane) {
     constexpr int PF = PfRows<MB>::v;
     constexpr int NBAT = MB / PF;                  // copy groups in flight = batches per block
     constexpr int XQ = (MB % 3 == 0) ? 3 : 4;      // X registers; LA rows of look-ahead
     constexpr int LA = XQ - 1;
     static_assert(PF >= 6 && MB % PF == 0 && MB % XQ == 0 && MB <= kFifoRows && 2 * PF <= kPartRows, "geometry");
     constexpr unsigned kRowB = kPartPitch * 8;     // bytes per emit-buffer row
-    double acc[MB], xq[XQ];
+    F acc[MB], xq[XQ];
 #pragma unroll
-    for (int u = 0; u < MB; ++u) acc[u] = 0.0;
+    for (int u = 0; u < MB; ++u) acc[u] = (F)0;
     const unsigned fl = c.fifo + (unsigned)(lane * 8);
     const long long rstride = (long long)c.stp;
     int row_issue = 0;                             // next row to copy
@@ -334,7 +334,7 @@ __device__ __forceinline__ void march_pipe(const Cls& c, const It& it, const dou
     }
     cp_async_wait<NBAT - 1>();
 #pragma unroll
-    for (int k = 0; k < LA; ++k) xq[k] = lds64(fl + (unsigned)(k * 256));
+    for (int k = 0; k < LA; ++k) xq[k] = (F)lds64(fl + (unsigned)(k * 256));
 
     // column-sum roles: lane = (window slot sl, quarter r); quarter r adds lanes r, r+4, ..., r+28
     const int sl = lane >> 2, r = lane & 3;
@@ -367,15 +367,15 @@ __device__ __forceinline__ void march_pipe(const Cls& c, const It& it, const dou
                 cp_async_commit();
                 cp_async_wait<NBAT - 1>();
             }
-            xq[(u + LA) % XQ] = lds64(fl + (unsigned)(((u + LA) % MB) * 256));
-            const double x = xq[u % XQ];
+            xq[(u + LA) % XQ] = (F)lds64(fl + (unsigned)(((u + LA) % MB) * 256));
+            const F x = xq[u % XQ];
 #pragma unroll
             for (int m = 0; m < MB; ++m) {
                 const int a = (u - m + MB) % MB;
                 if (m == 0) acc[a] = T[0] * x;                      // window gamma starts at this row
                 else acc[a] = fma(T[m], x, acc[a]);
             }
-            sts64(pcur + (unsigned)((u % PF) * kRowB), acc[(u + 1) % MB]);   // window gamma-(MB-1) complete
+            sts64(pcur + (unsigned)((u % PF) * kRowB), (double)acc[(u + 1) % MB]);   // window gamma-(MB-1) complete
             // column sums of the previous batch, one stage per row
             if (u % PF == 0) {
                 sa = (v0 + v1) + (v2 + v3);
@@ -427,19 +427,19 @@ __device__ __forceinline__ double tmpl_lerp(const double* __restrict__ tm, int n
 
 // One march of the lanes' (segment, column) slots: taps, bounds, then the ring.
 //   seg/col: this lane's slot (active == false: an idle lane, zero taps);  row0: first row of seg.
-template <int MB, bool PIPE, bool NARROW>
+template <int MB, bool PIPE, bool NARROW, typename F>
 __device__ __forceinline__ void run_march(const Cls& c, const It& it, const int n, const int n_tmpl,
                                           const double tscale, const double* __restrict__ tm,
                                           const double* __restrict__ x, const bool square,
                                           const bool active, const int row0, const int col,
                                           const int lane, Cand& best) {
-    double T[MB];
+    F T[MB];                                                         // taps: fp64 template, rounded once to F
 #pragma unroll
     for (int m = 0; m < MB; ++m) {
         const int j = m * c.stp + col;
         double g = 0.0;
         if (active && j < c.D) g = tmpl_lerp(tm, n_tmpl, j, tscale);
-        T[m] = square ? g * g : g;
+        T[m] = (F)(square ? g * g : g);
     }
     const int nblk = (it.L + MB - 1 + MB - 1) / MB;
     const int rows_all = nblk * MB + kFifoBatches * PfRows<MB>::v;   // rows ever requested
@@ -451,11 +451,11 @@ __device__ __forceinline__ void run_march(const Cls& c, const It& it, const int 
         rows_valid = rv > rows_all ? rows_all : (int)rv;
     }
     const int rows_min = __reduce_min_sync(0xffffffffu, rows_valid);
-    if constexpr (PIPE) march_pipe<MB>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane);
-    else march<MB, NARROW>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane, best);
+    if constexpr (PIPE) march_pipe<MB, F>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane);
+    else march<MB, NARROW, F>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane, best);
 }
 
-template <int MB, bool NARROW>
+template <int MB, bool NARROW, typename F>
 __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n_tmpl, const double tscale,
                                           const double* __restrict__ tm, const double* __restrict__ x1,
                                           const double* __restrict__ x0, const int lane, Cand& best) {
@@ -476,7 +476,7 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
         const bool active = lane < it.G * c.stp;
         const int seg = min(lane / c.stp, it.G - 1);
         const int col = lane - seg * c.stp;      // idle lanes read on behind the last segment (zero taps)
-        run_march<MB, false, true>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best);
+        run_march<MB, false, true, F>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best);
         return;
     }
     // ---- wide: window tiles of the table size; the tile's stp columns are cut into nc balanced chunks of
@@ -501,7 +501,7 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
                 const bool active = lane < cw && c0 + lane < c.stp;
                 const int col = c0 + lane;     // idle lanes read on behind the chunk (zero taps): the warp's
                                                // copies stay one contiguous, conflict-free 256-byte row
-                run_march<MB, kPipe, false>(c, it, n, n_tmpl, tscale, tm, pass == 0 ? x1 : x0, pass == 1, active, k0,
+                run_march<MB, kPipe, false, F>(c, it, n, n_tmpl, tscale, tm, pass == 0 ? x1 : x0, pass == 1, active, k0,
                                      col, lane, best);
             }
         }
@@ -511,7 +511,7 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
     }
 }
 
-template <int MB, bool NARROW, bool UNIFORM>
+template <int MB, bool NARROW, bool UNIFORM, typename F>
 __global__ void __launch_bounds__(kRT, 6) k_chi2_ring(TileArgs a, const int* __restrict__ list,
                                                       const int* __restrict__ count) {
     extern __shared__ double dsm[];                 // per warp: emit buffer, X FIFO, window table
@@ -580,7 +580,7 @@ __global__ void __launch_bounds__(kRT, 6) k_chi2_ring(TileArgs a, const int* __r
     for (int r = 0; r < ncls; ++r) {
         c.off = r * st;
         c.nWr = nW > r ? (nW - r + ncls - 1) / ncls : 0;
-        run_class<MB, NARROW>(c, a.n, a.n_tmpl, tscale, tm, x1, x0, lane, best);
+        run_class<MB, NARROW, F>(c, a.n, a.n_tmpl, tscale, tm, x1, x0, lane, best);
     }
 
     // warp-wide lexicographic min on (d, s)
@@ -598,22 +598,26 @@ __global__ void __launch_bounds__(kRT, 6) k_chi2_ring(TileArgs a, const int* __r
 
 }  // namespace
 
-template <int MB, bool NARROW, bool UNIFORM>
-static void launch_variant(const TileArgs& a, int v, cudaStream_t st) {
+template <int MB, bool NARROW, bool UNIFORM, typename F>
+static void launch_variant_t(const TileArgs& a, int v, cudaStream_t st) {
     const long long trials = (long long)a.tile * a.n_dur;
     const unsigned grid = (unsigned)((trials + kRW - 1) / kRW);     // worst case; surplus CTAs exit at once
     const size_t sm = (size_t)(kRW * kWarpSmem) * sizeof(double);
     static bool set = false;
     if (!set) {
-        cudaFuncSetAttribute(k_chi2_ring<MB, NARROW, UNIFORM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+        cudaFuncSetAttribute(k_chi2_ring<MB, NARROW, UNIFORM, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
         set = true;
     }
-    k_chi2_ring<MB, NARROW, UNIFORM><<<grid, kRT, sm, st>>>(a, a.trial_list + (long long)v * trials, a.trial_count + v);
+    k_chi2_ring<MB, NARROW, UNIFORM, F><<<grid, kRT, sm, st>>>(a, a.trial_list + (long long)v * trials, a.trial_count + v);
+}
+// fp64 ring (default) or the fp32 in-transit variant (gtls_opts.chi2_fp32: taps, X and the ring
+// accumulators in fp32 -- at most 24 products per sum; column sums, prefix sums and scoring stay fp64)
+template <int MB, bool NARROW, bool UNIFORM>
+static void launch_variant(const TileArgs& a, int v, cudaStream_t st) {
+    if (a.chi2_fp32) launch_variant_t<MB, NARROW, UNIFORM, float>(a, v, st);
+    else launch_variant_t<MB, NARROW, UNIFORM, double>(a, v, st);
 }
 
-// The variants other than the dominant one (21-ring, wide) often hold few, long trials: alone on the
-// device they leave most warp slots empty.  They are launched on a side stream of higher priority between
-// two events, so their CTAs take slots first and the dominant kernel fills the rest of the device.
 void launch_chi2_ring(const TileArgs& a, cudaStream_t st) {
     launch_bin_trials(a, st);
     cudaStream_t ss = st;

@@ -297,7 +297,8 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     if (n < 3 || n > 0x3fffffff || n_per < 1 || n_dur < 1 || n_dur > 4096 || n_tmpl < 2) return GTLS_EINVAL;
     if (!(o.dt0 >= 0.0) || o.sde_kernel < 0 || (o.sde_kernel > 1 && o.sde_kernel % 2 == 0)) return GTLS_EINVAL;
     if (o.path < 0 || o.path > 2 || o.period_tile < 0) return GTLS_EINVAL;
-    if (o.top_k != 0 || o.chi2_fp32 != 0) return GTLS_EUNSUPPORTED;
+    if (o.top_k != 0) return GTLS_EUNSUPPORTED;
+    if (o.chi2_fp32 != 0 && o.chi2_fp32 != 1) return GTLS_EINVAL;
     if (o.path == 1) return GTLS_EUNSUPPORTED;   // fused shared-memory path: not built yet
     CU(cudaSetDevice(o.device));
     cudaStream_t st = (cudaStream_t)o.stream;
@@ -401,7 +402,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     TileArgs a;
     memset(&a, 0, sizeof(a));
     a.n = (int)n; a.n_dur = n_dur; a.n_tmpl = n_tmpl; a.dur_per_period = o.dur_per_period;
-    a.dt0 = o.dt0; a.uniform = uniform ? 1 : 0; a.w_uniform = info.w_min;
+    a.dt0 = o.dt0; a.uniform = uniform ? 1 : 0; a.w_uniform = info.w_min; a.chi2_fp32 = o.chi2_fp32;
     a.pitch = pitch_for(n, info.q_max); a.spitch = a.pitch + 8;
     a.t = d_t; a.wr = d_wr; a.w = d_w; a.wr2 = d_wr2; a.periods = d_per; a.durs = d_dur;
     a.tmpl = d_tmpl; a.chi2_0 = &d_info->chi2_0;

@@ -146,6 +146,7 @@ struct TileArgs {
     const int* seg_count;  // number of entries of seg_list (device)
     int* trial_list;       // [kChi2Variants][tile*n_dur] trial indices binned by chi2 kernel variant
     int* trial_count;      // [kChi2Variants]
+    int chi2_fp32;         // 1: fp32 ring arithmetic in the chi2 kernels (gtls_opts.chi2_fp32)
     const double* gtab;    // [2*(gtab_max+1)] sum g_D, sum g_D^2 for D = 1 .. gtab_max (k_gtab)
     int gtab_max;
     int dbg_min_st, dbg_max_st;   // timing experiments only (GTLS_DBG_MIN_ST / GTLS_DBG_MAX_ST): skip other trials

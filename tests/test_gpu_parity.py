@@ -307,6 +307,29 @@ def test_two_stage_search_matches_oracle(cfg, every, n_refine):
     assert np.all(chi2[np.setdiff1d(np.arange(w.n_per), refined)] == np.asarray(coarse.chi2)[np.setdiff1d(np.arange(w.n_per), refined)])
 
 
+@pytest.mark.parametrize("cfg,every,hetero", [(1, 7, False), (2, 101, True), (3, 8375, False)])
+def test_fp32_in_transit_variant(cfg, every, hetero):
+    """gtls_opts.chi2_fp32 = 1: taps, X and the ring accumulators in fp32 (at most 24 products per sum),
+    everything else fp64.  north_star allows 1e-4 relative on chi2 for an fp32 variant; the construction
+    keeps it below 1e-6, which is what is asserted.  Two near-equal windows may swap, so indices are
+    required to agree on 99 % of the periods and exactly at the global best period."""
+    _cuda()
+    w = gi.make_workload(cfg, hetero=hetero).subset(every)
+    ora = oracle.search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05)
+    res = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05, sde_kernel=31,
+                        chi2_fp32=1)
+    assert res.code == 0
+    chi2 = np.asarray(res.chi2)
+    rel = np.max(np.abs(chi2 - ora.chi2) / ora.chi2)
+    assert rel <= 1e-6, rel
+    b = res.best()
+    same = (b["dur_idx"] == ora.best["dur_idx"]) & (b["start"] == ora.best["start"])
+    assert same.mean() >= 0.99
+    s = oracle.sde(ora.chi2, 31)
+    assert res.summary["best_period_idx"] == s.best_period_idx and same[s.best_period_idx]
+    assert np.abs(np.asarray(res.sde) - s.sde).max() <= 1e-3
+
+
 def test_tiny_and_degenerate_inputs(tmpl512):
     _cuda()
     rng = np.random.default_rng(3)
