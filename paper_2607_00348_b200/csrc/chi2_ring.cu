@@ -557,7 +557,7 @@ __global__ void __launch_bounds__(kRT, 6) k_chi2_ring(TileArgs a, const int* __r
     const int st = e.stride;
     const int nW = (a.n + st - 1) / st;
     const int M = (e.D + st - 1) / st;
-    const int ncls = chi2_classes(M, st);           // window classes: at most MB taps each
+    const int ncls = chi2_classes(M, st, UNIFORM);           // window classes: at most MB taps each
     Cls c;
     c.D = e.D; c.stp = ncls * st;
     c.uniform = UNIFORM;
@@ -634,14 +634,12 @@ void launch_chi2_ring(const TileArgs& a, cudaStream_t st) {
         launch_variant<4, true, true>(a, 11, ss);
         launch_variant<24, true, true>(a, 6, ss);
         launch_variant<21, true, true>(a, 7, ss);
-        launch_variant<24, false, true>(a, 0, ss);
         launch_variant<16, false, true>(a, 2, ss);
         launch_variant<12, false, true>(a, 3, ss);
         launch_variant<8, false, true>(a, 4, ss);
         launch_variant<4, false, true>(a, 5, ss);
         launch_variant<21, false, true>(a, 1, st);
     } else {
-        launch_variant<24, false, false>(a, 0, ss);
         launch_variant<16, false, false>(a, 2, ss);
         launch_variant<12, false, false>(a, 3, ss);
         launch_variant<8, false, false>(a, 4, ss);

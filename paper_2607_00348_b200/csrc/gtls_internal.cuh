@@ -45,10 +45,15 @@ constexpr int kChi2Rings = 6;
 constexpr int kChi2Variants = 2 * kChi2Rings;
 constexpr int kChi2NarrowMax = 16;   // largest class stride handled by the narrow variants
 // Window classes of a trial with M = ceil(D/stride) taps: the smallest count that leaves at most 24 taps
-// per class (21 when the stride is 1: 32 side-by-side segments of a 24-ring do not fit the window table).
-// (A 28-ring was measured: its unrolled body outgrows the instruction cache and spills; 2 classes win.)
-__host__ __device__ __forceinline__ int chi2_classes(int M, int stride) {
-    return stride == 1 ? (M + 20) / 21 : (M + 23) / 24;
+// per class when the class stride stays narrow (<= kChi2NarrowMax), at most 21 otherwise and when the
+// stride is 1 (32 side-by-side segments of a 24-ring do not fit the window table).  The 24-ring is a
+// narrow-path ring only: as a wide kernel it is slower per tap than the pipelined 21-ring (measured on
+// c3 at dt0 = 0.01).  (A 28-ring was measured too: its unrolled body outgrows the instruction cache.)
+// (Non-uniform dy has no narrow path: 21 throughout.)
+__host__ __device__ __forceinline__ int chi2_classes(int M, int stride, bool uniform) {
+    if (stride == 1 || !uniform) return (M + 20) / 21;
+    const int c = (M + 23) / 24;
+    return c * stride <= kChi2NarrowMax ? c : (M + 20) / 21;
 }
 __host__ __device__ __forceinline__ int chi2_ring_index(int taps) {
     return taps > 21 ? 0 : (taps > 16 ? 1 : (taps > 12 ? 2 : (taps > 8 ? 3 : (taps > 4 ? 4 : 5))));

@@ -145,7 +145,7 @@ __global__ void __launch_bounds__(256) k_durtab(TileArgs a) {
 __device__ __forceinline__ int chi2_variant(const DurEntry& e, const TileArgs& a) {
     if (e.skip || e.stride < a.dbg_min_st || e.stride > a.dbg_max_st) return -1;
     const int M = (e.D + e.stride - 1) / e.stride;
-    const int ncls = chi2_classes(M, e.stride);
+    const int ncls = chi2_classes(M, e.stride, a.uniform != 0);
     const int stp = ncls * e.stride;
     const int mbi = chi2_ring_index((e.D + stp - 1) / stp);
     const int narrow = (a.uniform && stp <= kChi2NarrowMax) ? 1 : 0;
