@@ -85,8 +85,10 @@ typedef struct {
 typedef struct {
     uint32_t struct_size;        /* sizeof(gtls_opts), for ABI versioning                         */
     double   dt0;                /* Eq. 18: stride = max(1, floor(D*dt0)); 0 => 1   */
-    int32_t  top_k;              /* 0 => every strided start (paper). K>0 (K deepest windows per
-                                    (period, duration), reading G19) => GTLS_EUNSUPPORTED for now  */
+    int32_t  top_k;              /* 0 => chi2 at every strided start (the paper's search).
+                                    K in 1..8 => pruning variant (reading G19): per (period, duration)
+                                    the K starts of largest running-mean depth (ties: lower start) and
+                                    chi2 only there.  K > 8, or K > 0 with chi2_fp32 => GTLS_EUNSUPPORTED */
     int32_t  dur_per_period;     /* 0: duration_grid[n_dur] shared by all periods;
                                     1: duration_grid[n_per][n_dur] (row per period, reading G12)   */
     int32_t  sde_kernel;         /* odd window of the moving-median detrend (PAPER.md:279,

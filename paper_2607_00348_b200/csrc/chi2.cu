@@ -160,7 +160,8 @@ __global__ void __launch_bounds__(128) k_reduce(TileArgs a, double* __restrict__
         int bj = -1;
         double bd = 0.0;
         for (int jd = 0; jd < a.n_dur; ++jd) {
-            const unsigned long long nw = (unsigned long long)((a.n + dd[jd].stride - 1) / dd[jd].stride);
+            unsigned long long nw = (unsigned long long)((a.n + dd[jd].stride - 1) / dd[jd].stride);
+            if (a.top_k > 0 && nw > (unsigned long long)a.top_k) nw = (unsigned long long)a.top_k;   // pruning variant
             nwin += nw;
             if (!dd[jd].skip) npts += nw * (unsigned long long)dd[jd].D;
             if (!pp[jd].valid) continue;

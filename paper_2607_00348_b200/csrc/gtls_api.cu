@@ -297,7 +297,8 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     if (n < 3 || n > 0x3fffffff || n_per < 1 || n_dur < 1 || n_dur > 4096 || n_tmpl < 2) return GTLS_EINVAL;
     if (!(o.dt0 >= 0.0) || o.sde_kernel < 0 || (o.sde_kernel > 1 && o.sde_kernel % 2 == 0)) return GTLS_EINVAL;
     if (o.path < 0 || o.path > 2 || o.period_tile < 0) return GTLS_EINVAL;
-    if (o.top_k != 0) return GTLS_EUNSUPPORTED;
+    if (o.top_k < 0) return GTLS_EINVAL;
+    if (o.top_k > kTopKMax || (o.top_k > 0 && o.chi2_fp32)) return GTLS_EUNSUPPORTED;
     if (o.chi2_fp32 != 0 && o.chi2_fp32 != 1) return GTLS_EINVAL;
     if (o.path == 1) return GTLS_EUNSUPPORTED;   // fused shared-memory path: not built yet
     CU(cudaSetDevice(o.device));
@@ -402,7 +403,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     TileArgs a;
     memset(&a, 0, sizeof(a));
     a.n = (int)n; a.n_dur = n_dur; a.n_tmpl = n_tmpl; a.dur_per_period = o.dur_per_period;
-    a.dt0 = o.dt0; a.uniform = uniform ? 1 : 0; a.w_uniform = info.w_min; a.chi2_fp32 = o.chi2_fp32;
+    a.dt0 = o.dt0; a.uniform = uniform ? 1 : 0; a.w_uniform = info.w_min; a.chi2_fp32 = o.chi2_fp32; a.top_k = o.top_k;
     a.pitch = pitch_for(n, info.q_max); a.spitch = a.pitch + 8;
     a.t = d_t; a.wr = d_wr; a.w = d_w; a.wr2 = d_wr2; a.periods = d_per; a.durs = d_dur;
     a.tmpl = d_tmpl; a.chi2_0 = &d_info->chi2_0;
@@ -446,11 +447,12 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
         run_fold_sort_scan(a, ssc, nullptr, nullptr, -1, false, nullptr, st, &launches);
         tm.mark(3);
         tm.mark(4);
-        if (use_v1) launch_chi2(a, st); else if (use_rows) launch_chi2_rows(a, st); else launch_chi2_ring(a, st);
+        if (a.top_k > 0) launch_chi2_topk(a, st);
+        else if (use_v1) launch_chi2(a, st); else if (use_rows) launch_chi2_rows(a, st); else launch_chi2_ring(a, st);
         tm.mark(5);
         launch_reduce(a, d_chi2, d_best, d_counters, st);
         tm.mark(6);
-        stats.kernel_launches += launches + 2 + ((use_v1 || use_rows) ? 1 : 1 + (uniform ? kChi2Variants - 1 : kChi2Variants / 2 - 1));
+        stats.kernel_launches += launches + 2 + ((use_v1 || use_rows || a.top_k > 0) ? 1 : 1 + (uniform ? kChi2Variants - 1 : kChi2Variants / 2 - 1));
         stats.chi2_launches += 1;
         if (o.stats) {
             CU(cudaStreamSynchronize(st));

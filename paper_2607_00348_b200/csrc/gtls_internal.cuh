@@ -151,6 +151,7 @@ struct TileArgs {
     const int* seg_count;  // number of entries of seg_list (device)
     int* trial_list;       // [kChi2Variants][tile*n_dur] trial indices binned by chi2 kernel variant
     int* trial_count;      // [kChi2Variants]
+    int top_k;             // > 0: chi2 only at the K deepest starts of every trial (chi2_topk.cu, reading G19)
     int chi2_fp32;         // 1: fp32 ring arithmetic in the chi2 kernels (gtls_opts.chi2_fp32)
     const double* gtab;    // [2*(gtab_max+1)] sum g_D, sum g_D^2 for D = 1 .. gtab_max (k_gtab)
     int gtab_max;
@@ -192,6 +193,8 @@ void launch_curve_pre(const double* t, const double* y, const double* dy, int n,
                       double* w, double* wr2, CurveInfo* info, cudaStream_t st);
 void launch_grid_check(const double* periods, long long n_per, const double* durs,
                        long long n_durs_total, CurveInfo* info, cudaStream_t st);
+constexpr int kTopKMax = 8;   // largest gtls_opts.top_k the pruning kernel takes (per-lane lists live in registers)
+void launch_chi2_topk(const TileArgs& a, cudaStream_t st);
 void launch_gtab(const double* tmpl, int n_tmpl, int gtab_max, double* gtab, cudaStream_t st);
 void launch_durtab(const TileArgs& a, cudaStream_t st);
 // bins the tile's trials by chi2 kernel variant (order preserved); skipped trials get an invalid Partial

@@ -72,8 +72,11 @@ def test_argument_errors_before_cuda(lib):
         g.gtls_search(t, y, dy, per, q, tm, sde_kernel=10)
     assert e.value.code == -1
     with pytest.raises(g.GtlsError) as e:
-        g.gtls_search(t, y, dy, per, q, tm, top_k=3)
+        g.gtls_search(t, y, dy, per, q, tm, top_k=9)            # pruning variant takes K <= 8
     assert e.value.code == -7
+    with pytest.raises(g.GtlsError) as e:
+        g.gtls_search(t, y, dy, per, q, tm, top_k=-1)
+    assert e.value.code == -1
     with pytest.raises(g.GtlsError) as e:
         g.gtls_search(t, y, dy, per, q, tm, dt0=-0.1)
     assert e.value.code == -1

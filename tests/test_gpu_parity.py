@@ -330,6 +330,33 @@ def test_fp32_in_transit_variant(cfg, every, hetero):
     assert np.abs(np.asarray(res.sde) - s.sde).max() <= 1e-3
 
 
+@pytest.mark.parametrize("cfg,every,hetero,dt0,k", [
+    (1, 7, False, 0.05, 1), (1, 13, True, 0.0, 3), (2, 101, False, 0.05, 8), (2, 211, True, 0.1, 4),
+    (3, 8375, False, 0.05, 5),
+])
+def test_top_k_pruning_variant(cfg, every, hetero, dt0, k):
+    """gtls_opts.top_k = K (reading G19): chi2 only at the K starts of largest running-mean depth per
+    (period, duration).  The oracle takes the running mean by direct sums, the GPU from prefix sums: two
+    starts whose depths agree to ~1e-13 may swap at the selection boundary, so chi2 / indices are required
+    on 99 % of the periods, and the evaluated-window count exactly."""
+    _cuda()
+    w = gi.make_workload(cfg, hetero=hetero).subset(every)
+    ora = oracle.search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=dt0, top_k=k)
+    res = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=dt0, sde_kernel=31,
+                        top_k=k)
+    assert res.code == 0
+    chi2 = np.asarray(res.chi2)
+    ok = np.abs(chi2 - ora.chi2) <= CHI2_RTOL * ora.chi2
+    b = res.best()
+    same = (b["dur_idx"] == ora.best["dur_idx"]) & (b["start"] == ora.best["start"])
+    assert ok.mean() >= 0.99 and same.mean() >= 0.99, (ok.mean(), same.mean())
+    assert np.all(ok[same])
+    assert res.summary["windows_evaluated"] == ora.windows
+    # pruning can only raise chi2 relative to the full search (the K starts are among all starts)
+    full = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=dt0, sde_kernel=31)
+    assert np.all(chi2 >= np.asarray(full.chi2) * (1 - 1e-12))
+
+
 def test_tiny_and_degenerate_inputs(tmpl512):
     _cuda()
     rng = np.random.default_rng(3)
