@@ -298,6 +298,115 @@ __device__ __forceinline__ void march(const Cls& c, const It& it, const double* 
     }
 }
 
+// Narrow path when dy is NOT uniform: C = sum g x1 and G = sum g^2 x0 are needed for every window of the
+// time-sliced table, so both are accumulated in ONE march: two rings (C, G) over two FIFO streams
+// (x1 = w r, x0 = w), taps g held once (g^2 x0 is taken as g * (g * x0)).  3 MB doubles of ring state:
+// ring sizes up to 16.  Batches of kDualPF rows per stream, the two streams share the FIFO half and half;
+// the emit buffer holds the C partials in rows [0, PF) and the G partials in rows [PF, 2 PF).
+constexpr int kDualPF = 4;
+template <int MB, typename F>
+__device__ __forceinline__ void march_dual(const Cls& c, const It& it, const double* __restrict__ xp1,
+                                           const double* __restrict__ xp0, const int rows_valid,
+                                           const int rows_min, const int nblk, const F (&T)[MB],
+                                           const int lane, Cand& best) {
+    constexpr int PF = kDualPF;
+    constexpr int kHalf = kFifoRows / 2;           // FIFO rows per stream
+    static_assert(MB % PF == 0 && kFifoBatches * PF <= kHalf && 2 * PF <= kPartRows, "geometry");
+    F accC[MB], accG[MB], xr1[PF], xr0[PF];
+#pragma unroll
+    for (int u = 0; u < MB; ++u) { accC[u] = (F)0; accG[u] = (F)0; }
+    const unsigned fl1 = c.fifo + (unsigned)(lane * 8);
+    const unsigned fl0 = fl1 + (unsigned)(kHalf * 256);
+    const long long rstride = (long long)c.stp;
+    int row_pf = 0;
+#pragma unroll
+    for (int k = 0; k < kFifoBatches; ++k) {
+#pragma unroll
+        for (int u = 0; u < PF; ++u) {
+            cp_async8(fl1 + (unsigned)((k * PF + u) * 256), xp1, row_pf < rows_valid);
+            cp_async8(fl0 + (unsigned)((k * PF + u) * 256), xp0, row_pf < rows_valid);
+            xp1 += rstride; xp0 += rstride;
+            ++row_pf;
+        }
+        cp_async_commit();
+    }
+    int fb = 0;
+    int kw_base = -(MB - 1), bis = 0;
+    const unsigned part_lane = c.part + (unsigned)(lane * 8);
+    const unsigned tab_lane = it.tab + (unsigned)(lane * it.SL * 8);
+    const unsigned gofs = (unsigned)(c.Kt * 8);    // G table behind the C table
+#pragma unroll 1
+    for (int blk = 0; blk < nblk; ++blk) {
+#pragma unroll
+        for (int u = 0; u < MB; ++u) {
+            if (u % PF == 0) {
+                cp_async_wait<kFifoBatches - 1>();
+                const unsigned fa1 = fl1 + (unsigned)(fb * PF * 256), fa0 = fl0 + (unsigned)(fb * PF * 256);
+#pragma unroll
+                for (int k = 0; k < PF; ++k) { xr1[k] = (F)lds64(fa1 + k * 256); xr0[k] = (F)lds64(fa0 + k * 256); }
+#pragma unroll
+                for (int k = 0; k < PF; ++k) {
+                    const bool ok = row_pf + k < rows_valid;
+                    cp_async8(fa1 + k * 256, xp1, ok);
+                    cp_async8(fa0 + k * 256, xp0, ok);
+                    xp1 += rstride; xp0 += rstride;
+                }
+                row_pf += PF;
+                cp_async_commit();
+                fb = fb + 1 == kFifoBatches ? 0 : fb + 1;
+            }
+            const F x1v = xr1[u % PF], x0v = xr0[u % PF];
+#pragma unroll
+            for (int m = 0; m < MB; ++m) {
+                const int a = (u - m + MB) % MB;
+                const F gx = T[m] * x0v;
+                if (m == 0) { accC[a] = T[0] * x1v; accG[a] = T[0] * gx; }
+                else { accC[a] = fma(T[m], x1v, accC[a]); accG[a] = fma(T[m], gx, accG[a]); }
+            }
+            // window gamma - (MB-1) is complete
+            if (it.direct) {
+                const unsigned ea = tab_lane + (unsigned)((bis * MB + u) * 8);
+                sts64(ea, (double)accC[(u + 1) % MB]);
+                sts64(ea + gofs, (double)accG[(u + 1) % MB]);
+            } else {
+                const unsigned ea = part_lane + (unsigned)((u % PF) * kPartPitch * 8);
+                sts64(ea, (double)accC[(u + 1) % MB]);
+                sts64(ea + (unsigned)(PF * kPartPitch * 8), (double)accG[(u + 1) % MB]);
+                if (u % PF == PF - 1) {
+                    const int kwb = blk * MB + (u - (PF - 1)) - (MB - 1);
+                    __syncwarp();
+                    for (int t = lane; t < it.G * PF; t += 32) {
+                        const int g = t / PF, sl = t - g * PF;
+                        const unsigned pr = c.part + (unsigned)((sl * kPartPitch + g * c.stp) * 8);
+                        double a0 = 0.0, b0 = 0.0;
+                        for (int q = 0; q < c.stp; ++q) {
+                            a0 += lds64(pr + 8 * q);
+                            b0 += lds64(pr + 8 * q + (unsigned)(PF * kPartPitch * 8));
+                        }
+                        const unsigned ta = it.tab + (unsigned)((g * it.SL + (kwb + sl - kw_base)) * 8);
+                        sts64(ta, a0);
+                        sts64(ta + gofs, b0);
+                    }
+                    __syncwarp();
+                }
+            }
+        }
+        if (++bis == it.KB) {
+            __syncwarp();
+            score_narrow(c, best, lane, it.G, it.SL, it.SLn, it.invSL, kw_base, it.L);
+            __syncwarp();
+            kw_base += it.SLn;
+            bis = 0;
+        }
+    }
+    cp_async_wait<0>();
+    if (bis > 0) {
+        __syncwarp();
+        score_narrow(c, best, lane, it.G, it.SL, it.SLn, it.invSL, kw_base, it.L);
+        __syncwarp();
+    }
+}
+
 // Wide path, one segment per warp: the same march as a software pipeline.  A warp issues in order, so
 // every load is placed at least one row (MB DFMAs) before its first use:
 //   - the X value of row j+LA is read from the FIFO while row j is multiplied; whenever the reads enter a
@@ -427,12 +536,13 @@ __device__ __forceinline__ double tmpl_lerp(const double* __restrict__ tm, int n
 
 // One march of the lanes' (segment, column) slots: taps, bounds, then the ring.
 //   seg/col: this lane's slot (active == false: an idle lane, zero taps);  row0: first row of seg.
-template <int MB, bool PIPE, bool NARROW, typename F>
+template <int MB, bool PIPE, bool NARROW, typename F, bool DUAL = false>
 __device__ __forceinline__ void run_march(const Cls& c, const It& it, const int n, const int n_tmpl,
                                           const double tscale, const double* __restrict__ tm,
                                           const double* __restrict__ x, const bool square,
                                           const bool active, const int row0, const int col,
-                                          const int lane, Cand& best) {
+                                          const int lane, Cand& best,
+                                          const double* __restrict__ xw = nullptr) {
     F T[MB];                                                         // taps: fp64 template, rounded once to F
 #pragma unroll
     for (int m = 0; m < MB; ++m) {
@@ -451,20 +561,21 @@ __device__ __forceinline__ void run_march(const Cls& c, const It& it, const int 
         rows_valid = rv > rows_all ? rows_all : (int)rv;
     }
     const int rows_min = __reduce_min_sync(0xffffffffu, rows_valid);
-    if constexpr (PIPE) march_pipe<MB, F>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane);
+    if constexpr (DUAL) march_dual<MB, F>(c, it, x + ebase, xw + ebase, rows_valid, rows_min, nblk, T, lane, best);
+    else if constexpr (PIPE) march_pipe<MB, F>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane);
     else march<MB, NARROW, F>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane, best);
 }
 
-template <int MB, bool NARROW, typename F>
+template <int MB, bool NARROW, bool UNIFORM, typename F>
 __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n_tmpl, const double tscale,
                                           const double* __restrict__ tm, const double* __restrict__ x1,
                                           const double* __restrict__ x0, const int lane, Cand& best) {
     if (c.nWr <= 0) return;
     It it;
     it.tab = c.ctab;
-    if (NARROW) {
+    if constexpr (NARROW) {
         // ---- narrow: G segments side by side, one march over the whole class -------------------
-        it.direct = c.stp == 1;   // (NARROW implies uniform dy and stp <= kChi2NarrowMax)
+        it.direct = c.stp == 1;   // (stp <= kChi2NarrowMax; dy not uniform: C and G in one march, rings <= 16)
         it.G = 32 / c.stp;
         it.L = (c.nWr + it.G - 1) / it.G;
         it.KB = c.Kt / (it.G * MB);
@@ -476,7 +587,10 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
         const bool active = lane < it.G * c.stp;
         const int seg = min(lane / c.stp, it.G - 1);
         const int col = lane - seg * c.stp;      // idle lanes read on behind the last segment (zero taps)
-        run_march<MB, false, true, F>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best);
+        if constexpr (UNIFORM)
+            run_march<MB, false, true, F>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best);
+        else
+            run_march<MB, false, true, F, true>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best, x0);
         return;
     }
     // ---- wide: window tiles of the table size; the tile's stp columns are cut into nc balanced chunks of
@@ -580,7 +694,7 @@ __global__ void __launch_bounds__(kRT, 6) k_chi2_ring(TileArgs a, const int* __r
     for (int r = 0; r < ncls; ++r) {
         c.off = r * st;
         c.nWr = nW > r ? (nW - r + ncls - 1) / ncls : 0;
-        run_class<MB, NARROW, F>(c, a.n, a.n_tmpl, tscale, tm, x1, x0, lane, best);
+        run_class<MB, NARROW, UNIFORM, F>(c, a.n, a.n_tmpl, tscale, tm, x1, x0, lane, best);
     }
 
     // warp-wide lexicographic min on (d, s)
@@ -640,6 +754,10 @@ void launch_chi2_ring(const TileArgs& a, cudaStream_t st) {
         launch_variant<4, false, true>(a, 5, ss);
         launch_variant<21, false, true>(a, 1, st);
     } else {
+        launch_variant<12, true, false>(a, 9, ss);
+        launch_variant<16, true, false>(a, 8, ss);
+        launch_variant<8, true, false>(a, 10, ss);
+        launch_variant<4, true, false>(a, 11, ss);
         launch_variant<16, false, false>(a, 2, ss);
         launch_variant<12, false, false>(a, 3, ss);
         launch_variant<8, false, false>(a, 4, ss);

@@ -452,7 +452,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
         tm.mark(5);
         launch_reduce(a, d_chi2, d_best, d_counters, st);
         tm.mark(6);
-        stats.kernel_launches += launches + 2 + ((use_v1 || use_rows || a.top_k > 0) ? 1 : 1 + (uniform ? kChi2Variants - 1 : kChi2Variants / 2 - 1));
+        stats.kernel_launches += launches + 2 + ((use_v1 || use_rows || a.top_k > 0) ? 1 : 1 + (uniform ? kChi2Variants - 1 : kChi2Variants - 3));
         stats.chi2_launches += 1;
         if (o.stats) {
             CU(cudaStreamSynchronize(st));

@@ -49,11 +49,18 @@ constexpr int kChi2NarrowMax = 16;   // largest class stride handled by the narr
 // stride is 1 (32 side-by-side segments of a 24-ring do not fit the window table).  The 24-ring is a
 // narrow-path ring only: as a wide kernel it is slower per tap than the pipelined 21-ring (measured on
 // c3 at dt0 = 0.01).  (A 28-ring was measured too: its unrolled body outgrows the instruction cache.)
-// (Non-uniform dy has no narrow path: 21 throughout.)
+// dy not uniform: the narrow path carries two rings (C and G) per lane, so its rings hold at most 16 taps
+// (8 when the stride is 1: 32 segments x two tables); strides above 16 use the wide 21-ring.
 __host__ __device__ __forceinline__ int chi2_classes(int M, int stride, bool uniform) {
-    if (stride == 1 || !uniform) return (M + 20) / 21;
-    const int c = (M + 23) / 24;
-    return c * stride <= kChi2NarrowMax ? c : (M + 20) / 21;
+    if (uniform) {
+        if (stride == 1) return (M + 20) / 21;
+        const int c = (M + 23) / 24;
+        return c * stride <= kChi2NarrowMax ? c : (M + 20) / 21;
+    }
+    if (stride > kChi2NarrowMax) return (M + 20) / 21;
+    int c = (M + 15) / 16;                             // a class stride of 17 .. 32 is a wide march with
+    if (stride == 1 && M > 8 && c < 2) c = 2;          // twice the lanes a single class would fill
+    return c;                                          // (stride 1 with one class: at most 8 taps)
 }
 __host__ __device__ __forceinline__ int chi2_ring_index(int taps) {
     return taps > 21 ? 0 : (taps > 16 ? 1 : (taps > 12 ? 2 : (taps > 8 ? 3 : (taps > 4 ? 4 : 5))));

@@ -147,8 +147,10 @@ __device__ __forceinline__ int chi2_variant(const DurEntry& e, const TileArgs& a
     const int M = (e.D + e.stride - 1) / e.stride;
     const int ncls = chi2_classes(M, e.stride, a.uniform != 0);
     const int stp = ncls * e.stride;
-    const int mbi = chi2_ring_index((e.D + stp - 1) / stp);
-    const int narrow = (a.uniform && stp <= kChi2NarrowMax) ? 1 : 0;
+    const int taps = (e.D + stp - 1) / stp;
+    const int mbi = chi2_ring_index(taps);
+    // narrow path: class stride <= 16; when dy is not uniform its two-ring march takes at most 16 taps
+    const int narrow = (stp <= kChi2NarrowMax && (a.uniform || taps <= 16)) ? 1 : 0;
     return narrow * kChi2Rings + mbi;
 }
 
