@@ -88,7 +88,7 @@ int auto_tile(long long n_per, const Sizes& s, size_t budget) {
     return (int)t;
 }
 
-constexpr size_t kDefaultTileBudget = 12ull << 30;  // bytes of per-tile scratch when automatic
+constexpr size_t kDefaultTileBudget = 24ull << 30;  // bytes of per-tile scratch when automatic
 
 gtls_opts resolve_opts(const gtls_opts* in) {
     gtls_opts o;
@@ -398,6 +398,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     long long tile_cap = (long long)(avail / align_up(sz.per_period + 8 * 256));
     int tile = o.period_tile > 0 ? o.period_tile : auto_tile(n_per, sz, kDefaultTileBudget);
     if (tile > tile_cap) tile = (int)tile_cap;
+    if (o.period_tile <= 0 && tile >= kFinishSlots && tile < n_per) tile -= (int)(tile % kFinishSlots);   // see auto_tile
     if (tile > n_per) tile = (int)n_per;
     if (tile < 1) return GTLS_ENOMEM;
     TileArgs a;
