@@ -20,7 +20,7 @@ from typing import Any, Optional
 
 import numpy as np
 
-__all__ = ["gtls_search", "gtls_search_two_stage", "gtls_fold_sort", "gtls_fold_scan", "gtls_window_chi2", "gtls_sde",
+__all__ = ["gtls_search", "gtls_search_two_stage", "gtls_search_sharded", "gtls_fold_sort", "gtls_fold_scan", "gtls_window_chi2", "gtls_sde",
            "gtls_workspace_bytes", "gtls_strerror", "gtls_version", "GtlsError", "SearchResult",
            "BEST_DTYPE", "lib_path", "load_library"]
 
@@ -360,3 +360,56 @@ def gtls_sde(chi2, *, sde_kernel: int = 151, stream=None):
     if rc not in (GTLS_OK, GTLS_EDEGENERATE):
         raise GtlsError(rc, "gtls_sde")
     return raw, sde, summ.as_dict(), rc
+
+
+def gtls_search_sharded(t, y, dy, period_grid, duration_grid, tmpl, *, group=None, dt0: float = 0.05,
+                        sde_kernel: int = 151, _search=None, _sde=None, **kw) -> SearchResult:
+    """Period-sharded search over the ranks of a ``torch.distributed`` group (one process per GPU).
+
+    Trial periods are independent (the paper reports 1.75x on two GPUs), so
+    rank r searches periods r, r+W, r+2W, ... (interleaved: every rank gets the same mix of long and short
+    periods, i.e. of durations), the only exchange is ONE all-gather of 32 bytes per period (chi2 + the
+    24-byte best record), and every rank then runs the SR / SDE epilogue (``gtls_sde``) over the full
+    spectrum in grid order.  Every rank passes the same full arrays and gets the same full result.
+    ``_search`` / ``_sde`` replace the two library calls in the CPU (gloo) test of this plumbing."""
+    import torch
+    import torch.distributed as dist
+    search = _search or gtls_search
+    sde_fn = _sde or gtls_sde
+    world, rank = dist.get_world_size(group), dist.get_rank(group)
+    n_per = int(period_grid.shape[0])
+    per_period = duration_grid.ndim == 2
+    mine = slice(rank, n_per, world)
+    cont = (lambda a: a.contiguous()) if _is_torch(period_grid) else np.ascontiguousarray
+    res = search(t, y, dy, cont(period_grid[mine]), cont(duration_grid[mine]) if per_period else duration_grid,
+                 tmpl, dt0=dt0, sde_kernel=0, **kw)
+    # ---- one all-gather: [m, 4] doubles per rank = chi2 + the best record's 24 bytes, padded to m rows ----
+    m = (n_per + world - 1) // world
+    on_gpu = _is_torch(res.chi2)
+    comm_dev = res.chi2.device if (on_gpu and dist.get_backend(group) == "nccl") else torch.device("cpu")
+    as_t = (lambda a: a) if on_gpu else (lambda a: torch.from_numpy(np.ascontiguousarray(a)))
+    chi2_l = as_t(res.chi2).to(comm_dev)
+    best_l = as_t(res.best_raw).to(comm_dev).contiguous().view(torch.float64).reshape(-1, 3)
+    pack = torch.full((m, 4), float("inf"), dtype=torch.float64, device=comm_dev)
+    pack[: chi2_l.shape[0], 0] = chi2_l
+    pack[: chi2_l.shape[0], 1:] = best_l
+    parts = [torch.empty_like(pack) for _ in range(world)]
+    dist.all_gather(parts, pack, group=group)
+    gathered = torch.stack(parts)                                        # [world, m, 4]
+    nwin = torch.tensor([int(res.summary.get("windows_evaluated", 0))], dtype=torch.int64, device=comm_dev)
+    dist.all_reduce(nwin, group=group)
+    full = gathered.permute(1, 0, 2).reshape(world * m, 4)[:n_per]     # row i*W + r  <-  rank r's row i
+    chi2 = full[:, 0].contiguous()
+    best_raw = full[:, 1:].contiguous().view(torch.uint8).reshape(n_per, BEST_DTYPE.itemsize)
+    if on_gpu:
+        chi2, best_raw = chi2.to(res.chi2.device), best_raw.to(res.chi2.device)
+    else:
+        chi2, best_raw = chi2.numpy(), best_raw.numpy()
+    sde_raw, sde, summ, rc = sde_fn(chi2, sde_kernel=sde_kernel)
+    # the epilogue knows chi2 only: fill the best-period fields from the gathered records
+    ib = int(summ["best_period_idx"])
+    rec = (best_raw[ib].cpu().numpy() if _is_torch(best_raw) else best_raw[ib]).view(BEST_DTYPE)[0]
+    summ = dict(summ, best_period=float(period_grid[ib]), best_dur_idx=int(rec["dur_idx"]),
+                best_start=int(rec["start"]), best_depth=float(rec["depth"]), best_t0=float(rec["t0"]),
+                chi2_null=res.summary.get("chi2_null", 0.0), windows_evaluated=int(nwin.item()))
+    return SearchResult(chi2, sde_raw, sde, best_raw, summ, rc, None, [res])

@@ -423,3 +423,28 @@ def test_v1_kernel_still_matches(monkeypatch):
     ora = oracle.search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05)
     res = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05, sde_kernel=5)
     _check_search(w, res, ora, sde_kernel=5, label="v1")
+
+
+def test_period_sharded_helper_on_one_gpu():
+    """gtls_search_sharded with a one-rank NCCL group: the plumbing around the real library calls (device
+    tensors, pack / all-gather / unpack, gtls_sde on the gathered spectrum) reproduces gtls_search."""
+    _cuda()
+    import os
+    import torch
+    import torch.distributed as dist
+    w = gi.make_workload(2).subset(53)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    args = [dev(x) for x in (w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl)]
+    ref = g.gtls_search(*args, dt0=0.05, sde_kernel=31)
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    os.environ.setdefault("MASTER_PORT", str(33000 + os.getpid() % 2000))
+    dist.init_process_group("nccl", rank=0, world_size=1)
+    try:
+        res = g.gtls_search_sharded(*args, dt0=0.05, sde_kernel=31)
+    finally:
+        dist.destroy_process_group()
+    assert torch.equal(res.chi2, ref.chi2) and torch.equal(res.sde, ref.sde)
+    assert np.array_equal(res.best(), ref.best())
+    for k in ("best_period_idx", "best_period", "best_dur_idx", "best_start", "best_t0", "best_depth",
+              "sde_argmax", "windows_evaluated", "chi2_null"):
+        assert res.summary[k] == ref.summary[k], k
