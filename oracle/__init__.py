@@ -51,6 +51,14 @@ def lib():
         _lib.oracle_search.argtypes = [_dp, _dp, _dp, C.c_int64, _dp, C.c_int64, _dp, C.c_int32,
                                        C.c_int32, _dp, C.c_int32, C.c_double, C.c_int32, C.c_int32,
                                        _dp, C.c_void_p, _dp, _lp]
+        _lib.oracle_roche_fmax_hz.restype = C.c_double
+        _lib.oracle_roche_fmax_hz.argtypes = [C.c_double, C.c_double]
+        _lib.oracle_period_grid_size.restype = C.c_int64
+        _lib.oracle_period_grid_size.argtypes = [C.c_double] * 5
+        _lib.oracle_period_grid.restype = C.c_int64
+        _lib.oracle_period_grid.argtypes = [C.c_double] * 5 + [_dp, C.c_int64]
+        _lib.oracle_duration_grid.restype = None
+        _lib.oracle_duration_grid.argtypes = [_dp, C.c_int64, C.c_int32, C.c_double, C.c_double, C.c_double, _dp]
         _lib.oracle_sde.restype = C.c_int
         _lib.oracle_sde.argtypes = [_dp, C.c_int64, C.c_int32, _dp, _dp, _dp, _lp, _lp]
     return _lib
@@ -63,6 +71,32 @@ def _d(a):
 
 def num_threads() -> int:
     return int(lib().oracle_num_threads())
+
+
+def roche_fmax_hz(r_star: float = 1.0, m_star: float = 1.0) -> float:
+    """Eq. 3 (PAPER.md:92)."""
+    return float(lib().oracle_roche_fmax_hz(float(r_star), float(m_star)))
+
+
+def period_grid(span_days: float, r_star: float = 1.0, m_star: float = 1.0, oversampling: float = 3.0,
+                p_min_days: float = 0.0) -> np.ndarray:
+    """Ofir cubic frequency sampling, Eq. 1-6; periods in days, longest first."""
+    args = (float(span_days), float(r_star), float(m_star), float(oversampling), float(p_min_days))
+    n = int(lib().oracle_period_grid_size(*args))
+    out = np.empty(n, dtype=np.float64)
+    got = int(lib().oracle_period_grid(*args, out.ctypes.data_as(_dp), n))
+    assert got == n
+    return out
+
+
+def duration_grid(periods_days, n_dur: int, k_min: float = 20.05, k_max: float = 620.84,
+                  q_cap: float = 0.15) -> np.ndarray:
+    """[n_per, n_dur] fractions T14/P, Eq. 8-9 + cap, log-spaced (G12)."""
+    p, pp = _d(periods_days)
+    out = np.empty((p.size, int(n_dur)), dtype=np.float64)
+    lib().oracle_duration_grid(pp, p.size, int(n_dur), float(k_min), float(k_max), float(q_cap),
+                               out.ctypes.data_as(_dp))
+    return out
 
 
 def points_in_duration(q: float, n: int) -> int:

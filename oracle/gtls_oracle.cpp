@@ -19,7 +19,8 @@
 // P4 fold; P5 sort vs numpy stable argsort + constructed ties; P6 window sums vs cumsum;
 // P7 invariants; P8 template resampling; P9/P10 SDE vs closed forms / scipy median filter;
 // P11 stride example of PAPER.md:291; P13 noise-free folded-domain construction;
-// P14 top-K.  Parity unpinned: behaviour for n < 3 and D = n-1 (fixed only by this text).
+// P14 top-K; P12 grids (paper-printed f_max, N ~ 190 000, k values; S/2 first period).
+// Parity unpinned: behaviour for n < 3 and D = n-1 (fixed only by this text).
 // =====================================================================================
 #include <algorithm>
 #include <cmath>
@@ -355,6 +356,68 @@ int oracle_sde(const double* chi2, int64_t n_per, int32_t kernel, double* sr, do
     for (int64_t i = 1; i < n_per; ++i) if (sde[i] > sde[imax]) imax = i;
     *sde_argmax = imax;
     return 0;
+}
+
+// ---- Period and duration grids (paper section 2.2) ---------------
+// SI constants: CODATA G, IAU nominal solar mass / radius.  Span and periods are in days,
+// stellar radius and mass in solar units.
+static const double kG = 6.67430e-11, kMsun = 1.98847e30, kRsun = 6.957e8, kDay = 86400.0;
+
+// Eq. 3: f_max = 1/(2 pi) sqrt(G M / (3R)^3), Hz.
+double oracle_roche_fmax_hz(double r_star, double m_star) {
+    const double a_min = 3.0 * r_star * kRsun;
+    return std::sqrt(kG * m_star * kMsun / (a_min * a_min * a_min)) / (2.0 * M_PI);
+}
+
+// Eq. 1, 5, 6, reading G21: the S of Eq. 5 is the time span in seconds
+// and OS the oversampling factor.  p_min_days <= 0 takes f_max from Eq. 3.  Writes A, C, N.
+void oracle_ofir_constants(double span_days, double r_star, double m_star, double oversampling,
+                           double p_min_days, double* A, double* Cc, double* n_exact) {
+    const double S = span_days * kDay;
+    const double f_min = 2.0 / S;                                                       // Eq. 1
+    const double f_max = p_min_days > 0.0 ? 1.0 / (p_min_days * kDay) : oracle_roche_fmax_hz(r_star, m_star);
+    *A = std::pow(2.0 * M_PI, 2.0 / 3.0) / M_PI * (r_star * kRsun) / std::cbrt(kG * m_star * kMsun)
+         / (S * oversampling);                                                          // Eq. 5
+    *Cc = std::cbrt(f_min) - *A / 3.0;
+    *n_exact = (std::cbrt(f_max) - std::cbrt(f_min) + *A / 3.0) * 3.0 / *A;             // Eq. 6
+}
+
+// N = ceil(Eq. 6).
+int64_t oracle_period_grid_size(double span_days, double r_star, double m_star, double oversampling,
+                                double p_min_days) {
+    double A, Cc, n_exact;
+    oracle_ofir_constants(span_days, r_star, m_star, oversampling, p_min_days, &A, &Cc, &n_exact);
+    return (int64_t)std::ceil(n_exact);
+}
+
+// Eq. 4: f_i = (A/3 i + C)^3, i = 1..N; periods in days in ascending-frequency
+// order (the first is S/2 by Eq. 1, the last ~P_min).  Returns N.
+int64_t oracle_period_grid(double span_days, double r_star, double m_star, double oversampling,
+                           double p_min_days, double* out_periods, int64_t capacity) {
+    double A, Cc, n_exact;
+    oracle_ofir_constants(span_days, r_star, m_star, oversampling, p_min_days, &A, &Cc, &n_exact);
+    const int64_t N = (int64_t)std::ceil(n_exact);
+    for (int64_t i = 1; i <= N && i <= capacity; ++i) {
+        const double c = A / 3.0 * (double)i + Cc;
+        const double f = c * c * c;
+        out_periods[i - 1] = 1.0 / f / kDay;
+    }
+    return N;
+}
+
+// Eq. 8-9 with the cap of PAPER.md:159, reading G12: per period n_dur
+// fractions q = T14/P log-spaced from min(k_min P^(-2/3), cap) to min(k_max P^(-2/3), cap),
+// P in seconds; out[ip*n_dur + j].  n_dur = 1 gives the lower edge.
+void oracle_duration_grid(const double* periods_days, int64_t n_per, int32_t n_dur, double k_min,
+                          double k_max, double q_cap, double* out) {
+    for (int64_t ip = 0; ip < n_per; ++ip) {
+        const double scale = std::pow(periods_days[ip] * kDay, -2.0 / 3.0);
+        const double q_lo = std::min(k_min * scale, q_cap), q_hi = std::min(k_max * scale, q_cap);
+        for (int32_t j = 0; j < n_dur; ++j) {
+            const double x = n_dur > 1 ? (double)j / (double)(n_dur - 1) : 0.0;
+            out[ip * n_dur + j] = std::exp(std::log(q_lo) * (1.0 - x) + std::log(q_hi) * x);
+        }
+    }
 }
 
 }  // extern "C"

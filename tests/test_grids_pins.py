@@ -72,3 +72,56 @@ def test_template_shape():
     area = (p * p * k0 + k1 - 0.5 * math.sqrt(4 * z * z - (1 + z * z - p * p) ** 2)) / math.pi
     assert abs(gi.quad_ld_deficit([1.0], 0.1, 0.0, 0.0)[0] - area) < 1e-8
     assert abs(gi.quad_ld_deficit([0.3], 0.1, 0.0, 0.0)[0] - 0.01) < 1e-10
+
+
+# ---- the oracle's own grid functions (oracle/gtls_oracle.cpp), pinned to the paper's printed values,
+# ---- to closed forms / invariants, and to the independent numpy generators of gtls_inputs
+def test_oracle_fmax_and_count_match_paper():
+    import oracle
+    pin = PINS["f_max_hz_solar"]
+    assert abs(oracle.roche_fmax_hz() / pin["value"] - 1.0) < pin["rel_tol"]
+    p = oracle.period_grid(1500.0)                   # S = 1500 d, OS = 3 -> N ~ 190 000
+    pin = PINS["n_periods_1500d"]
+    assert abs(p.size / pin["value"] - 1.0) < pin["rel_tol"]
+    assert abs(p[0] - 750.0) < 1e-9                  # Eq. 1: P_max = S/2 exactly (C fixes f_1 = f_min)
+    assert abs(p[-1] - PINS["p_min_days_solar"]["value"]) < PINS["p_min_days_solar"]["abs_tol"]
+    assert p[-1] <= 1.0 / oracle.roche_fmax_hz() / 86400.0 * (1 + 1e-12)   # N = ceil: reaches f_max
+    assert np.all(np.diff(p) < 0)
+    d = np.diff((1.0 / p) ** (1.0 / 3.0))            # Eq. 4: f^(1/3) uniformly spaced
+    assert np.allclose(d, d[0], rtol=1e-6)
+
+
+def test_oracle_period_grid_scaling_and_oversampling():
+    import oracle
+    a = oracle.period_grid(90.0, p_min_days=0.5)
+    assert abs(a[0] - 45.0) < 1e-10 and a[-1] <= 0.5 * (1 + 1e-12) and a[-2] > 0.5
+    b = oracle.period_grid(90.0, oversampling=6.0, p_min_days=0.5)
+    assert abs((b.size - 1) / (a.size - 1) - 2.0) < 2e-3            # Eq. 5: A ~ 1/OS, Eq. 6: N ~ 1/A
+    # Eq. 5: A ~ R / M^(1/3); a star with R = 2, M = 8 has the same A as the Sun
+    c = oracle.period_grid(90.0, r_star=2.0, m_star=8.0, p_min_days=0.5)
+    assert c.size == a.size and np.allclose(c, a, rtol=1e-12)
+    # independent numpy implementation (gtls_inputs.grids)
+    assert a.size == gi.ofir_period_grid(90.0, p_min_days=0.5).size
+    assert np.allclose(a, gi.ofir_period_grid(90.0, p_min_days=0.5), rtol=1e-13, atol=0)
+
+
+def test_oracle_duration_grid():
+    import oracle
+    p = oracle.period_grid(90.0, p_min_days=0.5)
+    q = oracle.duration_grid(p, 25)
+    assert q.shape == (p.size, 25) and q.max() <= 0.15 * (1 + 1e-15)
+    ps = p * 86400.0
+    # Eq. 8-9 in the form T14 = k P^(1/3): lower edge in seconds, cube of it is linear in P
+    t14_lo = q[:, 0] * ps
+    free = q[:, 0] < 0.15 * (1 - 1e-12)
+    assert np.allclose(t14_lo[free] ** 3 / ps[free], PINS["k_min_gtls"]["value"] ** 3, rtol=1e-12)
+    capped = q[:, -1] >= 0.15 * (1 - 1e-12)
+    assert capped.any() and (~capped).any()
+    assert np.allclose((q[~capped, -1] * ps[~capped]) ** 3 / ps[~capped], PINS["k_max_gtls"]["value"] ** 3, rtol=1e-12)
+    r = q[:, 1:] / q[:, :-1]
+    assert np.allclose(r, r[:, :1], rtol=1e-12)                      # log spacing
+    assert np.allclose(q, gi.duration_grid(p, 25), rtol=1e-13, atol=0)
+    assert np.allclose(oracle.duration_grid(p[:5], 1)[:, 0], q[:5, 0], rtol=1e-15)
+    # TLS constants with the TLS cap
+    qt = oracle.duration_grid(p, 10, 41.39, 546.94, 0.112)
+    assert qt.max() <= 0.112 * (1 + 1e-15) and np.all(qt[:, 0] >= q[:, 0])
