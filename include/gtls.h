@@ -203,6 +203,51 @@ int64_t gtls_window_chi2(const double* t, const double* y, const double* dy, int
 int gtls_sde(const double* chi2, int64_t n_per, const gtls_opts* opts,
              double* out_sde_raw, double* out_sde, gtls_summary* out_summary);
 
+/* ---- Trial grids built on the device (paper section 2.2) ------------------------------------------
+ * Period grid: Ofir (2014) cubic frequency sampling, f_i = (A/3 i + C)^3, i = 1..N (Eq. 4)
+ * with f_min = 2/S (Eq. 1), A of Eq. 5 (reading G21: its S is the time span in seconds, OS the
+ * oversampling factor), C = f_min^(1/3) - A/3 and N = ceil(Eq. 6).  span and p_min in days, r_star and
+ * m_star in solar units; p_min <= 0 takes f_max from the Roche limit (Eq. 3).  Periods come
+ * out in days in ascending-frequency order (first = span/2, last ~ p_min).
+ * gtls_period_grid_size returns N (>= 1) or a negative error code (GTLS_EINVAL: a parameter <= 0 or not
+ * finite; GTLS_EGRID: f_max <= f_min, or N above 2^31).  gtls_period_grid writes out_periods[n_per]
+ * (host or device per opts->pointers_on_device); n_per must equal gtls_period_grid_size(...). */
+int64_t gtls_period_grid_size(double span, double r_star, double m_star, double oversampling, double p_min);
+int gtls_period_grid(double span, double r_star, double m_star, double oversampling, double p_min,
+                     const gtls_opts* opts, double* out_periods, int64_t n_per);
+
+/* Duration grid: for every period n_dur fractions q = T14/P, log-spaced from min(k_min P^(-2/3), q_cap)
+ * to min(k_max P^(-2/3), q_cap) with P in seconds (Eq. 8-9; cap PAPER.md:159; reading
+ * G12).  GTLS defaults: k_min 20.05, k_max 620.84 s^(2/3), q_cap 0.15.  periods [n_per] in days (host or
+ * device like the output), out_durations [n_per][n_dur] (the dur_per_period = 1 layout of gtls_search).
+ * n_dur = 1 gives the lower edge.  GTLS_EINVAL: k_min <= 0, k_max < k_min, q_cap outside (0, 0.5];
+ * GTLS_EGRID: a period <= 0 or not finite (its row is NaN). */
+int gtls_duration_grid(const double* periods, int64_t n_per, int32_t n_dur, double k_min, double k_max,
+                       double q_cap, const gtls_opts* opts, double* out_durations);
+
+/* ---- Survey mode: many independent light curves in one call (BASELINE.json config 5) -----------------
+ * Curve c is t/y/dy[curve_offset[c] .. curve_offset[c+1]) with its own period grid
+ * period_grid[period_offset[c] .. period_offset[c+1]); duration_grid is [n_dur] shared by everything
+ * (opts->dur_per_period = 0) or [period_offset[n_curves]][n_dur], rows in the order of period_grid
+ * (dur_per_period = 1).  The offset arrays are HOST arrays of n_curves + 1 ascending entries starting at
+ * 0; every other array is host or device per opts->pointers_on_device.  Outputs are concatenated in the
+ * same order as period_grid: out_chi2 [total periods] (required), out_best / out_sde_raw / out_sde (may
+ * be NULL); out_summary [n_curves] and out_status [n_curves] are HOST arrays and may be NULL.
+ * Each curve is one gtls_search (same options, same results bit for bit); the curves run concurrently
+ * on a few internal streams (ordered after opts->stream at entry, joined before return), each stream
+ * with its own slice of the scratch: opts->workspace, when given, must hold
+ * gtls_batch_workspace_bytes(...).  The call returns after all curves have finished.
+ * Return: GTLS_OK when every curve returned GTLS_OK or GTLS_EDEGENERATE (see out_status), else the
+ * error code of the first failing curve; curves after a failure are still searched. */
+int gtls_search_batch(int32_t n_curves, const double* t, const double* y, const double* dy,
+                      const int64_t* curve_offset, const double* period_grid,
+                      const int64_t* period_offset, const double* duration_grid, int32_t n_dur,
+                      const double* tmpl, int32_t n_tmpl, const gtls_opts* opts,
+                      double* out_chi2, gtls_best* out_best, double* out_sde_raw, double* out_sde,
+                      gtls_summary* out_summary, int32_t* out_status);
+size_t gtls_batch_workspace_bytes(int32_t n_curves, const int64_t* curve_offset,
+                                  const int64_t* period_offset, int32_t n_dur, const gtls_opts* opts);
+
 /* Device scratch needed by gtls_search for these sizes and options (tile = opts->period_tile
  * or the automatic choice).  Pass a buffer of at least this size in opts->workspace to avoid
  * allocation inside the call. */

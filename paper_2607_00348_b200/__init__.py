@@ -20,7 +20,8 @@ from typing import Any, Optional
 
 import numpy as np
 
-__all__ = ["gtls_search", "gtls_search_two_stage", "gtls_search_sharded", "gtls_fold_sort", "gtls_fold_scan", "gtls_window_chi2", "gtls_sde",
+__all__ = ["gtls_search", "gtls_search_two_stage", "gtls_search_batch", "gtls_batch_workspace_bytes",
+           "gtls_period_grid_size", "gtls_period_grid", "gtls_duration_grid", "BatchResult", "gtls_search_sharded", "gtls_fold_sort", "gtls_fold_scan", "gtls_window_chi2", "gtls_sde",
            "gtls_workspace_bytes", "gtls_strerror", "gtls_version", "GtlsError", "SearchResult",
            "BEST_DTYPE", "lib_path", "load_library"]
 
@@ -112,6 +113,18 @@ def load_library():
     lib.gtls_window_chi2.restype = C.c_int64
     lib.gtls_sde.argtypes = [dp, C.c_int64, C.POINTER(GtlsOpts), dp, dp, C.POINTER(GtlsSummary)]
     lib.gtls_sde.restype = C.c_int
+    lib.gtls_period_grid_size.argtypes = [C.c_double] * 5
+    lib.gtls_period_grid_size.restype = C.c_int64
+    lib.gtls_period_grid.argtypes = [C.c_double] * 5 + [C.POINTER(GtlsOpts), dp, C.c_int64]
+    lib.gtls_period_grid.restype = C.c_int
+    lib.gtls_duration_grid.argtypes = [dp, C.c_int64, C.c_int32, C.c_double, C.c_double, C.c_double,
+                                       C.POINTER(GtlsOpts), dp]
+    lib.gtls_duration_grid.restype = C.c_int
+    lib.gtls_search_batch.argtypes = [C.c_int32, dp, dp, dp, vp, dp, vp, dp, C.c_int32, dp, C.c_int32,
+                                      C.POINTER(GtlsOpts), dp, vp, dp, dp, vp, vp]
+    lib.gtls_search_batch.restype = C.c_int
+    lib.gtls_batch_workspace_bytes.argtypes = [C.c_int32, vp, vp, C.c_int32, C.POINTER(GtlsOpts)]
+    lib.gtls_batch_workspace_bytes.restype = C.c_size_t
     lib.gtls_workspace_bytes.argtypes = [C.c_int64, C.c_int64, C.c_int32, C.POINTER(GtlsOpts)]
     lib.gtls_workspace_bytes.restype = C.c_size_t
     lib.gtls_strerror.argtypes = [C.c_int]
@@ -247,6 +260,130 @@ def gtls_search(t, y, dy, period_grid, duration_grid, tmpl, *, dt0: float = 0.05
         raise GtlsError(rc, "gtls_search")
     return SearchResult(chi2, sde_raw, sde, best, summ.as_dict(), rc,
                         st.as_dict() if stats else None, [kt, ky, kd, kp, kq, km])
+
+
+def gtls_period_grid_size(span: float, r_star: float = 1.0, m_star: float = 1.0, oversampling: float = 3.0,
+                          p_min: float = 0.0) -> int:
+    """N = ceil(Eq. 6) of the Ofir period grid (``gtls_period_grid_size`` in include/gtls.h)."""
+    n = int(load_library().gtls_period_grid_size(float(span), float(r_star), float(m_star),
+                                                  float(oversampling), float(p_min)))
+    if n < 0:
+        raise GtlsError(n, "gtls_period_grid_size")
+    return n
+
+
+def gtls_period_grid(span: float, r_star: float = 1.0, m_star: float = 1.0, oversampling: float = 3.0,
+                     p_min: float = 0.0, *, device=None, stream=None):
+    """Ofir period grid (Eq. 1-6) built on the device.  ``device`` = a torch CUDA device: the result is
+    a CUDA tensor; ``None``: a numpy array (the library copies it back)."""
+    lib = load_library()
+    args = (float(span), float(r_star), float(m_star), float(oversampling), float(p_min))
+    n = gtls_period_grid_size(*args)
+    if device is not None:
+        import torch
+        out = torch.empty(n, dtype=torch.float64, device=device)
+        o = _opts(True, out, stream)
+    else:
+        out = np.empty(n, dtype=np.float64)
+        o = _opts(False)
+    rc = lib.gtls_period_grid(*args, C.byref(o), _ptr(out), n)
+    if rc != GTLS_OK:
+        raise GtlsError(rc, "gtls_period_grid")
+    return out
+
+
+def gtls_duration_grid(periods, n_dur: int, k_min: float = 20.05, k_max: float = 620.84,
+                       q_cap: float = 0.15, *, stream=None):
+    """[n_per, n_dur] duration fractions T14/P (Eq. 8-9 + cap, reading G12) built on the device."""
+    lib = load_library()
+    kp, pp, dev = _prep(periods)
+    n_per = int(kp.shape[0])
+    out = _empty((n_per, int(n_dur)), kp)
+    o = _opts(dev, kp, stream)
+    rc = lib.gtls_duration_grid(pp, n_per, int(n_dur), float(k_min), float(k_max), float(q_cap),
+                                C.byref(o), _ptr(out))
+    if rc != GTLS_OK:
+        raise GtlsError(rc, "gtls_duration_grid")
+    return out
+
+
+@dataclass
+class BatchResult:
+    chi2: Any                      # [total periods], curve after curve
+    sde_raw: Any
+    sde: Any
+    best_raw: Any                  # [total periods, 24] bytes
+    period_offset: np.ndarray      # [n_curves + 1]
+    summaries: list                # one dict per curve
+    status: np.ndarray             # [n_curves] int32: GTLS_OK / GTLS_EDEGENERATE per curve
+    _keep: list = field(default_factory=list, repr=False)
+
+    def best(self) -> np.ndarray:
+        raw = self.best_raw.cpu().numpy() if _is_torch(self.best_raw) else self.best_raw
+        return np.ascontiguousarray(raw).view(BEST_DTYPE).reshape(-1)
+
+
+def _offsets(x, name: str) -> np.ndarray:
+    a = np.ascontiguousarray(np.asarray(x.cpu() if _is_torch(x) else x), dtype=np.int64)
+    if a.ndim != 1 or a.size < 2:
+        raise ValueError(f"{name} must hold n_curves + 1 entries")
+    return a
+
+
+def gtls_batch_workspace_bytes(curve_offset, period_offset, n_dur: int, period_tile: int = 0) -> int:
+    co, po = _offsets(curve_offset, "curve_offset"), _offsets(period_offset, "period_offset")
+    o = GtlsOpts()
+    lib = load_library()
+    lib.gtls_opts_default(C.byref(o))
+    o.period_tile = int(period_tile)
+    return int(lib.gtls_batch_workspace_bytes(co.size - 1, co.ctypes.data, po.ctypes.data, int(n_dur), C.byref(o)))
+
+
+def gtls_search_batch(t, y, dy, curve_offset, period_grid, period_offset, duration_grid, tmpl, *,
+                      dt0: float = 0.05, sde_kernel: int = 151, top_k: int = 0, chi2_fp32: int = 0,
+                      period_tile: int = 0, workspace=None, stream=None) -> BatchResult:
+    """Survey mode (``gtls_search_batch`` in include/gtls.h): concatenated light curves and period
+    grids with host offset arrays; ``duration_grid`` is [n_dur] (shared) or [total periods, n_dur]."""
+    lib = load_library()
+    co, po = _offsets(curve_offset, "curve_offset"), _offsets(period_offset, "period_offset")
+    if co.size != po.size:
+        raise ValueError("curve_offset and period_offset must have the same length")
+    n_curves = co.size - 1
+    kt, pt, dev = _prep(t)
+    ky, py, d2 = _prep(y)
+    kd, pd, d3 = _prep(dy)
+    kp, pp, d4 = _prep(period_grid)
+    kq, pq, d5 = _prep(duration_grid)
+    km, pm, d6 = _prep(tmpl)
+    if len({dev, d2, d3, d4, d5, d6}) != 1:
+        raise ValueError("all arrays must be either CUDA tensors or host arrays")
+    if int(kt.shape[0]) != int(co[-1]) or int(kp.shape[0]) != int(po[-1]):
+        raise ValueError("offsets do not match the array lengths")
+    per_total, n_tmpl = int(po[-1]), int(km.shape[0])
+    per_period = 1 if kq.ndim == 2 else 0
+    n_dur = int(kq.shape[-1])
+    if per_period and int(kq.shape[0]) != per_total:
+        raise ValueError("duration_grid rows must match period_grid")
+    o = _opts(dev, kt, stream, dt0=float(dt0), sde_kernel=int(sde_kernel), top_k=int(top_k),
+              chi2_fp32=int(chi2_fp32), dur_per_period=per_period, period_tile=int(period_tile))
+    if workspace is not None:
+        if not (_is_torch(workspace) and workspace.is_cuda):
+            raise ValueError("workspace must be a CUDA uint8 tensor")
+        o.workspace = workspace.data_ptr()
+        o.workspace_bytes = workspace.numel() * workspace.element_size()
+    chi2 = _empty((per_total,), kt)
+    sde_raw = _empty((per_total,), kt)
+    sde = _empty((per_total,), kt)
+    best = _empty((per_total, BEST_DTYPE.itemsize), kt, np.uint8)
+    summ = (GtlsSummary * n_curves)()
+    status = np.zeros(n_curves, dtype=np.int32)
+    rc = lib.gtls_search_batch(n_curves, pt, py, pd, co.ctypes.data, pp, po.ctypes.data, pq, n_dur, pm, n_tmpl,
+                               C.byref(o), _ptr(chi2), _ptr(best), _ptr(sde_raw), _ptr(sde),
+                               C.cast(summ, C.c_void_p), status.ctypes.data)
+    if rc != GTLS_OK:
+        raise GtlsError(rc, "gtls_search_batch")
+    return BatchResult(chi2, sde_raw, sde, best, po, [s_.as_dict() for s_ in summ], status,
+                       [kt, ky, kd, kp, kq, km])
 
 
 def gtls_search_two_stage(t, y, dy, period_grid, duration_grid, tmpl, *, dt0: float = 0.05,

@@ -4,7 +4,9 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <cmath>
 #include <new>
+#include <thread>
 #include <vector>
 
 #include "gtls_internal.cuh"
@@ -64,6 +66,7 @@ Sizes workspace_sizes(long long n, long long n_per, int n_dur, double q_max, boo
     s.fixed = 3 * align_up(n * sizeof(double)) + align_up(sizeof(CurveInfo)) +
               align_up(sizeof(SdeScratch)) + align_up(2 * sizeof(unsigned long long)) +
               2 * align_up(n_per * sizeof(double)) + align_up(n_per * sizeof(gtls_best)) + 4096 +
+              align_up((size_t)kChi2Variants * (1 + kBinBlocks) * sizeof(int)) +
               align_up(2 * (size_t)(pitch - n + 2) * sizeof(double));       // gtab: D <= pitch - n
     s.per_period = 2 * n * sizeof(u64) + 256ull * nt * sizeof(u32) + n_dur * sizeof(DurEntry) +
                    n_dur * sizeof(Partial) + (size_t)kChi2Variants * n_dur * sizeof(int) +
@@ -173,6 +176,11 @@ SideStream* gtls::side_stream(int which) {
             if (cudaEventCreateWithFlags(&ss.fork, cudaEventDisableTiming) != cudaSuccess) return;
             if (cudaEventCreateWithFlags(&ss.join, cudaEventDisableTiming) != cudaSuccess) return;
             ok = true;
+        }
+        ~Slot() {     // worker threads of gtls_search_batch end after every call
+            if (ss.s) cudaStreamDestroy(ss.s);
+            if (ss.fork) cudaEventDestroy(ss.fork);
+            if (ss.join) cudaEventDestroy(ss.join);
         }
     };
     static const bool enabled = [] { const char* e = getenv("GTLS_STREAMS"); return !(e && atoi(e) == 0); }();
@@ -419,7 +427,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     a.gtab = gtab_dev; a.gtab_max = gtab_max;
     a.partial = ws.take<Partial>((size_t)tile * n_dur);
     a.trial_list = ws.take<int>((size_t)kChi2Variants * tile * n_dur);
-    a.trial_count = ws.take<int>(kChi2Variants);
+    a.trial_count = ws.take<int>((size_t)kChi2Variants * (1 + kBinBlocks));   // totals, then the per-CTA counts of k_bin_trials
     a.x1 = ws.take<double>((size_t)tile * a.pitch);
     a.s1 = ws.take<double>((size_t)tile * a.spitch);
     if (!uniform) {
@@ -453,7 +461,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
         tm.mark(5);
         launch_reduce(a, d_chi2, d_best, d_counters, st);
         tm.mark(6);
-        stats.kernel_launches += launches + 2 + ((use_v1 || use_rows || a.top_k > 0) ? 1 : 1 + (uniform ? kChi2Variants - 1 : kChi2Variants - 3));
+        stats.kernel_launches += launches + 2 + ((use_v1 || use_rows || a.top_k > 0) ? 1 : 2 + (uniform ? kChi2Variants - 1 : kChi2Variants - 3));   // k_bin_trials is two launches
         stats.chi2_launches += 1;
         if (o.stats) {
             CU(cudaStreamSynchronize(st));
@@ -822,6 +830,244 @@ int gtls_search_two_stage(const double* t, const double* y, const double* dy, in
     CU(cudaStreamSynchronize(st));
     CU(cudaGetLastError());
     return rc_final;
+}
+
+}  // extern "C"
+
+// ---- trial grids on the device (paper section 2.2) --------------------------------------------------
+namespace {
+// SI constants: CODATA G, IAU nominal solar mass and radius.
+constexpr double kGrav = 6.67430e-11, kMassSun = 1.98847e30, kRadiusSun = 6.957e8, kDaySeconds = 86400.0;
+constexpr double kPi = 3.14159265358979323846;
+
+// A/3, C and the real-valued N of Eq. 4-6.  Returns a gtls error code.
+int ofir_constants(double span, double r_star, double m_star, double oversampling, double p_min,
+                   double* a3, double* c, double* n_exact) {
+    if (!(span > 0.0) || !(r_star > 0.0) || !(m_star > 0.0) || !(oversampling > 0.0) ||
+        std::isinf(span) || std::isinf(r_star) || std::isinf(m_star) || std::isinf(oversampling) ||
+        std::isnan(p_min) || std::isinf(p_min)) return GTLS_EINVAL;
+    const double S = span * kDaySeconds;
+    const double gm = kGrav * m_star * kMassSun;
+    const double f_min = 2.0 / S;                                                          // Eq. 1
+    double f_max;
+    if (p_min > 0.0) f_max = 1.0 / (p_min * kDaySeconds);
+    else { const double a_min = 3.0 * r_star * kRadiusSun; f_max = std::sqrt(gm / (a_min * a_min * a_min)) / (2.0 * kPi); }  // Eq. 3
+    if (!(f_max > f_min)) return GTLS_EGRID;
+    const double A = std::pow(2.0 * kPi, 2.0 / 3.0) / kPi * (r_star * kRadiusSun) / std::pow(gm, 1.0 / 3.0)
+                     / (S * oversampling);                                                 // Eq. 5
+    const double cf_min = std::pow(f_min, 1.0 / 3.0);
+    *a3 = A / 3.0;
+    *c = cf_min - A / 3.0;
+    *n_exact = (std::pow(f_max, 1.0 / 3.0) - cf_min + A / 3.0) * 3.0 / A;                  // Eq. 6
+    if (!(*n_exact >= 0.0) || *n_exact > 2147483647.0) return GTLS_EGRID;
+    return GTLS_OK;
+}
+
+int batch_lanes(int n_curves) {
+    static const int env = [] { const char* e = getenv("GTLS_BATCH_LANES"); return e ? atoi(e) : 0; }();
+    int lanes = env > 0 ? env : 4;
+    if (lanes > 16) lanes = 16;
+    return lanes < n_curves ? lanes : (n_curves < 1 ? 1 : n_curves);
+}
+
+// scratch of one lane: the largest gtls_workspace_bytes over the curves
+size_t batch_lane_bytes(int32_t n_curves, const int64_t* co, const int64_t* po, int32_t n_dur, const gtls_opts* o) {
+    size_t m = 0;
+    for (int c = 0; c < n_curves; ++c) {
+        const size_t b = gtls_workspace_bytes(co[c + 1] - co[c], po[c + 1] - po[c], n_dur, o);
+        if (b > m) m = b;
+    }
+    return align_up(m);
+}
+}  // namespace
+
+extern "C" {
+
+int64_t gtls_period_grid_size(double span, double r_star, double m_star, double oversampling, double p_min) {
+    double a3, c, n_exact;
+    const int rc = ofir_constants(span, r_star, m_star, oversampling, p_min, &a3, &c, &n_exact);
+    if (rc) return rc;
+    const int64_t n = (int64_t)std::ceil(n_exact);
+    return n < 1 ? GTLS_EGRID : n;
+}
+
+int gtls_period_grid(double span, double r_star, double m_star, double oversampling, double p_min,
+                     const gtls_opts* opts, double* out_periods, int64_t n_per) {
+    g_cuda_err[0] = 0;
+    const gtls_opts o = resolve_opts(opts);
+    double a3, c, n_exact;
+    const int rc0 = ofir_constants(span, r_star, m_star, oversampling, p_min, &a3, &c, &n_exact);
+    if (rc0) return rc0;
+    if (!out_periods || n_per < 1 || n_per != (int64_t)std::ceil(n_exact)) return GTLS_EINVAL;
+    CU(cudaSetDevice(o.device));
+    cudaStream_t st = (cudaStream_t)o.stream;
+    if (o.pointers_on_device) {
+        launch_period_grid(a3, c, n_per, out_periods, st);
+        CU(cudaGetLastError());
+        return GTLS_OK;
+    }
+    Arena ar;
+    int rc = alloc_arena(ar, align_up(n_per * 8) + 256);
+    if (rc) return rc;
+    double* d = ar.take<double>(n_per);
+    launch_period_grid(a3, c, n_per, d, st);
+    CU(cudaMemcpyAsync(out_periods, d, n_per * 8, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    CU(cudaGetLastError());
+    return GTLS_OK;
+}
+
+int gtls_duration_grid(const double* periods, int64_t n_per, int32_t n_dur, double k_min, double k_max,
+                       double q_cap, const gtls_opts* opts, double* out_durations) {
+    g_cuda_err[0] = 0;
+    const gtls_opts o = resolve_opts(opts);
+    if (!periods || !out_durations || n_per < 1 || n_dur < 1 || n_dur > 4096) return GTLS_EINVAL;
+    if (!(k_min > 0.0) || !(k_max >= k_min) || std::isinf(k_max) || !(q_cap > 0.0) || !(q_cap <= 0.5)) return GTLS_EINVAL;
+    CU(cudaSetDevice(o.device));
+    cudaStream_t st = (cudaStream_t)o.stream;
+    const bool dev = o.pointers_on_device != 0;
+    const size_t total = (size_t)n_per * n_dur;
+    Arena ar;
+    int rc = alloc_arena(ar, dev ? 512 : align_up(n_per * 8) + align_up(total * 8) + 1024);
+    if (rc) return rc;
+    const double* d_per;
+    if ((rc = stage_in(periods, n_per, dev, ar, st, &d_per))) return rc;
+    double* d_out = dev ? out_durations : ar.take<double>(total);
+    int* d_bad = ar.take<int>(1);
+    if (!d_bad) return GTLS_ENOMEM;
+    CU(cudaMemsetAsync(d_bad, 0, sizeof(int), st));
+    launch_duration_grid(d_per, n_per, n_dur, k_min, k_max, q_cap, d_out, d_bad, st);
+    int bad = 0;
+    CU(cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+    if (!dev) CU(cudaMemcpyAsync(out_durations, d_out, total * 8, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    CU(cudaGetLastError());
+    return bad ? GTLS_EGRID : GTLS_OK;
+}
+
+size_t gtls_batch_workspace_bytes(int32_t n_curves, const int64_t* curve_offset,
+                                  const int64_t* period_offset, int32_t n_dur, const gtls_opts* opts) {
+    if (n_curves < 1 || !curve_offset || !period_offset) return 0;
+    const gtls_opts o = resolve_opts(opts);
+    const size_t lane = batch_lane_bytes(n_curves, curve_offset, period_offset, n_dur, &o);
+    return lane ? (size_t)batch_lanes(n_curves) * lane + 256 : 0;
+}
+
+int gtls_search_batch(int32_t n_curves, const double* t, const double* y, const double* dy,
+                      const int64_t* curve_offset, const double* period_grid,
+                      const int64_t* period_offset, const double* duration_grid, int32_t n_dur,
+                      const double* tmpl, int32_t n_tmpl, const gtls_opts* opts,
+                      double* out_chi2, gtls_best* out_best, double* out_sde_raw, double* out_sde,
+                      gtls_summary* out_summary, int32_t* out_status) {
+    g_cuda_err[0] = 0;
+    const gtls_opts o = resolve_opts(opts);
+    if (n_curves < 1 || !t || !y || !dy || !curve_offset || !period_grid || !period_offset ||
+        !duration_grid || !tmpl || !out_chi2 || n_dur < 1 || n_tmpl < 2) return GTLS_EINVAL;
+    if (curve_offset[0] != 0 || period_offset[0] != 0) return GTLS_EINVAL;
+    for (int c = 0; c < n_curves; ++c)
+        if (curve_offset[c + 1] - curve_offset[c] < 3 || period_offset[c + 1] - period_offset[c] < 1) return GTLS_EINVAL;
+    const int64_t n_total = curve_offset[n_curves], per_total = period_offset[n_curves];
+    CU(cudaSetDevice(o.device));
+    cudaStream_t st = (cudaStream_t)o.stream;
+    const bool dev = o.pointers_on_device != 0;
+    const int64_t durs_total = o.dur_per_period ? per_total * (int64_t)n_dur : n_dur;
+
+    // host mode: everything is staged once; the curves then run on device pointers
+    Arena io;
+    if (!dev) {
+        const size_t bytes = 3 * align_up(n_total * 8) + align_up(per_total * 8) + align_up(durs_total * 8) +
+                             align_up(n_tmpl * 8) + 3 * align_up(per_total * 8) +
+                             align_up(per_total * sizeof(gtls_best)) + 16 * 256;
+        int rc = alloc_arena(io, bytes);
+        if (rc) return rc;
+    }
+    const double *d_t, *d_y, *d_dy, *d_per, *d_dur, *d_tmpl;
+    int rc;
+    if ((rc = stage_in(t, n_total, dev, io, st, &d_t))) return rc;
+    if ((rc = stage_in(y, n_total, dev, io, st, &d_y))) return rc;
+    if ((rc = stage_in(dy, n_total, dev, io, st, &d_dy))) return rc;
+    if ((rc = stage_in(period_grid, per_total, dev, io, st, &d_per))) return rc;
+    if ((rc = stage_in(duration_grid, durs_total, dev, io, st, &d_dur))) return rc;
+    if ((rc = stage_in(tmpl, n_tmpl, dev, io, st, &d_tmpl))) return rc;
+    double* d_chi2 = dev ? out_chi2 : io.take<double>(per_total);
+    gtls_best* d_best = dev ? out_best : (out_best ? io.take<gtls_best>(per_total) : nullptr);
+    double* d_raw = dev ? out_sde_raw : (out_sde_raw ? io.take<double>(per_total) : nullptr);
+    double* d_sde = dev ? out_sde : (out_sde ? io.take<double>(per_total) : nullptr);
+    if (!d_chi2 || (out_best && !d_best) || (out_sde_raw && !d_raw) || (out_sde && !d_sde)) return GTLS_ENOMEM;
+
+    // scratch: one slice per lane
+    const int lanes = batch_lanes(n_curves);
+    gtls_opts sized = o;                      // the per-curve tile choice without the caller's scratch
+    sized.workspace = nullptr; sized.workspace_bytes = 0;
+    size_t lane_bytes = batch_lane_bytes(n_curves, curve_offset, period_offset, n_dur, &sized);
+    if (!lane_bytes) return GTLS_EINVAL;
+    Arena ws;
+    if (o.workspace) {
+        if (((uintptr_t)o.workspace & 255) != 0) return GTLS_EINVAL;
+        if (o.workspace_bytes < (size_t)lanes * lane_bytes) return GTLS_ENOMEM;
+        ws.base = (char*)o.workspace; ws.size = o.workspace_bytes; ws.owned = false;
+    } else {
+        size_t free_b = 0, total_b = 0;
+        if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && (size_t)lanes * lane_bytes > free_b / 2)
+            lane_bytes = (free_b / 2 / lanes) & ~(size_t)255;      // gtls_search shrinks its tile to fit
+        if ((rc = alloc_arena(ws, (size_t)lanes * lane_bytes + 256))) return rc;
+    }
+
+    cudaEvent_t ev_in = nullptr;
+    CU(cudaEventCreateWithFlags(&ev_in, cudaEventDisableTiming));
+    CU(cudaEventRecord(ev_in, st));
+    std::vector<int> status((size_t)n_curves, GTLS_OK);
+    std::vector<cudaEvent_t> ev_done((size_t)lanes, nullptr);
+    std::vector<int> lane_rc((size_t)lanes, GTLS_OK);
+    std::vector<std::thread> workers;
+    for (int lane = 0; lane < lanes; ++lane) {
+        workers.emplace_back([&, lane]() {
+            cudaStream_t ls = nullptr;
+            if (cudaSetDevice(o.device) != cudaSuccess ||
+                cudaStreamCreateWithFlags(&ls, cudaStreamNonBlocking) != cudaSuccess ||
+                cudaEventCreateWithFlags(&ev_done[lane], cudaEventDisableTiming) != cudaSuccess ||
+                cudaStreamWaitEvent(ls, ev_in, 0) != cudaSuccess) {
+                lane_rc[lane] = GTLS_ECUDA;
+                for (int c = lane; c < n_curves; c += lanes) status[c] = GTLS_ECUDA;
+                if (ls) cudaStreamDestroy(ls);
+                return;
+            }
+            gtls_opts lo = o;
+            lo.pointers_on_device = 1;
+            lo.stream = (void*)ls;
+            lo.workspace = ws.base + (size_t)lane * lane_bytes;
+            lo.workspace_bytes = lane_bytes;
+            lo.stats = nullptr;
+            for (int c = lane; c < n_curves; c += lanes) {
+                const int64_t c0 = curve_offset[c], p0 = period_offset[c];
+                status[c] = gtls_search(d_t + c0, d_y + c0, d_dy + c0, curve_offset[c + 1] - c0,
+                                        d_per + p0, period_offset[c + 1] - p0,
+                                        o.dur_per_period ? d_dur + p0 * n_dur : d_dur, n_dur, d_tmpl, n_tmpl, &lo,
+                                        d_chi2 + p0, d_best ? d_best + p0 : nullptr, d_raw ? d_raw + p0 : nullptr,
+                                        d_sde ? d_sde + p0 : nullptr, out_summary ? out_summary + c : nullptr);
+            }
+            cudaEventRecord(ev_done[lane], ls);
+            cudaStreamSynchronize(ls);
+            cudaStreamDestroy(ls);
+        });
+    }
+    for (auto& w : workers) w.join();
+    for (int lane = 0; lane < lanes; ++lane)
+        if (ev_done[lane]) { cudaStreamWaitEvent(st, ev_done[lane], 0); cudaEventDestroy(ev_done[lane]); }
+    cudaEventDestroy(ev_in);
+    int first = GTLS_OK;
+    for (int c = 0; c < n_curves; ++c) {
+        if (out_status) out_status[c] = status[c];
+        if (first == GTLS_OK && status[c] != GTLS_OK && status[c] != GTLS_EDEGENERATE) first = status[c];
+    }
+    if (!dev) {
+        CU(cudaMemcpyAsync(out_chi2, d_chi2, per_total * sizeof(double), cudaMemcpyDeviceToHost, st));
+        if (out_best) CU(cudaMemcpyAsync(out_best, d_best, per_total * sizeof(gtls_best), cudaMemcpyDeviceToHost, st));
+        if (out_sde_raw) CU(cudaMemcpyAsync(out_sde_raw, d_raw, per_total * sizeof(double), cudaMemcpyDeviceToHost, st));
+        if (out_sde) CU(cudaMemcpyAsync(out_sde, d_sde, per_total * sizeof(double), cudaMemcpyDeviceToHost, st));
+    }
+    CU(cudaStreamSynchronize(st));
+    return first;
 }
 
 }  // extern "C"

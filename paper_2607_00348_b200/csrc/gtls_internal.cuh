@@ -43,6 +43,7 @@ struct CurveInfo {
 // chi2 ring kernel variants: ring size index (0..5 = 24, 21, 16, 12, 8, 4 taps) + 6 * narrow
 constexpr int kChi2Rings = 6;
 constexpr int kChi2Variants = 2 * kChi2Rings;
+constexpr int kBinBlocks = 148;      // CTAs of k_bin_trials; trial_count holds kChi2Variants * (1 + kBinBlocks) ints
 constexpr int kChi2NarrowMax = 16;   // largest class stride handled by the narrow variants
 // Window classes of a trial with M = ceil(D/stride) taps: the smallest count that leaves at most 24 taps
 // per class when the class stride stays narrow (<= kChi2NarrowMax), at most 21 otherwise and when the
@@ -157,7 +158,7 @@ struct TileArgs {
     const int* seg_list;   // LSD path: periods (tile-local) to process, or nullptr = all of the tile
     const int* seg_count;  // number of entries of seg_list (device)
     int* trial_list;       // [kChi2Variants][tile*n_dur] trial indices binned by chi2 kernel variant
-    int* trial_count;      // [kChi2Variants]
+    int* trial_count;      // [kChi2Variants] totals + [kBinBlocks][kChi2Variants] per-CTA counts
     int top_k;             // > 0: chi2 only at the K deepest starts of every trial (chi2_topk.cu, reading G19)
     int chi2_fp32;         // 1: fp32 ring arithmetic in the chi2 kernels (gtls_opts.chi2_fp32)
     const double* gtab;    // [2*(gtab_max+1)] sum g_D, sum g_D^2 for D = 1 .. gtab_max (k_gtab)
@@ -204,6 +205,10 @@ constexpr int kTopKMax = 8;   // largest gtls_opts.top_k the pruning kernel take
 void launch_chi2_topk(const TileArgs& a, cudaStream_t st);
 void launch_gtab(const double* tmpl, int n_tmpl, int gtab_max, double* gtab, cudaStream_t st);
 void launch_durtab(const TileArgs& a, cudaStream_t st);
+// grids.cu: Eq. 4 period grid from the host-side constants A/3 and C; Eq. 8-9 duration fractions
+void launch_period_grid(double a3, double c, long long n_per, double* out, cudaStream_t st);
+void launch_duration_grid(const double* periods, long long n_per, int n_dur, double k_min, double k_max,
+                          double q_cap, double* out, int* bad, cudaStream_t st);
 // bins the tile's trials by chi2 kernel variant (order preserved); skipped trials get an invalid Partial
 void launch_bin_trials(const TileArgs& a, cudaStream_t st);
 void launch_fold_keys(const TileArgs& a, double* phase_out, cudaStream_t st);

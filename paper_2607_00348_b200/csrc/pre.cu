@@ -154,14 +154,21 @@ __device__ __forceinline__ int chi2_variant(const DurEntry& e, const TileArgs& a
     return narrow * kChi2Rings + mbi;
 }
 
-// One CTA: every thread owns a contiguous chunk of trials, so the lists keep trial order (the
-// trials of a period stay neighbours and share its x1 in L2).
-__global__ void __launch_bounds__(1024) k_bin_trials(TileArgs a) {
-    __shared__ int s_warp[kChi2Variants][32];
+// Trials are binned in order (the trials of a period stay neighbours and share its x1 in L2):
+// kBinBlocks CTAs own contiguous segments of the trial range and, inside a CTA, every thread a
+// contiguous chunk.  PHASE 0 counts per (CTA, variant) into a.trial_count[kChi2Variants * (1 + b)];
+// PHASE 1 adds the counts of the CTAs before it, writes the lists and (last CTA) the totals.
+template <int PHASE>
+__global__ void __launch_bounds__(256) k_bin_trials(TileArgs a) {
+    __shared__ int s_warp[kChi2Variants][8];
+    __shared__ int s_base[kChi2Variants];
     const int T = a.tile * a.n_dur;
-    const int chunk = (T + blockDim.x - 1) / blockDim.x;
-    const int t0 = threadIdx.x * chunk, t1 = min(T, t0 + chunk);
+    const int seg = (T + gridDim.x - 1) / gridDim.x;
+    const int b0 = min(T, (int)blockIdx.x * seg), b1 = min(T, b0 + seg);
+    const int chunk = (b1 - b0 + blockDim.x - 1) / blockDim.x;
+    const int t0 = min(b1, b0 + (int)threadIdx.x * chunk), t1 = min(b1, t0 + chunk);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int* block_counts = a.trial_count + kChi2Variants;
     int cnt[kChi2Variants];
 #pragma unroll
     for (int v = 0; v < kChi2Variants; ++v) cnt[v] = 0;
@@ -169,7 +176,12 @@ __global__ void __launch_bounds__(1024) k_bin_trials(TileArgs a) {
         const int v = chi2_variant(a.durtab[t], a);
 #pragma unroll
         for (int k = 0; k < kChi2Variants; ++k) cnt[k] += (v == k) ? 1 : 0;
-        if (v < 0) { Partial p; p.dchi2 = 0.0; p.depth = 0.0; p.start = 0; p.valid = 0; a.partial[t] = p; }
+        if (PHASE == 0 && v < 0) { Partial p; p.dchi2 = 0.0; p.depth = 0.0; p.start = 0; p.valid = 0; a.partial[t] = p; }
+    }
+    if (PHASE == 1 && threadIdx.x < kChi2Variants) {
+        int base = 0;
+        for (int b = 0; b < (int)blockIdx.x; ++b) base += block_counts[b * kChi2Variants + threadIdx.x];
+        s_base[threadIdx.x] = base;
     }
     int excl[kChi2Variants];
 #pragma unroll
@@ -184,18 +196,22 @@ __global__ void __launch_bounds__(1024) k_bin_trials(TileArgs a) {
     if (warp == 0) {
 #pragma unroll
         for (int v = 0; v < kChi2Variants; ++v) {
-            const int c = lane < (int)(blockDim.x >> 5) ? s_warp[v][lane] : 0;
+            const int c = lane < (int)(blockDim.x >> 5) ? s_warp[v][lane & 7] : 0;
             int x = c;
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
-            s_warp[v][lane] = x - c;
-            if (lane == 31) a.trial_count[v] = x;
+            for (int o = 1; o < 8; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+            if (lane < 8) s_warp[v][lane] = x - c;
+            if (lane == 7) {
+                if (PHASE == 0) block_counts[blockIdx.x * kChi2Variants + v] = x;
+                else if (blockIdx.x == gridDim.x - 1) a.trial_count[v] = s_base[v] + x;
+            }
         }
     }
+    if (PHASE == 0) return;
     __syncthreads();
     int pos[kChi2Variants];
 #pragma unroll
-    for (int v = 0; v < kChi2Variants; ++v) pos[v] = s_warp[v][warp] + excl[v];
+    for (int v = 0; v < kChi2Variants; ++v) pos[v] = s_base[v] + s_warp[v][warp] + excl[v];
     for (int t = t0; t < t1; ++t) {
         const int v = chi2_variant(a.durtab[t], a);
 #pragma unroll
@@ -219,7 +235,10 @@ void launch_grid_check(const double* periods, long long n_per, const double* dur
     k_grid_check<<<blocks, 256, 0, st>>>(periods, n_per, durs, n_durs_total, info);
 }
 
-void launch_bin_trials(const TileArgs& a, cudaStream_t st) { k_bin_trials<<<1, 1024, 0, st>>>(a); }
+void launch_bin_trials(const TileArgs& a, cudaStream_t st) {
+    k_bin_trials<0><<<kBinBlocks, 256, 0, st>>>(a);
+    k_bin_trials<1><<<kBinBlocks, 256, 0, st>>>(a);
+}
 
 void launch_gtab(const double* tmpl, int n_tmpl, int gtab_max, double* gtab, cudaStream_t st) {
     const int blocks = (int)(((long long)gtab_max * 32 + 255) / 256);

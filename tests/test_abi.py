@@ -30,7 +30,8 @@ def test_every_declared_symbol_is_exported(lib):
     syms = _declared_symbols()
     assert {"gtls_search", "gtls_fold_sort", "gtls_fold_scan", "gtls_window_chi2", "gtls_sde",
             "gtls_workspace_bytes", "gtls_strerror", "gtls_version", "gtls_last_cuda_error",
-            "gtls_opts_default"} <= set(syms)
+            "gtls_opts_default", "gtls_period_grid_size", "gtls_period_grid", "gtls_duration_grid",
+            "gtls_search_batch", "gtls_batch_workspace_bytes", "gtls_search_two_stage"} <= set(syms)
     for s in syms:
         assert hasattr(lib, s), s
 
@@ -100,3 +101,25 @@ def test_product_never_imports_oracle():
                 src = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in src and "from oracle" not in src, f
                 assert "liboracle" not in src, f
+
+
+def test_period_grid_size_is_host_logic_and_matches_oracle():
+    """N = ceil(Eq. 6) needs no GPU; the oracle computes it with its own code."""
+    import oracle
+    for span, kw in [(30.0, dict(p_min=0.5)), (90.0, dict(p_min=0.5)), (1470.0, dict(p_min=0.5)),
+                     (3000.0, dict(p_min=0.5)), (1500.0, dict()), (200.0, dict(r_star=0.7, m_star=0.6, oversampling=2.0))]:
+        okw = {("p_min_days" if k == "p_min" else k): v for k, v in kw.items()}
+        assert g.gtls_period_grid_size(span, **kw) == oracle.period_grid(span, **okw).size
+    for bad in [dict(span=0.0), dict(span=10.0, r_star=-1.0), dict(span=10.0, oversampling=0.0),
+                dict(span=float("nan")), dict(span=1.0, p_min=0.5)]:
+        with pytest.raises(g.GtlsError):
+            g.gtls_period_grid_size(**bad)
+
+
+def test_batch_workspace_bytes():
+    co = np.array([0, 4000, 8200, 12000], dtype=np.int64)
+    po = np.array([0, 10000, 20500, 30000], dtype=np.int64)
+    a = g.gtls_batch_workspace_bytes(co, po, 25, period_tile=64)
+    one = max(g.gtls_workspace_bytes(int(co[i + 1] - co[i]), int(po[i + 1] - po[i]), 25, period_tile=64) for i in range(3))
+    assert 3 * one <= a <= 3 * one + 4096            # three curves -> three lanes, each fits the largest curve
+    assert g.gtls_batch_workspace_bytes(co[:2], po[:2], 25, period_tile=64) < a
