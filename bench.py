@@ -149,6 +149,60 @@ def run_reference(args, w):
     }
 
 
+def run_survey(args, g, torch, devname):
+    """c5: `--survey N` curves (each with its own Ofir grid and per-period durations) per step through
+    gtls_search_batch, device-resident inputs; the same curves as a loop of gtls_search calls beside it."""
+    ws_ = [gi.make_workload(5, curve=c) for c in range(args.survey)]
+    cat = lambda xs, ax=0: np.ascontiguousarray(np.concatenate(xs, axis=ax))
+    co = np.concatenate([[0], np.cumsum([w.lc.n for w in ws_])]).astype(np.int64)
+    po = np.concatenate([[0], np.cumsum([w.n_per for w in ws_])]).astype(np.int64)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(devname)
+    t, y, dy = (dev(cat([getattr(w.lc, k) for w in ws_])) for k in ("t", "y", "dy"))
+    per, dur, tm = dev(cat([w.periods for w in ws_])), dev(cat([w.durations for w in ws_])), dev(ws_[0].tmpl)
+    wsp = torch.empty(g.gtls_batch_workspace_bytes(co, po, ws_[0].n_dur), dtype=torch.uint8, device=devname)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=devname)
+    trials = int(sum(w.trials for w in ws_))
+
+    def timed(fn):
+        for _ in range(max(args.warmup, 3)):
+            fn()
+        torch.cuda.synchronize()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        for _ in range(args.steps):
+            flush.zero_()
+            r = fn()
+        ev1.record()
+        torch.cuda.synchronize()
+        return ev0.elapsed_time(ev1) / args.steps, r
+
+    dt0 = ws_[0].dt0 if args.dt0 is None else float(args.dt0)
+    sampler = ClockSampler(int(devname.split(":")[1]))
+    sampler.start()
+    ms_batch, res = timed(lambda: g.gtls_search_batch(t, y, dy, co, per, po, dur, tm, dt0=dt0, sde_kernel=151,
+                                                      workspace=wsp))
+    clocks = sampler.stop()
+    one_ws = wsp[:max(g.gtls_workspace_bytes(w.lc.n, w.n_per, w.n_dur) for w in ws_)]
+
+    def loop():
+        for c in range(len(ws_)):
+            r = g.gtls_search(t[co[c]:co[c + 1]], y[co[c]:co[c + 1]], dy[co[c]:co[c + 1]], per[po[c]:po[c + 1]],
+                              dur[po[c]:po[c + 1]], tm, dt0=dt0, sde_kernel=151, workspace=one_ws)
+        return r
+    ms_loop, _ = timed(loop)
+    found = sum(1 for c, w in enumerate(ws_) if c % 2 == 0 and res.summaries[c]["sde_max"] > 9.0)
+    return {"metric": METRIC, "value": trials / (ms_batch / 1e3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_batch, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"c5 survey batch: {len(ws_)} independent 90-day curves (~{int(co[-1] / len(ws_))} points, "
+                                   f"~{int(po[-1] / len(ws_))} periods x {ws_[0].n_dur} durations each), dt0={dt0}, one gtls_search_batch call",
+                       "l2_flush": "256 MiB memset between timed steps"},
+            "curves_per_s": len(ws_) / (ms_batch / 1e3), "ms_per_curve": ms_batch / len(ws_),
+            "loop_of_single_calls": {"curves_per_s": len(ws_) / (ms_loop / 1e3), "ms_per_curve": ms_loop / len(ws_)},
+            "curves_with_injected_transit_above_sde_9": f"{found} of {(len(ws_) + 1) // 2}",
+            "clocks": clocks}
+
+
 def max_over_ranks(x: float, world: int, device="cpu") -> float:
     """Multi-rank runs (replicas only): the job time is the slowest rank's."""
     if world <= 1:
@@ -181,6 +235,9 @@ def main():
     ap.add_argument("--every", type=int, default=1,
                     help="profiling aid: search only every k-th period of the workload (default 1 = the "
                          "full workload; any other value is named in config.workload)")
+    ap.add_argument("--survey", type=int, default=0,
+                    help="survey mode (BASELINE.json config 5): search this many c5 curves per step with one "
+                         "gtls_search_batch call and report curves/s beside trials/s")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -205,6 +262,11 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(devname))
     g.load_library()
+
+    if args.survey > 0:
+        if rank == 0:
+            print(json.dumps(run_survey(args, g, torch, devname)), flush=True)
+        return 0
 
     # every rank searches its own curve of the same shape (independent problems)
     w = build_workload(args.workload, curve=rank, every=args.every, dt0=args.dt0)
