@@ -317,15 +317,15 @@ def main():
         achieved = flops_per_launch / (chi2_ms_per_launch * 1e-3) / 1e12
         sm_max = float(peaks.get("sm_max_mhz", 1965.0))
         peak = SM_COUNT * DFMA_PER_CLK_PER_SM * 2 * sm_max * 1e6 / 1e12
-        # DRAM traffic of one such launch from the ncu --set full capture of this workload's tile (sum of
-        # dram__bytes_read.sum + dram__bytes_write.sum over the ring-kernel variants of one 2081-period c4
-        # tile of the every-64th-period subsample, profiles/r1_E_final_c4e64.md; the full c4 run uses
-        # 2085-period tiles of the same kernels; the tile with the longest periods moves 75 GB, profile D);
-        # other workloads / tile sizes have no capture: null
-        traffic = 2.084e10 if (args.workload == "c4" and args.dt0 is None and abs(st_acc["period_tile"] - 2083) <= 3) else None
+        # DRAM traffic of one such launch from the ncu --set full capture of this workload's tile: sum of
+        # dram__bytes_read.sum + dram__bytes_write.sum over the eleven ring-kernel launches of one
+        # 4144-period tile of c4 (profiles/r1_F_final_c4e64.md: the first tile of the every-64th-period
+        # subsample, periods spread over the longer 63 % of the grid; the full run's tiles are 4144
+        # consecutive periods of the same kernels).  Other workloads / tile sizes have no capture: null
+        traffic = 9.12e10 if (args.workload == "c4" and args.dt0 is None and st_acc["period_tile"] == 4144) else None
         roofline = {"bound": "alu", "kernel": "k_chi2_ring (in-transit chi2, a5-a8; one 'launch' = the chi2 stage of one period tile: trial binning + the ring-kernel variants)", "achieved": achieved,
                     "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
-                    "traffic_unit": "bytes per launch (ncu dram read + write, profiles/r1_E_final_c4e64.md)",
+                    "traffic_unit": "bytes per launch (ncu dram read + write, profiles/r1_F_final_c4e64.md)",
                     "peak_source": f"derived: {SM_COUNT} SMs x {DFMA_PER_CLK_PER_SM} DFMA/clk x 2 flop x "
                                    f"{sm_max:.0f} MHz ({peak_src} sm_max_mhz); a dependent-chain DFMA microbenchmark on this "
                                    f"pool sustains 34.1 TFLOP/s",
