@@ -385,7 +385,7 @@ def main():
             d2h = int(w.n_per * (8 * 3 + 24))
             out["e2e"] = {"value": world * w.trials / dt, "unit": UNIT, "h2d_bytes_per_step": h2d,
                           "d2h_bytes_per_step": d2h, "ms_per_step": dt * 1e3, "steps": n_e2e,
-                          "note": "gtls_search with host pointers: cudaMalloc + H2D + search + D2H per call"}
+                          "note": "gtls_search with host pointers: H2D + search + D2H per call; device blocks up to 8 GiB come from the library's pool after the warm-up call, larger ones are cudaMalloc'ed per call"}
 
     if rank == 0:
         if not args.no_cpu_baseline:

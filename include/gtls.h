@@ -253,6 +253,12 @@ size_t gtls_batch_workspace_bytes(int32_t n_curves, const int64_t* curve_offset,
  * allocation inside the call. */
 size_t gtls_workspace_bytes(int64_t n, int64_t n_per, int32_t n_dur, const gtls_opts* opts);
 
+/* Device blocks the library allocates itself (the staged copies of host arrays, the scratch when
+ * opts->workspace is NULL) are kept in a small pool between calls instead of being freed: at most four
+ * free blocks of at most GTLS_CACHE_MB MiB each (environment, default 8192; 0 = no pool).  This call frees
+ * them.  Caller-owned memory is never retained. */
+void gtls_release_cache(void);
+
 const char* gtls_strerror(int code);
 const char* gtls_version(void);
 /* Text of the last CUDA error seen by the calling thread ("" if none). */

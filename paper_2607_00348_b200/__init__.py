@@ -22,7 +22,7 @@ import numpy as np
 
 __all__ = ["gtls_search", "gtls_search_two_stage", "gtls_search_batch", "gtls_batch_workspace_bytes",
            "gtls_period_grid_size", "gtls_period_grid", "gtls_duration_grid", "BatchResult", "gtls_search_sharded", "gtls_fold_sort", "gtls_fold_scan", "gtls_window_chi2", "gtls_sde",
-           "gtls_workspace_bytes", "gtls_strerror", "gtls_version", "GtlsError", "SearchResult",
+           "gtls_workspace_bytes", "gtls_release_cache", "gtls_strerror", "gtls_version", "GtlsError", "SearchResult",
            "BEST_DTYPE", "lib_path", "load_library"]
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
@@ -127,6 +127,8 @@ def load_library():
     lib.gtls_batch_workspace_bytes.restype = C.c_size_t
     lib.gtls_workspace_bytes.argtypes = [C.c_int64, C.c_int64, C.c_int32, C.POINTER(GtlsOpts)]
     lib.gtls_workspace_bytes.restype = C.c_size_t
+    lib.gtls_release_cache.argtypes = []
+    lib.gtls_release_cache.restype = None
     lib.gtls_strerror.argtypes = [C.c_int]
     lib.gtls_strerror.restype = C.c_char_p
     lib.gtls_version.restype = C.c_char_p
@@ -205,6 +207,11 @@ class SearchResult:
 
 def gtls_version() -> str:
     return load_library().gtls_version().decode()
+
+
+def gtls_release_cache() -> None:
+    """Free the device blocks the library keeps between calls (``gtls_release_cache`` in include/gtls.h)."""
+    load_library().gtls_release_cache()
 
 
 def gtls_strerror(code: int) -> str:

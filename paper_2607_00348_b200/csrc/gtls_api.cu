@@ -5,6 +5,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <cmath>
+#include <mutex>
 #include <new>
 #include <thread>
 #include <vector>
@@ -30,11 +31,53 @@ int cuda_fail(cudaError_t e, const char* what) {
 
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
+// Device blocks the library allocated itself are kept in a small pool between calls (cudaMalloc and
+// cudaFree of a few GB cost milliseconds each and cudaFree synchronises the device: half of the end-to-end
+// time of a short light curve through host buffers).  At most kPoolSlots free blocks, each at most
+// GTLS_CACHE_MB (default 8192) MiB; gtls_release_cache() frees them; GTLS_CACHE_MB=0 switches the pool off.
+constexpr int kPoolSlots = 4;
+struct PoolBlock { char* base; size_t size; int dev; };
+std::mutex g_pool_mu;
+PoolBlock g_pool[kPoolSlots] = {};
+size_t pool_cap() {
+    static const size_t cap = [] { const char* e = getenv("GTLS_CACHE_MB"); return (size_t)(e ? atoll(e) : 8192) << 20; }();
+    return cap;
+}
+char* pool_take(size_t bytes, size_t* got) {
+    int dev = -1;
+    if (pool_cap() == 0 || cudaGetDevice(&dev) != cudaSuccess) return nullptr;
+    std::lock_guard<std::mutex> lk(g_pool_mu);
+    int best = -1;
+    for (int i = 0; i < kPoolSlots; ++i)
+        if (g_pool[i].base && g_pool[i].dev == dev && g_pool[i].size >= bytes &&
+            (best < 0 || g_pool[i].size < g_pool[best].size)) best = i;
+    if (best < 0) return nullptr;
+    char* p = g_pool[best].base; *got = g_pool[best].size;
+    g_pool[best] = PoolBlock{};
+    return p;
+}
+void pool_give(char* base, size_t size) {
+    int dev = -1;
+    if (size <= pool_cap() && cudaGetDevice(&dev) == cudaSuccess) {
+        std::lock_guard<std::mutex> lk(g_pool_mu);
+        int slot = -1;
+        for (int i = 0; i < kPoolSlots; ++i) if (!g_pool[i].base) { slot = i; break; }
+        if (slot < 0) {                       // full: the smallest block makes room if it is smaller than this one
+            int sm = 0;
+            for (int i = 1; i < kPoolSlots; ++i) if (g_pool[i].size < g_pool[sm].size) sm = i;
+            if (g_pool[sm].size < size) { cudaFree(g_pool[sm].base); slot = sm; }
+        }
+        if (slot >= 0) { g_pool[slot] = PoolBlock{base, size, dev}; return; }
+    }
+    cudaFree(base);
+}
+
 // Bump allocator over one device block.
 struct Arena {
     char* base = nullptr;
     size_t size = 0, off = 0;
     bool owned = false;
+    bool idle = false;      // set by the owner after its last stream synchronisation: nothing uses the block any more
     template <typename T>
     T* take(size_t count) {
         off = align_up(off);
@@ -42,7 +85,11 @@ struct Arena {
         off += count * sizeof(T);
         return off <= size ? p : nullptr;
     }
-    ~Arena() { if (owned && base) cudaFree(base); }
+    ~Arena() {
+        if (!owned || !base) return;
+        if (!idle) cudaDeviceSynchronize();   // early returns: kernels of this call may still be running
+        pool_give(base, size);
+    }
 };
 
 struct Sizes {
@@ -130,8 +177,16 @@ int stage_in(const T* src, size_t count, bool on_device, Arena& ar, cudaStream_t
 }
 
 int alloc_arena(Arena& ar, size_t bytes) {
+    size_t got = 0;
+    if (char* p = pool_take(bytes, &got)) { ar.base = p; ar.size = got; ar.off = 0; ar.owned = true; return GTLS_OK; }
+    if (pool_cap() && bytes <= pool_cap()) bytes = align_up(bytes + bytes / 16, 2u << 20);   // slack: the next, slightly larger request fits too
     cudaError_t e = cudaMalloc((void**)&ar.base, bytes);
-    if (e != cudaSuccess) { cudaGetLastError(); snprintf(g_cuda_err, sizeof(g_cuda_err), "cudaMalloc(%zu): %s", bytes, cudaGetErrorString(e)); return GTLS_ENOMEM; }
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        gtls_release_cache();                  // the pool may hold what this request needs
+        e = cudaMalloc((void**)&ar.base, bytes);
+    }
+    if (e != cudaSuccess) { cudaGetLastError(); ar.base = nullptr; snprintf(g_cuda_err, sizeof(g_cuda_err), "cudaMalloc(%zu): %s", bytes, cudaGetErrorString(e)); return GTLS_ENOMEM; }
     ar.size = bytes; ar.off = 0; ar.owned = true;
     return GTLS_OK;
 }
@@ -269,6 +324,11 @@ void gtls_opts_default(gtls_opts* o) {
 }
 
 const char* gtls_version(void) { return "gtls-b200 0.1.0 (sm_100a)"; }
+
+void gtls_release_cache(void) {
+    std::lock_guard<std::mutex> lk(g_pool_mu);
+    for (auto& b : g_pool) { if (b.base) cudaFree(b.base); b = PoolBlock{}; }
+}
 const char* gtls_last_cuda_error(void) { return g_cuda_err; }
 
 const char* gtls_strerror(int code) {
@@ -523,6 +583,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
         *o.stats = stats;
         cudaEventDestroy(ev_begin); cudaEventDestroy(ev_end);
     }
+    io.idle = ws.idle = true;                 // the stream was synchronised after the last use of both
     return sc.degenerate ? GTLS_EDEGENERATE : GTLS_OK;
 }
 

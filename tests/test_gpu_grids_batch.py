@@ -166,3 +166,28 @@ def test_search_batch_shared_durations_workspace_and_status():
                                po.ctypes.data, q.ctypes.data, 9, tm.ctypes.data, tm.size, C.byref(o),
                                chi2.ctypes.data, None, None, None, None, status.ctypes.data)
     assert rc == -2 and list(status) == [0, 0, -2]                           # GTLS_ENONFINITE
+
+
+def test_block_pool_reuse_and_release():
+    """Host-buffer calls keep their device blocks between calls: results do not depend on whether a block is
+    fresh or reused (also by a call of another size), and gtls_release_cache gives the memory back."""
+    torch = _cuda()
+    g.gtls_release_cache()
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    w = gi.make_workload(2).subset(211)
+    a = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, sde_kernel=5)      # fresh blocks
+    held = free0 - torch.cuda.mem_get_info()[0]
+    assert held > 0                                                                                # pooled
+    w1 = gi.make_workload(1).subset(61)
+    c = g.gtls_search(w1.lc.t, w1.lc.y, w1.lc.dy, w1.periods, w1.durations, w1.tmpl, sde_kernel=5)  # smaller: reuses
+    b = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, sde_kernel=5)      # reused blocks
+    assert np.array_equal(a.chi2, b.chi2) and np.array_equal(a.best(), b.best()) and np.array_equal(a.sde, b.sde)
+    ora = oracle.search(w1.lc.t, w1.lc.y, w1.lc.dy, w1.periods, w1.durations, w1.tmpl, dt0=0.05)
+    assert np.max(np.abs(c.chi2 / ora.chi2 - 1.0)) <= 1e-9
+    with pytest.raises(g.GtlsError):                                                               # error path returns its blocks too
+        bad = w.lc.dy.copy(); bad[3] = 0.0
+        g.gtls_search(w.lc.t, w.lc.y, bad, w.periods, w.durations, w.tmpl)
+    assert torch.cuda.mem_get_info()[0] >= free0 - 2 * held - (64 << 20)                           # bounded, no growth per call
+    g.gtls_release_cache()
+    assert torch.cuda.mem_get_info()[0] >= free0 - (8 << 20)
