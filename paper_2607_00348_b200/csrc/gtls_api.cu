@@ -1081,8 +1081,7 @@ int gtls_search_batch(int32_t n_curves, const double* t, const double* y, const 
     std::vector<cudaEvent_t> ev_done((size_t)lanes, nullptr);
     std::vector<int> lane_rc((size_t)lanes, GTLS_OK);
     std::vector<std::thread> workers;
-    for (int lane = 0; lane < lanes; ++lane) {
-        workers.emplace_back([&, lane]() {
+    auto lane_body = [&](int lane) {
             cudaStream_t ls = nullptr;
             if (cudaSetDevice(o.device) != cudaSuccess ||
                 cudaStreamCreateWithFlags(&ls, cudaStreamNonBlocking) != cudaSuccess ||
@@ -1110,8 +1109,12 @@ int gtls_search_batch(int32_t n_curves, const double* t, const double* y, const 
             cudaEventRecord(ev_done[lane], ls);
             cudaStreamSynchronize(ls);
             cudaStreamDestroy(ls);
-        });
+    };
+    for (int lane = 1; lane < lanes; ++lane) {
+        try { workers.emplace_back(lane_body, lane); }
+        catch (...) { lane_body(lane); }          // no thread to be had: the lane runs here, in turn
     }
+    lane_body(0);                                 // the calling thread is lane 0
     for (auto& w : workers) w.join();
     for (int lane = 0; lane < lanes; ++lane)
         if (ev_done[lane]) { cudaStreamWaitEvent(st, ev_done[lane], 0); cudaEventDestroy(ev_done[lane]); }
