@@ -57,16 +57,22 @@ class ClockSampler:
         self.idx = gpu_index
         self.proc = None
         self.lines = []
+        self.first = 0
 
     def start(self):
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", f"--id={self.idx}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                 "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                 "-lms", "500"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
         except Exception:
             self.proc = None
+
+    def mark(self):
+        """Start of the timed region: nvidia-smi is started before the warm-up (its start-up takes driver
+        locks for most of a second, which a 10 ms step would see); samples before this call are dropped."""
+        self.first = len(self.lines)
 
     def _read(self):
         for line in self.proc.stdout:
@@ -82,7 +88,7 @@ class ClockSampler:
             self.proc.kill()
         sm, mx, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for ln in self.lines:
+        for ln in self.lines[self.first:] or self.lines[-1:]:
             f = [x.strip() for x in ln.split(",")]
             if len(f) < 9:
                 continue
@@ -163,10 +169,12 @@ def run_survey(args, g, torch, devname):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=devname)
     trials = int(sum(w.trials for w in ws_))
 
-    def timed(fn):
+    def timed(fn, sampler=None):
         for _ in range(max(args.warmup, 3)):
             fn()
         torch.cuda.synchronize()
+        if sampler:
+            sampler.mark()
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         ev0.record()
         for _ in range(args.steps):
@@ -180,8 +188,7 @@ def run_survey(args, g, torch, devname):
     sampler = ClockSampler(int(devname.split(":")[1]))
     sampler.start()
     ms_batch, res = timed(lambda: g.gtls_search_batch(t, y, dy, co, per, po, dur, tm, dt0=dt0, sde_kernel=151,
-                                                      workspace=wsp))
-    clocks = sampler.stop()
+                                                      workspace=wsp), sampler)
     one_ws = wsp[:max(g.gtls_workspace_bytes(w.lc.n, w.n_per, w.n_dur) for w in ws_)]
 
     def loop():
@@ -190,6 +197,7 @@ def run_survey(args, g, torch, devname):
                               dur[po[c]:po[c + 1]], tm, dt0=dt0, sde_kernel=151, workspace=one_ws)
         return r
     ms_loop, _ = timed(loop)
+    clocks = sampler.stop()                      # both legs ran with the sampler polling
     found = sum(1 for c, w in enumerate(ws_) if c % 2 == 0 and res.summaries[c]["sde_max"] > 9.0)
     return {"metric": METRIC, "value": trials / (ms_batch / 1e3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_batch, "higher_is_better": True, "scaling": "weak",
@@ -285,14 +293,15 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    sampler = ClockSampler(local_rank)
+    sampler.start()
     for _ in range(max(args.warmup, 3)):
         res = step()
     barrier()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     st_acc = {}
     barrier()
+    sampler.mark()
     ev0.record()
     for _ in range(args.steps):
         flush.zero_()                                   # L2 flush between timed iterations

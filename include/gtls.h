@@ -233,10 +233,11 @@ int gtls_duration_grid(const double* periods, int64_t n_per, int32_t n_dur, doub
  * 0; every other array is host or device per opts->pointers_on_device.  Outputs are concatenated in the
  * same order as period_grid: out_chi2 [total periods] (required), out_best / out_sde_raw / out_sde (may
  * be NULL); out_summary [n_curves] and out_status [n_curves] are HOST arrays and may be NULL.
- * Each curve is one gtls_search (same options, same results bit for bit); the curves run concurrently
- * on a few internal streams (ordered after opts->stream at entry, joined before return), each stream
- * with its own slice of the scratch: opts->workspace, when given, must hold
- * gtls_batch_workspace_bytes(...).  The call returns after all curves have finished.
+ * Each curve is one gtls_search (same options, same results bit for bit) on an internal stream (ordered
+ * after opts->stream at entry, joined before return).  GTLS_BATCH_LANES (environment, default 1, at most
+ * 16) curves run concurrently, each lane on its own stream and host thread with its own slice of the
+ * scratch: opts->workspace, when given, must hold gtls_batch_workspace_bytes(...).  The call returns
+ * after all curves have finished.
  * Return: GTLS_OK when every curve returned GTLS_OK or GTLS_EDEGENERATE (see out_status), else the
  * error code of the first failing curve; curves after a failure are still searched. */
 int gtls_search_batch(int32_t n_curves, const double* t, const double* y, const double* dy,

@@ -50,11 +50,11 @@ constexpr int kFifoRows = 24;            // >= kFifoBatches * max PfRows
 constexpr int kCW = 704;                 // window-table doubles per warp (>= 32 * 21)
 constexpr int kTmplSmem = 512;           // template nodes cached in shared memory
 #ifndef GTLS_GRID_WAVES
-#define GTLS_GRID_WAVES 8
+#define GTLS_GRID_WAVES 16
 #endif
 constexpr unsigned kGridCap = 148u * 6u * GTLS_GRID_WAVES;   // CTAs per launch: waves of the 6 resident CTAs per SM
 // The cap applies to short light curves only: there the trials are short and tens of thousands of empty CTAs
-// per variant launch are 5 % of a search (c2 9.73 -> 9.27 ms, c1 1.70 -> 1.61 ms).  On long curves the fixed
+// per variant launch are 5 % of a search (c2 9.73 -> 9.14 ms, c1 1.70 -> 1.63 ms; 8 / 16 / 32 waves: c2 9.27 / 9.14 / 9.15 ms).  On long curves the fixed
 // round-robin assignment of trials to warps loses more at the tail than the empty CTAs cost (c4 6.2 -> 6.7 s,
 // c3 1.54 -> 1.70 s with the cap): there every CTA takes one pair of trials and the hardware balances them.
 constexpr int kGridCapMaxN = 16384;

@@ -926,7 +926,8 @@ int ofir_constants(double span, double r_star, double m_star, double oversamplin
 
 int batch_lanes(int n_curves) {
     static const int env = [] { const char* e = getenv("GTLS_BATCH_LANES"); return e ? atoi(e) : 0; }();
-    int lanes = env > 0 ? env : 2;     // measured on c5: a c2-sized search fills the device; 4 / 8 lanes are 10 % slower
+    int lanes = env > 0 ? env : 1;     // measured on c5: a c2-sized search fills the device; 2 lanes give 9.0-10.3 ms per
+                                       // curve from run to run against a steady 9.1 ms for one lane, 4 / 8 lanes are 10 % slower
     if (lanes > 16) lanes = 16;
     return lanes < n_curves ? lanes : (n_curves < 1 ? 1 : n_curves);
 }

@@ -121,5 +121,6 @@ def test_batch_workspace_bytes():
     po = np.array([0, 10000, 20500, 30000], dtype=np.int64)
     a = g.gtls_batch_workspace_bytes(co, po, 25, period_tile=64)
     one = max(g.gtls_workspace_bytes(int(co[i + 1] - co[i]), int(po[i + 1] - po[i]), 25, period_tile=64) for i in range(3))
-    assert 2 * one <= a <= 2 * one + 4096            # two lanes, each fits the largest curve
-    assert g.gtls_batch_workspace_bytes(co[:2], po[:2], 25, period_tile=64) < a      # one curve -> one lane
+    lanes = int(os.environ.get("GTLS_BATCH_LANES", "1"))
+    assert lanes * one <= a <= lanes * one + 4096    # every lane fits the largest curve
+    assert g.gtls_batch_workspace_bytes(co[:2], po[:2], 25, period_tile=64) <= a

@@ -191,3 +191,30 @@ def test_block_pool_reuse_and_release():
     assert torch.cuda.mem_get_info()[0] >= free0 - 2 * held - (64 << 20)                           # bounded, no growth per call
     g.gtls_release_cache()
     assert torch.cuda.mem_get_info()[0] >= free0 - (8 << 20)
+
+
+def test_search_batch_concurrent_lanes_subprocess():
+    """GTLS_BATCH_LANES is read once per process: three concurrent lanes (host threads, one stream and one
+    scratch slice each) in a child process, results bit-identical to single calls."""
+    _cuda()
+    import os, subprocess, sys
+    code = r'''
+import numpy as np, gtls_inputs as gi, paper_2607_00348_b200 as g
+ws = [gi.make_workload(5, curve=c).subset(131, offset=c) for c in range(7)]
+cat = lambda xs: np.ascontiguousarray(np.concatenate(xs, axis=0))
+co = np.concatenate([[0], np.cumsum([w.lc.n for w in ws])]).astype(np.int64)
+po = np.concatenate([[0], np.cumsum([w.n_per for w in ws])]).astype(np.int64)
+res = g.gtls_search_batch(cat([w.lc.t for w in ws]), cat([w.lc.y for w in ws]), cat([w.lc.dy for w in ws]), co,
+                          cat([w.periods for w in ws]), po, cat([w.durations for w in ws]), ws[0].tmpl, sde_kernel=21)
+assert g.gtls_batch_workspace_bytes(co, po, 25) >= 3 * max(g.gtls_workspace_bytes(w.lc.n, w.n_per, 25) for w in ws)
+for c, w in enumerate(ws):
+    one = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, sde_kernel=21)
+    sl = slice(po[c], po[c + 1])
+    assert np.array_equal(res.chi2[sl], one.chi2) and np.array_equal(res.sde[sl], one.sde)
+    assert np.array_equal(res.best()[sl], one.best()) and res.summaries[c] == one.summary
+print("lanes ok")
+'''
+    env = dict(os.environ, GTLS_BATCH_LANES="3")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, "-c", code], cwd=root, env=env, capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0 and "lanes ok" in out.stdout, out.stderr[-2000:]
