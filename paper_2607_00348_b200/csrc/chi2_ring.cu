@@ -49,15 +49,7 @@ constexpr int kFifoBatches = 3;          // batches of PfRows rows per lane in t
 constexpr int kFifoRows = 24;            // >= kFifoBatches * max PfRows
 constexpr int kCW = 704;                 // window-table doubles per warp (>= 32 * 21)
 constexpr int kTmplSmem = 512;           // template nodes cached in shared memory
-#ifndef GTLS_GRID_WAVES
-#define GTLS_GRID_WAVES 16
-#endif
-constexpr unsigned kGridCap = 148u * 6u * GTLS_GRID_WAVES;   // CTAs per launch: waves of the 6 resident CTAs per SM
-// The cap applies to short light curves only: there the trials are short and tens of thousands of empty CTAs
-// per variant launch are 5 % of a search (c2 9.73 -> 9.14 ms, c1 1.70 -> 1.63 ms; 8 / 16 / 32 waves: c2 9.27 / 9.14 / 9.15 ms).  On long curves the fixed
-// round-robin assignment of trials to warps loses more at the tail than the empty CTAs cost (c4 6.2 -> 6.7 s,
-// c3 1.54 -> 1.70 s with the cap): there every CTA takes one pair of trials and the hardware balances them.
-constexpr int kGridCapMaxN = 16384;
+constexpr unsigned kGridCap = 148u * 6u;   // CTAs per launch: the 6 resident CTAs per SM, persistent (dynamic trial queue)
 constexpr int kWarpSmem = kPartRows * kPartPitch + kFifoRows * 32 + kCW;   // doubles per warp
 
 struct Cand { double d; double depth; int s; int has; };
@@ -84,6 +76,11 @@ __device__ __forceinline__ void cp_async8(const unsigned dst, const double* src,
 }
 __device__ __forceinline__ void cp_async8(const unsigned dst, const double* src) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+}
+// 16-byte copy (both addresses 16-byte aligned); `valid == false` writes zeros without reading
+__device__ __forceinline__ void cp_async16(const unsigned dst, const double* src, const bool valid) {
+    const int sz = valid ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(sz) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
@@ -115,7 +112,7 @@ __device__ __forceinline__ void score_one(const Cls& c, Cand& best, const int s,
 }
 // Wide path: score the windows [k0, k0 + nWt) of the class from table entries [0, nWt).
 __device__ __forceinline__ void score_wide(const Cls& c, Cand& best, const int lane, const int k0,
-                                           const int nWt) {
+                                           const int nWt, const int toff) {
     for (int i0 = 0; i0 < nWt; i0 += 128) {
         double hi1[4], lo1[4], hi0[4], lo0[4];
 #pragma unroll
@@ -135,7 +132,7 @@ __device__ __forceinline__ void score_wide(const Cls& c, Cand& best, const int l
         for (int u = 0; u < 4; ++u) {
             const int w = i0 + 32 * u + lane;
             if (w < nWt) {
-                const unsigned ta = c.ctab + (unsigned)(w * 8);
+                const unsigned ta = c.ctab + (unsigned)((w + toff) * 8);
                 score_one(c, best, c.off + (k0 + w) * c.stp, hi1[u], lo1[u], hi0[u], lo0[u], lds64(ta),
                           c.uniform ? 0.0 : lds64(ta + (unsigned)(c.Kt * 8)));
             }
@@ -416,108 +413,123 @@ __device__ __forceinline__ void march_dual(const Cls& c, const It& it, const dou
     }
 }
 
-// Wide path, one segment per warp: the same march as a software pipeline.  A warp issues in order, so
-// every load is placed at least one row (MB DFMAs) before its first use:
-//   - the X value of row j+LA is read from the FIFO while row j is multiplied; whenever the reads enter a
-//     new group of PF rows, the PF slots of the group just left are refilled (cp.async) with their rows
-//     + MB in one burst (FIFO depth = MB rows);
-//   - the column sums of a completed batch of PF windows are spread over the rows of the NEXT batch:
-//     A (batch end) 4 loads, B 4 loads + first partial sum, C second partial sum, D/E the two shuffle
-//     steps and the table load, F the table store.  Two emit buffers alternate.
+// Wide path, one segment per warp, as a SHIFT REGISTER: acc[j] is the partial sum of the window that has
+// taken j taps so far; a row step is  acc[j+1] = T[j] * x + acc[j]  for j = MB-1 .. 1 (the destination of a
+// DFMA is not its addend, so nothing is moved), acc[1] = T[0] * x starts a window and acc[MB] is complete.
+// All register indices are static after unrolling ONE batch of 8 rows (the ring form needed MB rows), so the
+// body is 8 * MB DFMAs and the whole steady state is branch free:
+//   - the X FIFO is three groups of 8 rows; when the reads (3 rows ahead of the multiplies) enter the next
+//     group, the 8 slots just left are refilled by predicated zero-filling 8-byte cp.async copies, 19 - 26
+//     rows ahead of their use;
+//   - the column sums of batch b-1 (8 windows x 32 lanes in the emit buffer: four lanes per window, eight
+//     strided values each, two shuffle steps, then table[row] += sum) are spread over rows 0 .. 4 of batch b;
+//     the two emit buffers alternate.
+// Table entry rho holds the window that COMPLETES at row rho of the tile, i.e. window rho - (MB-1): the
+// first MB-1 entries (warm-up rows) and the 8 entries behind the table proper (the sums the first batch
+// takes from the still empty emit buffer) are slack that is never scored, so no store is predicated.
+constexpr int kSPF = 8;                         // rows per batch
+constexpr int kTabSlack = 8;                    // dummy entries behind the rows of a table
+constexpr int kChunkW = 31;                     // columns per chunk: any 31 consecutive doubles lie inside 16 aligned 16-byte pieces
+// X feed: a cp.async instruction costs the issuing sub-partition ~11 cycles of FP64 issue whatever its size
+// (measured: DFMA stream + one LDGSTS per k DFMAs), so the rows are copied in 16-byte pieces, TWO rows per
+// instruction: lanes 0-15 copy the 16 pieces of one row (the aligned 32-double window around the chunk's
+// 31 columns), lanes 16-31 the next row.  Lane l then reads its own column at (l + parity) * 8 of the row
+// slot, parity = (first element of the row) & 1; rows alternate between two parities when stp is odd, and a
+// lane half always copies rows of the same parity (its pointer advances by 2 stp per copy).
 template <int MB, typename F>
-__device__ __forceinline__ void march_pipe(const Cls& c, const It& it, const double* __restrict__ xp,
-                                           const int rows_valid, const int rows_min, const int nblk,
-                                           const F (&T)[MB], const int lane) {
-    constexpr int PF = PfRows<MB>::v;
-    constexpr int NBAT = MB / PF;                  // copy groups in flight = batches per block
-    constexpr int XQ = (MB % 3 == 0) ? 3 : 4;      // X registers; LA rows of look-ahead
-    constexpr int LA = XQ - 1;
-    static_assert(PF >= 6 && MB % PF == 0 && MB % XQ == 0 && MB <= kFifoRows && 2 * PF <= kPartRows, "geometry");
+__device__ __forceinline__ void march_shift(const Cls& c, const unsigned tab, const unsigned tab_dummy,
+                                            const double* __restrict__ x, const long long ebase0,
+                                            const int rows_valid, const int nbat, const F (&T)[MB],
+                                            const int lane) {
+    constexpr int PF = kSPF, XQ = 4, LA = 3, NG = 3;
+    static_assert(NG * PF <= kFifoRows && 2 * PF <= kPartRows && MB >= 2, "geometry");
     constexpr unsigned kRowB = kPartPitch * 8;     // bytes per emit-buffer row
-    F acc[MB], xq[XQ];
+    constexpr unsigned kGrpB = PF * 256;           // bytes per FIFO group
+    F acc[MB + 1], xq[XQ];
 #pragma unroll
-    for (int u = 0; u < MB; ++u) acc[u] = (F)0;
-    const unsigned fl = c.fifo + (unsigned)(lane * 8);
-    const long long rstride = (long long)c.stp;
-    int row_issue = 0;                             // next row to copy
+    for (int u = 0; u <= MB; ++u) acc[u] = (F)0;
+    // copy role: rows 2j + half of a group, piece `pc` (two doubles) of the row's aligned window
+    const int half = lane >> 4, pc = lane & 15;
+    const double* cp = x + (((ebase0 + (long long)half * c.stp) >> 1) << 1) + 2 * pc;
+    const long long cstride = 2ll * c.stp;
+    const unsigned cdst = c.fifo + (unsigned)(half * 256 + pc * 16);
+    int row_issue = half;                          // row index of this lane's next copy
 #pragma unroll
-    for (int k = 0; k < NBAT; ++k) {
+    for (int k = 0; k < NG; ++k) {
 #pragma unroll
-        for (int u = 0; u < PF; ++u) {
-            cp_async8(fl + (unsigned)((k * PF + u) * 256), xp, row_issue < rows_valid);
-            xp += rstride;
-            ++row_issue;
+        for (int j = 0; j < PF / 2; ++j) {
+            cp_async16(cdst + (unsigned)((k * PF + 2 * j) * 256), cp, row_issue < rows_valid);
+            cp += cstride;
+            row_issue += 2;
         }
         cp_async_commit();
     }
-    cp_async_wait<NBAT - 1>();
+    cp_async_wait<NG - 1>();
+    __syncwarp();
+    // read role: own column of even / odd rows of a batch (PF is even: the same parities in every batch)
+    const int p0 = (int)(ebase0 & 1), p1 = (int)((ebase0 + c.stp) & 1);
+    const unsigned fe = c.fifo + (unsigned)((lane + p0) * 8), fo = c.fifo + (unsigned)((lane + p1) * 8);
 #pragma unroll
-    for (int k = 0; k < LA; ++k) xq[k] = (F)lds64(fl + (unsigned)(k * 256));
+    for (int k = 0; k < LA; ++k) xq[k] = (F)lds64(((k & 1) ? fo : fe) + (unsigned)(k * 256));
+    unsigned gcur = 0, gnext = kGrpB;              // byte offsets of the FIFO group being multiplied / the next
 
     // column-sum roles: lane = (window slot sl, quarter r); quarter r adds lanes r, r+4, ..., r+28
     const int sl = lane >> 2, r = lane & 3;
-    const int slc = sl < PF ? sl : PF - 1;
-    const unsigned rd_off = (unsigned)((slc * kPartPitch + r) * 8);
-    const bool my_slot = r == 0 && sl < PF;
-    const unsigned tab0 = it.tab + (unsigned)(sl * 8);
+    const unsigned rd_off = (unsigned)((sl * kPartPitch + r) * 8);
     unsigned pcur = c.part + (unsigned)(lane * 8);            // emit buffer of the running batch (my column)
     unsigned pother = pcur + (unsigned)(PF * kRowB);
-    unsigned rprev = c.part + rd_off;                         // read base of the batch being summed
-    int kw_prev = -(1 << 30);                                 // no previous batch yet
+    unsigned rprev = c.part + (unsigned)(PF * kRowB) + rd_off;   // batch being summed (first: empty buffer -> dummy)
+    unsigned tprev = tab_dummy + (unsigned)(sl * 8);
     double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0, sa = 0.0, ta = 0.0;
-    bool oka = false;
 
 #pragma unroll 1
-    for (int blk = 0; blk < nblk; ++blk) {
+    for (int b = 0; b < nbat; ++b) {
 #pragma unroll
-        for (int u = 0; u < MB; ++u) {
-            if ((u + LA) % PF == 0) {
-                // the reads enter a new group: refill the group just left, then make sure the new one landed
-                const int g0 = ((u + LA - PF) % MB + MB) % MB;   // (compile-time after unrolling)
-                if (row_issue + PF <= rows_min) {
+        for (int u = 0; u < PF; ++u) {
+            if (u + LA == PF) {
+                // the reads enter the next group: refill the group just read, make sure the next one landed
 #pragma unroll
-                    for (int k = 0; k < PF; ++k) { cp_async8(fl + (unsigned)((g0 + k) * 256), xp); xp += rstride; }
-                } else {
-#pragma unroll
-                    for (int k = 0; k < PF; ++k) { cp_async8(fl + (unsigned)((g0 + k) * 256), xp, row_issue + k < rows_valid); xp += rstride; }
+                for (int j = 0; j < PF / 2; ++j) {
+                    cp_async16(cdst + gcur + (unsigned)(2 * j * 256), cp, row_issue < rows_valid);
+                    cp += cstride;
+                    row_issue += 2;
                 }
-                row_issue += PF;
                 cp_async_commit();
-                cp_async_wait<NBAT - 1>();
+                cp_async_wait<NG - 1>();
+                __syncwarp();                      // the pieces of a row come from 16 lanes
             }
-            xq[(u + LA) % XQ] = (F)lds64(fl + (unsigned)(((u + LA) % MB) * 256));
-            const F x = xq[u % XQ];
+            {
+                const int q = u + LA;              // row (of this batch) being read
+                const unsigned fb = (q & 1) ? fo : fe;
+                xq[q % XQ] = (F)lds64(q < PF ? fb + gcur + (unsigned)(q * 256) : fb + gnext + (unsigned)((q - PF) * 256));
+            }
+            const F xv = xq[u % XQ];
 #pragma unroll
-            for (int m = 0; m < MB; ++m) {
-                const int a = (u - m + MB) % MB;
-                if (m == 0) acc[a] = T[0] * x;                      // window gamma starts at this row
-                else acc[a] = fma(T[m], x, acc[a]);
-            }
-            sts64(pcur + (unsigned)((u % PF) * kRowB), (double)acc[(u + 1) % MB]);   // window gamma-(MB-1) complete
+            for (int m = MB - 1; m >= 1; --m) acc[m + 1] = fma(T[m], xv, acc[m]);
+            acc[1] = T[0] * xv;                                     // a window starts at this row
+            sts64(pcur + (unsigned)(u * kRowB), (double)acc[MB]);   // the window that took its last tap
             // column sums of the previous batch, one stage per row
-            if (u % PF == 0) {
+            if (u == 0) {
                 sa = (v0 + v1) + (v2 + v3);
                 v0 = lds64(rprev + 128); v1 = lds64(rprev + 160); v2 = lds64(rprev + 192); v3 = lds64(rprev + 224);
-            } else if (u % PF == 1) {
+            } else if (u == 1) {
                 sa += (v0 + v1) + (v2 + v3);
-            } else if (u % PF == 2) {
+            } else if (u == 2) {
                 sa += __shfl_xor_sync(0xffffffffu, sa, 1);
-            } else if (u % PF == 3) {
+            } else if (u == 3) {
                 sa += __shfl_xor_sync(0xffffffffu, sa, 2);
-                const int kw = kw_prev + sl;
-                oka = my_slot && kw >= 0 && kw < it.L && kw < it.nWt;
-                ta = oka ? lds64(tab0 + (unsigned)(kw_prev * 8)) : 0.0;
-            } else if (u % PF == 4) {
-                if (oka) sts64(tab0 + (unsigned)(kw_prev * 8), ta + sa);
-            }
-            if (u % PF == PF - 1) {                                 // batch complete: it becomes "previous"
-                __syncwarp();
-                rprev = (pcur - (unsigned)(lane * 8)) + rd_off;
-                v0 = lds64(rprev); v1 = lds64(rprev + 32); v2 = lds64(rprev + 64); v3 = lds64(rprev + 96);
-                kw_prev = blk * MB + (u - (PF - 1)) - (MB - 1);
-                const unsigned tmp = pcur; pcur = pother; pother = tmp;
+                ta = lds64(tprev);
+            } else if (u == 4) {
+                sts64(tprev, ta + sa);         // the four lanes of a slot store the same value
             }
         }
+        __syncwarp();                              // this batch's emit rows are complete
+        rprev = (pcur - (unsigned)(lane * 8)) + rd_off;
+        tprev = tab + (unsigned)((b * PF + sl) * 8);
+        v0 = lds64(rprev); v1 = lds64(rprev + 32); v2 = lds64(rprev + 64); v3 = lds64(rprev + 96);
+        { const unsigned tmp = pcur; pcur = pother; pother = tmp; }
+        gcur = gnext;
+        gnext = gnext + kGrpB == NG * kGrpB ? 0u : gnext + kGrpB;
     }
     // drain: the last batch's sums
     sa = (v0 + v1) + (v2 + v3);
@@ -525,11 +537,7 @@ __device__ __forceinline__ void march_pipe(const Cls& c, const It& it, const dou
     sa += (v0 + v1) + (v2 + v3);
     sa += __shfl_xor_sync(0xffffffffu, sa, 1);
     sa += __shfl_xor_sync(0xffffffffu, sa, 2);
-    {
-        const int kw = kw_prev + sl;
-        if (my_slot && kw >= 0 && kw < it.L && kw < it.nWt)
-            tab_add(tab0 + (unsigned)(kw_prev * 8), sa);
-    }
+    sts64(tprev, lds64(tprev) + sa);
     cp_async_wait<0>();
     __syncwarp();
 }
@@ -545,7 +553,7 @@ __device__ __forceinline__ double tmpl_lerp(const double* __restrict__ tm, int n
 
 // One march of the lanes' (segment, column) slots: taps, bounds, then the ring.
 //   seg/col: this lane's slot (active == false: an idle lane, zero taps);  row0: first row of seg.
-template <int MB, bool PIPE, bool NARROW, typename F, bool DUAL = false>
+template <int MB, bool NARROW, typename F, bool DUAL = false>
 __device__ __forceinline__ void run_march(const Cls& c, const It& it, const int n, const int n_tmpl,
                                           const double tscale, const double* __restrict__ tm,
                                           const double* __restrict__ x, const bool square,
@@ -571,7 +579,6 @@ __device__ __forceinline__ void run_march(const Cls& c, const It& it, const int 
     }
     const int rows_min = __reduce_min_sync(0xffffffffu, rows_valid);
     if constexpr (DUAL) march_dual<MB, F>(c, it, x + ebase, xw + ebase, rows_valid, rows_min, nblk, T, lane, best);
-    else if constexpr (PIPE) march_pipe<MB, F>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane);
     else march<MB, NARROW, F>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane, best);
 }
 
@@ -580,9 +587,9 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
                                           const double* __restrict__ tm, const double* __restrict__ x1,
                                           const double* __restrict__ x0, const int lane, Cand& best) {
     if (c.nWr <= 0) return;
-    It it;
-    it.tab = c.ctab;
     if constexpr (NARROW) {
+        It it;
+        it.tab = c.ctab;
         // ---- narrow: G segments side by side, one march over the whole class -------------------
         it.direct = c.stp == 1;   // (stp <= kChi2NarrowMax; dy not uniform: C and G in one march, rings <= 16)
         it.G = 32 / c.stp;
@@ -597,53 +604,70 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
         const int seg = min(lane / c.stp, it.G - 1);
         const int col = lane - seg * c.stp;      // idle lanes read on behind the last segment (zero taps)
         if constexpr (UNIFORM)
-            run_march<MB, false, true, F>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best);
+            run_march<MB, true, F>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best);
         else
-            run_march<MB, false, true, F, true>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best, x0);
-        return;
-    }
+            run_march<MB, true, F, true>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best, x0);
+    } else {
     // ---- wide: window tiles of the table size; the tile's stp columns are cut into nc balanced chunks of
-    // at most 32 lanes, one march per chunk over all rows of the tile (one segment per warp: a few idle
-    // lanes when stp is just above a multiple of 32, but no halo rows between segments and every march
-    // takes the pipelined path).
-    it.direct = false;
-    it.G = 0; it.KB = 0; it.SL = 0; it.SLn = 0; it.invSL = 0.f;
-    constexpr bool kPipe = PfRows<MB>::v >= 6;
-    const int nc = (c.stp + 31) >> 5;
-    const int cw = (c.stp + nc - 1) / nc;
-    for (int k0 = 0; k0 < c.nWr; k0 += c.Kt) {
-        const int nWt = min(c.Kt, c.nWr - k0);
-        it.L = nWt;
-        it.nWt = nWt;
-        for (int i = lane; i < (c.uniform ? nWt : c.Kt + nWt); i += 32) sts64(c.ctab + (unsigned)(i * 8), 0.0);
+    // at most 32 lanes, one shift march per chunk over all rows of the tile (one segment per warp: a few idle
+    // lanes when stp is just above a multiple of 32, but no halo rows between segments).  c.Kt = table
+    // entries per quantity: rows of the tile + kTabSlack dummy entries.
+    const int Lmax = c.Kt - kTabSlack - (MB - 1);        // windows per tile (Kt - kTabSlack is a multiple of 8)
+    const unsigned dummy = (unsigned)((c.Kt - kTabSlack) * 8);
+    const int nc = (c.stp + kChunkW - 1) / kChunkW;
+    const int cw = (c.stp + nc - 1) / nc;                // balanced chunks of at most 31 columns
+    const long long lim = (long long)n + c.D;            // x entries >= lim are never needed
+    for (int k0 = 0; k0 < c.nWr; k0 += Lmax) {
+        const int nWt = min(Lmax, c.nWr - k0);
+        const int nbat = (nWt + MB - 1 + kSPF - 1) / kSPF;
+        const int rows_all = nbat * kSPF + 3 * kSPF;     // rows ever requested by a march
+        for (int i = lane; i < nbat * kSPF; i += 32) {
+            sts64(c.ctab + (unsigned)(i * 8), 0.0);
+            if (!c.uniform) sts64(c.ctab + (unsigned)((c.Kt + i) * 8), 0.0);
+        }
         __syncwarp();
         for (int pass = 0; pass < (c.uniform ? 1 : 2); ++pass) {
-            it.tab = c.ctab + (unsigned)(pass * c.Kt * 8);
+            const unsigned tab = c.ctab + (unsigned)(pass * c.Kt * 8);
+            const double* __restrict__ x = pass == 0 ? x1 : x0;
             for (int ch = 0; ch < nc; ++ch) {
-                const int c0 = ch * cw;
-                const bool active = lane < cw && c0 + lane < c.stp;
-                const int col = c0 + lane;     // idle lanes read on behind the chunk (zero taps): the warp's
-                                               // copies stay one contiguous, conflict-free 256-byte row
-                run_march<MB, kPipe, false, F>(c, it, n, n_tmpl, tscale, tm, pass == 0 ? x1 : x0, pass == 1, active, k0,
-                                     col, lane, best);
+                const int col = ch * cw + lane;          // idle lanes (zero taps) read what the row copies bring
+                const bool active = lane < cw && col < c.stp;
+                F T[MB];                                 // taps: fp64 template, rounded once to F
+#pragma unroll
+                for (int m = 0; m < MB; ++m) {
+                    const int j = m * c.stp + col;
+                    double g = 0.0;
+                    if (active && j < c.D) g = tmpl_lerp(tm, n_tmpl, j, tscale);
+                    T[m] = (F)(pass == 1 ? g * g : g);
+                }
+                // rows whose first element is < lim are copied (32 doubles from the aligned start: they stay
+                // inside the period's pad + zero margin, k_durtab); later rows are zero-filled
+                const long long ebase0 = (long long)c.off + (long long)k0 * c.stp + ch * cw;
+                int rows_valid = 0;
+                if (ebase0 < lim) {
+                    const long long rv = (lim - ebase0 + c.stp - 1) / c.stp;
+                    rows_valid = rv > rows_all ? rows_all : (int)rv;
+                }
+                march_shift<MB, F>(c, tab, tab + dummy, x, ebase0, rows_valid, nbat, T, lane);
             }
         }
         __syncwarp();
-        score_wide(c, best, lane, k0, nWt);
+        score_wide(c, best, lane, k0, nWt, MB - 1);
         __syncwarp();
+    }
     }
 }
 
 template <int MB, bool NARROW, bool UNIFORM, typename F>
 __global__ void __launch_bounds__(kRT, 6) k_chi2_ring(TileArgs a, const int* __restrict__ list,
-                                                      const int* __restrict__ count) {
+                                                      const int* __restrict__ count, int* __restrict__ next) {
     extern __shared__ double dsm[];                 // per warp: emit buffer, X FIFO, window table
     __shared__ __align__(16) double s_tmpl[kTmplSmem];
     __shared__ __align__(8) unsigned long long s_mbar;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int n_mine = *count;                      // trials of this variant in the tile
-    if ((int)blockIdx.x * kRW >= n_mine) return;
+    if ((int)blockIdx.x * kRW >= n_mine) return;    // (more CTAs than trials)
     // ---- template nodes -> shared memory: one TMA bulk copy when size / alignment allow ------
     const bool tmpl_in_smem = a.n_tmpl <= kTmplSmem;
     const unsigned tbytes = (unsigned)a.n_tmpl * 8u;
@@ -670,10 +694,13 @@ __global__ void __launch_bounds__(kRT, 6) k_chi2_ring(TileArgs a, const int* __r
                          : "=r"(done) : "r"(mb) : "memory");
         }
     }
-    // ---- from here on every warp works alone on its own trial ------------------------------------
-    // (grid-stride over the variant's trial list: for short light curves the grid is capped at GTLS_GRID_WAVES
-    // waves of resident CTAs, see kGridCapMaxN; otherwise the loop runs once)
-    for (int li = (int)blockIdx.x * kRW + warp; li < n_mine; li += (int)gridDim.x * kRW) {
+    // ---- from here on every warp works alone: it takes the next trial of the variant's list from a
+    // device-wide counter (persistent CTAs, one wave: a warp is idle only when the list is empty) --------
+    for (;;) {
+    int li = 0;
+    if (lane == 0) li = atomicAdd(next, 1);
+    li = __shfl_sync(0xffffffffu, li, 0);
+    if (li >= n_mine) break;
     const int trial = list[li];
     const int pl = trial / a.n_dur;
     const DurEntry e = a.durtab[trial];
@@ -727,15 +754,16 @@ __global__ void __launch_bounds__(kRT, 6) k_chi2_ring(TileArgs a, const int* __r
 template <int MB, bool NARROW, bool UNIFORM, typename F>
 static void launch_variant_t(const TileArgs& a, int v, cudaStream_t st) {
     const long long trials = (long long)a.tile * a.n_dur;
-    unsigned grid = (unsigned)((trials + kRW - 1) / kRW);           // worst case; surplus CTAs exit at once
-    if (a.n <= kGridCapMaxN && grid > kGridCap) grid = kGridCap;
+    unsigned grid = (unsigned)((trials + kRW - 1) / kRW);           // surplus CTAs exit at once
+    if (grid > kGridCap) grid = kGridCap;                           // one wave of persistent CTAs
     const size_t sm = (size_t)(kRW * kWarpSmem) * sizeof(double);
     static bool set = false;
     if (!set) {
         cudaFuncSetAttribute(k_chi2_ring<MB, NARROW, UNIFORM, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
         set = true;
     }
-    k_chi2_ring<MB, NARROW, UNIFORM, F><<<grid, kRT, sm, st>>>(a, a.trial_list + (long long)v * trials, a.trial_count + v);
+    k_chi2_ring<MB, NARROW, UNIFORM, F><<<grid, kRT, sm, st>>>(a, a.trial_list + (long long)v * trials, a.trial_count + v,
+                                                             a.trial_count + kChi2Variants * (1 + kBinBlocks) + v);
 }
 // fp64 ring (default) or the fp32 in-transit variant (gtls_opts.chi2_fp32: taps, X and the ring
 // accumulators in fp32 -- at most 24 products per sum; column sums, prefix sums and scoring stay fp64)

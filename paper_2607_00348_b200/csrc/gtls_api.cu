@@ -113,8 +113,9 @@ Sizes workspace_sizes(long long n, long long n_per, int n_dur, double q_max, boo
     s.fixed = 3 * align_up(n * sizeof(double)) + align_up(sizeof(CurveInfo)) +
               align_up(sizeof(SdeScratch)) + align_up(2 * sizeof(unsigned long long)) +
               2 * align_up(n_per * sizeof(double)) + align_up(n_per * sizeof(gtls_best)) + 4096 +
-              align_up((size_t)kChi2Variants * (1 + kBinBlocks) * sizeof(int)) +
-              align_up(2 * (size_t)(pitch - n + 2) * sizeof(double));       // gtab: D <= pitch - n
+              align_up((size_t)kChi2Variants * (2 + kBinBlocks) * sizeof(int)) +
+              align_up(2 * (size_t)(pitch - n + 2) * sizeof(double)) +      // gtab: D <= pitch - n
+              2 * align_up(kXMargin * sizeof(double));
     s.per_period = 2 * n * sizeof(u64) + 256ull * nt * sizeof(u32) + n_dur * sizeof(DurEntry) +
                    n_dur * sizeof(Partial) + (size_t)kChi2Variants * n_dur * sizeof(int) +
                    n * sizeof(u32) + (4ull * kMaxBuckets + 3) * sizeof(u32) + 3ull * kMaxBuckets * sizeof(double) +
@@ -487,21 +488,15 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     a.gtab = gtab_dev; a.gtab_max = gtab_max;
     a.partial = ws.take<Partial>((size_t)tile * n_dur);
     a.trial_list = ws.take<int>((size_t)kChi2Variants * tile * n_dur);
-    a.trial_count = ws.take<int>((size_t)kChi2Variants * (1 + kBinBlocks));   // totals, then the per-CTA counts of k_bin_trials
-    a.x1 = ws.take<double>((size_t)tile * a.pitch);
+    a.trial_count = ws.take<int>((size_t)kChi2Variants * (2 + kBinBlocks));   // totals, the per-CTA counts of k_bin_trials, the trial queues
+    a.x1 = ws.take<double>((size_t)tile * a.pitch + kXMargin);      // + the last period's zero margin
     a.s1 = ws.take<double>((size_t)tile * a.spitch);
     if (!uniform) {
-        a.x0 = ws.take<double>((size_t)tile * a.pitch);
+        a.x0 = ws.take<double>((size_t)tile * a.pitch + kXMargin);
         a.s0 = ws.take<double>((size_t)tile * a.spitch);
     }
     if (!a.s1 || (!uniform && !a.s0)) return GTLS_ENOMEM;
 
-    // GTLS_CHI2_KERNEL=v1 / rows select the older chi2 kernels (debugging / A-B runs)
-    const char* kenv = getenv("GTLS_CHI2_KERNEL");
-    const bool use_v1 = kenv && strcmp(kenv, "v1") == 0;
-    const bool use_rows = kenv && strcmp(kenv, "rows") == 0;
-    a.dbg_min_st = getenv("GTLS_DBG_MIN_ST") ? atoi(getenv("GTLS_DBG_MIN_ST")) : 0;
-    a.dbg_max_st = getenv("GTLS_DBG_MAX_ST") ? atoi(getenv("GTLS_DBG_MAX_ST")) : 0x7fffffff;
     SdeScratch sc;
     unsigned long long counters[2];
     // ---- period tiles ----------------------------------------------------------------------
@@ -517,11 +512,11 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
         tm.mark(3);
         tm.mark(4);
         if (a.top_k > 0) launch_chi2_topk(a, st);
-        else if (use_v1) launch_chi2(a, st); else if (use_rows) launch_chi2_rows(a, st); else launch_chi2_ring(a, st);
+        else launch_chi2_ring(a, st);
         tm.mark(5);
         launch_reduce(a, d_chi2, d_best, d_counters, st);
         tm.mark(6);
-        stats.kernel_launches += launches + 2 + ((use_v1 || use_rows || a.top_k > 0) ? 1 : 2 + (uniform ? kChi2Variants - 1 : kChi2Variants - 3));   // k_bin_trials is two launches
+        stats.kernel_launches += launches + 2 + (a.top_k > 0 ? 1 : 2 + (uniform ? kChi2Variants - 1 : kChi2Variants - 3));   // k_bin_trials is two launches
         stats.chi2_launches += 1;
         if (o.stats) {
             CU(cudaStreamSynchronize(st));

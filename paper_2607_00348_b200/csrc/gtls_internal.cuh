@@ -44,6 +44,7 @@ struct CurveInfo {
 constexpr int kChi2Rings = 6;
 constexpr int kChi2Variants = 2 * kChi2Rings;
 constexpr int kBinBlocks = 148;      // CTAs of k_bin_trials; trial_count holds kChi2Variants * (1 + kBinBlocks) ints
+constexpr int kXMargin = 40;         // zeroed doubles behind every period's wrap pad in x1 / x0 (k_durtab; read by the ring kernels' row copies)
 constexpr int kChi2NarrowMax = 16;   // largest class stride handled by the narrow variants
 // Window classes of a trial with M = ceil(D/stride) taps: the smallest count that leaves at most 24 taps
 // per class when the class stride stays narrow (<= kChi2NarrowMax), at most 21 otherwise and when the
@@ -158,12 +159,11 @@ struct TileArgs {
     const int* seg_list;   // LSD path: periods (tile-local) to process, or nullptr = all of the tile
     const int* seg_count;  // number of entries of seg_list (device)
     int* trial_list;       // [kChi2Variants][tile*n_dur] trial indices binned by chi2 kernel variant
-    int* trial_count;      // [kChi2Variants] totals + [kBinBlocks][kChi2Variants] per-CTA counts
+    int* trial_count;      // [kChi2Variants] totals + [kBinBlocks][kChi2Variants] per-CTA counts + [kChi2Variants] trial queues
     int top_k;             // > 0: chi2 only at the K deepest starts of every trial (chi2_topk.cu, reading G19)
     int chi2_fp32;         // 1: fp32 ring arithmetic in the chi2 kernels (gtls_opts.chi2_fp32)
     const double* gtab;    // [2*(gtab_max+1)] sum g_D, sum g_D^2 for D = 1 .. gtab_max (k_gtab)
     int gtab_max;
-    int dbg_min_st, dbg_max_st;   // timing experiments only (GTLS_DBG_MIN_ST / GTLS_DBG_MAX_ST): skip other trials
 };
 
 // Arguments of the fused fold / bucket sort / gather / scan fast path (bucket_sort.cu).
@@ -216,8 +216,6 @@ void launch_fold_keys(const TileArgs& a, double* phase_out, cudaStream_t st);
 u64* launch_phase_sort(const TileArgs& a, cudaStream_t st, int* n_launches);
 void launch_gather_scan(const TileArgs& a, const u64* sorted, double* x2, double* s2,
                         int pad_override, cudaStream_t st);
-void launch_chi2(const TileArgs& a, cudaStream_t st);        // v1: warp per window (fallback / A-B)
-void launch_chi2_rows(const TileArgs& a, cudaStream_t st);   // register-tiled rows kernel (A-B)
 void launch_chi2_ring(const TileArgs& a, cudaStream_t st);   // register-ring correlation kernel (default)
 // counters[0] += windows of all trials, counters[1] += sum of D over evaluated windows
 void launch_reduce(const TileArgs& a, double* out_chi2, gtls_best* out_best,

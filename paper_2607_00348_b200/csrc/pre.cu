@@ -119,8 +119,19 @@ __global__ void __launch_bounds__(256) k_durtab(TileArgs a) {
     const int pl = tr / a.n_dur, jd = tr % a.n_dur;
     const double* qrow = a.dur_per_period ? a.durs + (a.p0 + pl) * (long long)a.n_dur : a.durs;
     const int D = points_in_duration(qrow[jd], a.n);
-    int skip = 0;
-    for (int k = 0; k < jd; ++k) skip |= (points_in_duration(qrow[k], a.n) == D);
+    int skip = 0, dmax = D;
+    for (int k = 0; k < jd; ++k) {
+        const int Dk = points_in_duration(qrow[k], a.n);
+        skip |= (Dk == D);
+        dmax = max(dmax, Dk);
+    }
+    if (jd == a.n_dur - 1 && a.x1) {
+        // zero margin behind the period's wrap pad (written later by the sort stage, up to n + dmax): the
+        // ring kernels copy whole 32-double row windows, which may reach kXMargin entries past the pad
+        double* m1 = a.x1 + (long long)pl * a.pitch + a.n + dmax;
+        for (int i = 0; i < kXMargin; ++i) m1[i] = 0.0;
+        if (!a.uniform) { double* m0 = a.x0 + (long long)pl * a.pitch + a.n + dmax; for (int i = 0; i < kXMargin; ++i) m0[i] = 0.0; }
+    }
     double sg = 0.0, sg2 = 0.0;
     if (!skip) {
         if (D <= a.gtab_max) { sg = a.gtab[2 * D]; sg2 = a.gtab[2 * D + 1]; }
@@ -143,7 +154,7 @@ __global__ void __launch_bounds__(256) k_durtab(TileArgs a) {
 
 // chi2 variant of one trial (see chi2_ring.cu): classes of at most 21 taps, ring size, narrow/wide.
 __device__ __forceinline__ int chi2_variant(const DurEntry& e, const TileArgs& a) {
-    if (e.skip || e.stride < a.dbg_min_st || e.stride > a.dbg_max_st) return -1;
+    if (e.skip) return -1;
     const int M = (e.D + e.stride - 1) / e.stride;
     const int ncls = chi2_classes(M, e.stride, a.uniform != 0);
     const int stp = ncls * e.stride;
@@ -203,7 +214,10 @@ __global__ void __launch_bounds__(256) k_bin_trials(TileArgs a) {
             if (lane < 8) s_warp[v][lane] = x - c;
             if (lane == 7) {
                 if (PHASE == 0) block_counts[blockIdx.x * kChi2Variants + v] = x;
-                else if (blockIdx.x == gridDim.x - 1) a.trial_count[v] = s_base[v] + x;
+                else if (blockIdx.x == gridDim.x - 1) {
+                    a.trial_count[v] = s_base[v] + x;
+                    a.trial_count[kChi2Variants * (1 + kBinBlocks) + v] = 0;     // the variant's trial queue (chi2_ring.cu)
+                }
             }
         }
     }
