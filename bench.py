@@ -211,6 +211,20 @@ def run_survey(args, g, torch, devname):
             "clocks": clocks}
 
 
+def chi2_stage_traffic(workload, period_tile):
+    """DRAM bytes of the chi2 stage of one period tile, read from the committed ncu summary
+    profiles/chi2_stage_traffic.csv (columns: workload, period_tile, dram_bytes, capture); None when
+    no capture of this workload / tile size is on file."""
+    path = os.path.join(ROOT, "profiles", "chi2_stage_traffic.csv")
+    if workload is None or not os.path.exists(path):
+        return None, "no ncu capture of this workload and tile size on file (profiles/chi2_stage_traffic.csv)"
+    for ln in open(path).read().splitlines()[1:]:
+        f = [x.strip() for x in ln.split(",")]
+        if len(f) >= 4 and f[0] == workload and int(f[1]) == int(period_tile):
+            return float(f[2]), f"profiles/chi2_stage_traffic.csv: {f[3]}"
+    return None, "no ncu capture of this workload and tile size on file (profiles/chi2_stage_traffic.csv)"
+
+
 def max_over_ranks(x: float, world: int, device="cpu") -> float:
     """Multi-rank runs (replicas only): the job time is the slowest rank's."""
     if world <= 1:
@@ -243,6 +257,9 @@ def main():
     ap.add_argument("--every", type=int, default=1,
                     help="profiling aid: search only every k-th period of the workload (default 1 = the "
                          "full workload; any other value is named in config.workload)")
+    ap.add_argument("--peak-fp64", type=float, default=0.0, metavar="SECONDS",
+                    help="measure the fp64 FMA rate of this GPU (gtls_peak_fp64: register-only DFMA kernel) as a "
+                         "0.1 s burst and sustained over SECONDS, with the clocks seen; prints one JSON line")
     ap.add_argument("--survey", type=int, default=0,
                     help="survey mode (BASELINE.json config 5): search this many c5 curves per step with one "
                          "gtls_search_batch call and report curves/s beside trials/s")
@@ -270,6 +287,25 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(devname))
     g.load_library()
+
+    if args.peak_fp64 > 0:
+        if rank == 0:
+            peaks, peak_src = measured_peaks()
+            sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+            burst = g.gtls_peak_fp64(0.1, device=local_rank)
+            time.sleep(1.0)
+            sampler = ClockSampler(local_rank)
+            sampler.start()
+            time.sleep(1.0)
+            sampler.mark()
+            sus = g.gtls_peak_fp64(args.peak_fp64, device=local_rank)
+            clocks = sampler.stop()
+            print(json.dumps({"metric": "fp64 FMA rate (register-only DFMA kernel, 16 warps/SM)", "unit": "TFLOP/s",
+                              "burst_0.1s": burst["tflops"], "sustained": sus["tflops"], "sustained_seconds": sus["ms"] / 1e3,
+                              "derived_peak": SM_COUNT * DFMA_PER_CLK_PER_SM * 2 * sm_max * 1e6 / 1e12,
+                              "derived_from": f"{SM_COUNT} SMs x {DFMA_PER_CLK_PER_SM} DFMA/clk x 2 flop x {sm_max:.0f} MHz ({peak_src})",
+                              "clocks_during_sustained": clocks}), flush=True)
+        return 0
 
     if args.survey > 0:
         if rank == 0:
@@ -299,15 +335,12 @@ def main():
         res = step()
     barrier()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    st_acc = {}
     barrier()
     sampler.mark()
     ev0.record()
     for _ in range(args.steps):
         flush.zero_()                                   # L2 flush between timed iterations
-        res = step(stats=True)
-        for k, v in res.stats.items():
-            st_acc[k] = st_acc.get(k, 0) + v if k.startswith("ms_") or k.endswith("launches") else v
+        res = step()                                    # no per-stage events, no per-tile host syncs
     ev1.record()
     barrier()
     clocks = sampler.stop()
@@ -315,6 +348,10 @@ def main():
     ms_total = max_over_ranks(ms_total, world, devname)
     ms_step = ms_total / args.steps
     value = world * w.trials / (ms_step / 1e3)
+    # stage split, window counters and the roofline of the chi2 stage: ONE more step of the same workload
+    # with the library's per-stage CUDA events on (one stream synchronisation per period tile), untimed
+    flush.zero_()
+    st_acc = dict(step(stats=True).stats)
 
     out = None
     if rank == 0:
@@ -322,7 +359,7 @@ def main():
         # ---- roofline of the dominant kernel (in-transit chi2, fp64 FMA pipe) -------------------
         chi2_ms_per_launch = st_acc["ms_chi2"] / max(1, st_acc["chi2_launches"])
         flop_per_wp = 2.0 if st_acc["uniform_dy"] else 4.0          # 1 or 2 DFMA per window point
-        flops_per_launch = st_acc["window_points"] * flop_per_wp / max(1, st_acc["chi2_launches"] / args.steps)
+        flops_per_launch = st_acc["window_points"] * flop_per_wp / max(1, st_acc["chi2_launches"])
         achieved = flops_per_launch / (chi2_ms_per_launch * 1e-3) / 1e12
         sm_max = float(peaks.get("sm_max_mhz", 1965.0))
         peak = SM_COUNT * DFMA_PER_CLK_PER_SM * 2 * sm_max * 1e6 / 1e12
@@ -331,17 +368,20 @@ def main():
         # 4144-period tile of c4 (profiles/r1_F_final_c4e64.md: the first tile of the every-64th-period
         # subsample, periods spread over the longer 63 % of the grid; the full run's tiles are 4144
         # consecutive periods of the same kernels).  Other workloads / tile sizes have no capture: null
-        traffic = 9.12e10 if (args.workload == "c4" and args.dt0 is None and st_acc["period_tile"] == 4144) else None
+        traffic, traffic_src = chi2_stage_traffic(args.workload if args.dt0 is None and args.every == 1 else None,
+                                                   st_acc["period_tile"])
         roofline = {"bound": "alu", "kernel": "k_chi2_ring (in-transit chi2, a5-a8; one 'launch' = the chi2 stage of one period tile: trial binning + the ring-kernel variants)", "achieved": achieved,
                     "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
-                    "traffic_unit": "bytes per launch (ncu dram read + write, profiles/r1_F_final_c4e64.md)",
+                    "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum over the stage's kernels)",
+                    "traffic_source": traffic_src,
                     "peak_source": f"derived: {SM_COUNT} SMs x {DFMA_PER_CLK_PER_SM} DFMA/clk x 2 flop x "
-                                   f"{sm_max:.0f} MHz ({peak_src} sm_max_mhz); a dependent-chain DFMA microbenchmark on this "
-                                   f"pool sustains 34.1 TFLOP/s",
+                                   f"{sm_max:.0f} MHz ({peak_src} sm_max_mhz); measured beside it: `bench.py --peak-fp64` "
+                                   f"(register-only DFMA kernel), line kept in profiles/r2_peak_fp64.md",
+                    "measured_from": "one untimed step of the same workload with per-stage CUDA events (gtls_stats)",
                     "algorithmic_flops_per_launch": flops_per_launch,
                     "ms_per_launch": chi2_ms_per_launch,
                     "share_of_step": st_acc["ms_chi2"] / max(1e-9, st_acc["ms_total"])}
-        stages = {k: st_acc[k] / args.steps for k in st_acc if k.startswith("ms_")}
+        stages = {k: st_acc[k] for k in st_acc if k.startswith("ms_")}
         hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
         pp = float(st_acc["period_points"])
         # fold + sort + gather + scan are one fused stage (bucket_sort.cu); algorithmic HBM bytes per
@@ -365,7 +405,7 @@ def main():
                        "multi_gpu": "one independent light curve per rank, no collective"},
             "s_per_light_curve": ms_step / 1e3,
             "clocks": clocks,
-            "gpu_launches": int(st_acc["kernel_launches"]),
+            "gpu_launches": int(st_acc["kernel_launches"]) * args.steps,
             "stage_ms_per_step": stages, "stage_bandwidth": stage_roof,
             "roofline": roofline,
             "summary": res.summary,
@@ -396,6 +436,7 @@ def main():
                           "d2h_bytes_per_step": d2h, "ms_per_step": dt * 1e3, "steps": n_e2e,
                           "note": "gtls_search with host pointers: H2D + search + D2H per call; device blocks up to 8 GiB come from the library's pool after the warm-up call, larger ones are cudaMalloc'ed per call"}
 
+    parity_ok = True
     if rank == 0:
         if not args.no_cpu_baseline:
             import oracle
@@ -408,10 +449,23 @@ def main():
                 "value": sample.trials / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                 "sample": f"every {every}th period of {w.name} ({sample.n_per} of {w.n_per} periods), {dt:.1f} s",
                 "s_per_light_curve_extrapolated": w.trials / (sample.trials / dt)}
-            # parity spot check on the sample while we are here (not timed)
+            # parity spot check on the sample while we are here (not timed): chi2 within 1e-9 relative and the
+            # best (duration, start) indices identical wherever the oracle's runner-up gap is above 1e-12 chi2
             got = np.asarray(res.chi2.cpu())[::every][:sample.n_per]
-            out["cpu_baseline"]["chi2_max_rel_err_vs_gpu"] = float(np.max(np.abs(got - ro.chi2) / ro.chi2))
+            gb = res.best()[::every][:sample.n_per]
+            rel = float(np.max(np.abs(got - ro.chi2) / ro.chi2))
+            strict = ro.gap > 1e-12 * np.abs(ro.chi2)
+            mism = (gb["dur_idx"] != ro.best["dur_idx"]) | (gb["start"] != ro.best["start"])
+            t0_ok = bool(np.array_equal(gb["t0"][~mism], ro.best["t0"][~mism]))
+            out["cpu_baseline"]["chi2_max_rel_err_vs_gpu"] = rel
+            out["cpu_baseline"]["index_mismatches_vs_gpu"] = int(np.sum(mism & strict))
+            out["cpu_baseline"]["near_tie_periods"] = int(np.sum(~strict))
+            parity_ok = rel <= 1e-9 and not np.any(mism & strict) and t0_ok
+            out["cpu_baseline"]["parity_spot_check"] = "ok" if parity_ok else "FAILED"
         print(json.dumps(out), flush=True)
+        if not args.no_cpu_baseline and not parity_ok:
+            log("bench.py: parity spot check against the oracle FAILED")
+            return 1
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()

@@ -260,6 +260,16 @@ size_t gtls_workspace_bytes(int64_t n, int64_t n_per, int32_t n_dur, const gtls_
  * them.  Caller-owned memory is never retained. */
 void gtls_release_cache(void);
 
+/* Measurement aid (bench.py --peak-fp64), not part of the search: runs a register-only fp64 FMA kernel
+ * (16 independent chains per thread, three distinct register operands per DFMA, 16 warps per SM) back to
+ * back on opts->stream for about `seconds` (0 < seconds <= 60) of device time and returns the sustained
+ * rate in TFLOP/s (2 flop per FMA lane) in *out_tflops; *out_ms (may be NULL) = device time measured with
+ * CUDA events, *out_launches (may be NULL) = kernel launches timed.  This is the measured denominator
+ * beside the derived fp64 peak of the chi2 stage's roofline ("measure it first
+ * with a dependent-DFMA microbenchmark").  Uses opts->device and opts->stream only; synchronises. */
+int gtls_peak_fp64(double seconds, const gtls_opts* opts, double* out_tflops, double* out_ms,
+                   int64_t* out_launches);
+
 const char* gtls_strerror(int code);
 const char* gtls_version(void);
 /* Text of the last CUDA error seen by the calling thread ("" if none). */

@@ -22,7 +22,7 @@ import numpy as np
 
 __all__ = ["gtls_search", "gtls_search_two_stage", "gtls_search_batch", "gtls_batch_workspace_bytes",
            "gtls_period_grid_size", "gtls_period_grid", "gtls_duration_grid", "BatchResult", "gtls_search_sharded", "gtls_fold_sort", "gtls_fold_scan", "gtls_window_chi2", "gtls_sde",
-           "gtls_workspace_bytes", "gtls_release_cache", "gtls_strerror", "gtls_version", "GtlsError", "SearchResult",
+           "gtls_workspace_bytes", "gtls_release_cache", "gtls_peak_fp64", "gtls_strerror", "gtls_version", "GtlsError", "SearchResult",
            "BEST_DTYPE", "lib_path", "load_library"]
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
@@ -127,6 +127,9 @@ def load_library():
     lib.gtls_batch_workspace_bytes.restype = C.c_size_t
     lib.gtls_workspace_bytes.argtypes = [C.c_int64, C.c_int64, C.c_int32, C.POINTER(GtlsOpts)]
     lib.gtls_workspace_bytes.restype = C.c_size_t
+    lib.gtls_peak_fp64.argtypes = [C.c_double, C.POINTER(GtlsOpts), C.POINTER(C.c_double), C.POINTER(C.c_double),
+                                   C.POINTER(C.c_int64)]
+    lib.gtls_peak_fp64.restype = C.c_int
     lib.gtls_release_cache.argtypes = []
     lib.gtls_release_cache.restype = None
     lib.gtls_strerror.argtypes = [C.c_int]
@@ -212,6 +215,20 @@ def gtls_version() -> str:
 def gtls_release_cache() -> None:
     """Free the device blocks the library keeps between calls (``gtls_release_cache`` in include/gtls.h)."""
     load_library().gtls_release_cache()
+
+
+def gtls_peak_fp64(seconds: float, device: int = 0, stream: int = 0) -> dict:
+    """fp64 FMA microbenchmark (``gtls_peak_fp64`` in include/gtls.h): sustained TFLOP/s over `seconds`."""
+    lib = load_library()
+    o = GtlsOpts()
+    lib.gtls_opts_default(C.byref(o))
+    o.device = int(device)
+    o.stream = int(stream)
+    tf, ms, nl = C.c_double(0.0), C.c_double(0.0), C.c_int64(0)
+    rc = lib.gtls_peak_fp64(float(seconds), C.byref(o), C.byref(tf), C.byref(ms), C.byref(nl))
+    if rc != GTLS_OK:
+        raise GtlsError(rc, "gtls_peak_fp64")
+    return {"tflops": tf.value, "ms": ms.value, "launches": nl.value}
 
 
 def gtls_strerror(code: int) -> str:

@@ -50,6 +50,7 @@ constexpr int kFifoRows = 24;            // >= kFifoBatches * max PfRows
 constexpr int kCW = 704;                 // window-table doubles per warp (>= 32 * 21)
 constexpr int kTmplSmem = 512;           // template nodes cached in shared memory
 constexpr unsigned kGridCap = 148u * 6u;   // CTAs per launch: the 6 resident CTAs per SM, persistent (dynamic trial queue)
+constexpr unsigned kGridCapWide = 148u * 4u;
 constexpr int kWarpSmem = kPartRows * kPartPitch + kFifoRows * 32 + kCW;   // doubles per warp
 
 struct Cand { double d; double depth; int s; int has; };
@@ -756,6 +757,10 @@ static void launch_variant_t(const TileArgs& a, int v, cudaStream_t st) {
     const long long trials = (long long)a.tile * a.n_dur;
     unsigned grid = (unsigned)((trials + kRW - 1) / kRW);           // surplus CTAs exit at once
     if (grid > kGridCap) grid = kGridCap;                           // one wave of persistent CTAs
+    // wide variants: 4 of the 6 CTA slots per SM.  The shift march hides its latencies inside a warp (8 warps per SM
+    // run within 1 % of 12), and fewer trials in flight are fewer periods whose x1 competes for the L2
+    // (c4: 60 -> 36 GB of DRAM reads per 4144-period tile of the dominant variant, SM clock under the power cap 1845 -> 1890 MHz)
+    if (!NARROW && grid > kGridCapWide) grid = kGridCapWide;
     const size_t sm = (size_t)(kRW * kWarpSmem) * sizeof(double);
     static bool set = false;
     if (!set) {

@@ -48,6 +48,9 @@ __global__ void __launch_bounds__(kRedThreads) k_sde_stats(const double* __restr
     if (threadIdx.x == 0) {
         for (int k = 1; k < (int)(blockDim.x >> 5); ++k)
             if (s_val[k] < mv || (s_val[k] == mv && s_idx[k] < mi)) { mv = s_val[k]; mi = s_idx[k]; }
+        // no value compared below +inf (every chi2 is NaN or +inf): a degenerate spectrum whose argmin is
+        // the first period, so that nothing downstream indexes with the sentinel
+        if (mi == 0x7fffffffffffffffLL) { mi = 0; mv = __longlong_as_double(0x7ff8000000000000LL); }
         s_bcast[0] = mv;
         sc->chi2_min = mv; sc->argmin = mi;
     }

@@ -24,12 +24,14 @@ __global__ void __launch_bounds__(1024) k_curve_pre(const double* __restrict__ t
     int bad = 0;
     for (int i = threadIdx.x; i < n; i += blockDim.x) {
         const double ti = t[i], yi = y[i], di = dy[i];
-        const bool ok = isfinite(ti) && isfinite(yi) && isfinite(di) && di > 0.0;
-        bad += ok ? 0 : 1;
         const double wi = __ddiv_rn(1.0, di * di);     // w_i = 1/dy_i^2
         const double ri = 1.0 - yi;                    // flux deficit (model == 1)
         const double wri = wi * ri;
         const double wr2i = wri * ri;
+        // dy so small that dy^2 underflows gives w = inf and w r = NaN: rejected like a non-finite input
+        const bool ok = isfinite(ti) && isfinite(yi) && isfinite(di) && di > 0.0 && isfinite(wi) && isfinite(wri) &&
+                        isfinite(wr2i);
+        bad += ok ? 0 : 1;
         w[i] = wi; wr[i] = wri; wr2[i] = wr2i;
         acc += wr2i;
         wmin = fmin(wmin, wi); wmax = fmax(wmax, wi);

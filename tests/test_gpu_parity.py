@@ -21,14 +21,21 @@ def _cuda():
     return torch
 
 
-def _check_search(w, res, ora, sde_kernel=151, label=""):
+def _check_search(w, res, ora, sde_kernel=151, label="", expect_near_ties=0):
     chi2 = np.asarray(res.chi2)
     best = res.best()
     rel = np.abs(chi2 - ora.chi2) / np.maximum(np.abs(ora.chi2), 1e-300)
     assert rel.max() <= CHI2_RTOL, f"{label}: chi2 rel err {rel.max():.3e}"
     # near-tie rule: where the oracle's best / runner-up gap is below 1e-12 chi2
-    # either candidate is valid; everywhere else indices must match exactly
+    # either candidate is valid; everywhere else indices must match exactly.  The number of such
+    # periods is part of the test (SURVEY: "report the count, expected 0"): a runner-up that the
+    # oracle reported too close to its best would make the index check vacuous.  `gap` itself is
+    # pinned on the CPU (tests/test_oracle_chi2.py).
     strict = ora.gap > 1e-12 * np.abs(ora.chi2)
+    n_near = int((~strict).sum())
+    print(f"{label}: {n_near} of {strict.size} periods with a best / runner-up gap below 1e-12 chi2; "
+          f"min rel gap {np.min(ora.gap / np.abs(ora.chi2)):.2e}; chi2 max rel err {rel.max():.2e}")
+    assert n_near == expect_near_ties, f"{label}: {n_near} near-tie periods, expected {expect_near_ties}"
     mism = (best["dur_idx"] != ora.best["dur_idx"]) | (best["start"] != ora.best["start"])
     assert not np.any(mism & strict), f"{label}: {np.sum(mism & strict)} index mismatches"
     ok = ~mism
@@ -164,6 +171,53 @@ def test_search_c1_full():
     assert res.code == 0 and res.stats["uniform_dy"] == 1
     # recovered the injected planet (P3 on the GPU path)
     assert abs(res.summary["best_period"] - w.lc.meta["period"]) < 0.01
+
+
+def test_search_c2_full():
+    """SURVEY.md section 4 tier T3: configs 1-2 in full (10 483 periods x 25 durations, every window)."""
+    _cuda()
+    w = gi.make_workload(2)
+    ora = oracle.search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05)
+    res = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05, stats=True)
+    _check_search(w, res, ora, label="c2")
+
+
+@pytest.mark.timeout(1500)
+def test_search_c4_one_full_automatic_tile():
+    """The 3000-day curve on 4144 + 600 CONSECUTIVE periods from the middle of the Ofir grid: one full
+    automatic period tile (period_tile == 4144, the launch configuration bench.py times: 124 320 trials
+    binned per tile, the persistent ring-kernel grids, the side stream, 592 resident k_bucket_finish
+    CTAs) plus a ragged second tile, every chi2, index, t0 and depth against the oracle."""
+    _cuda()
+    w0 = gi.make_workload(4)
+    p0 = 150_000
+    sel = slice(p0, p0 + 4144 + 600)
+    w = gi.Workload(f"c4[{p0}:{p0 + 4744}]", w0.lc, np.ascontiguousarray(w0.periods[sel]),
+                    np.ascontiguousarray(w0.durations[sel]), w0.tmpl, w0.dt0)
+    res = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05, sde_kernel=151,
+                        stats=True)
+    assert res.stats["period_tile"] == 4144
+    ora = oracle.search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05)
+    _check_search(w, res, ora, sde_kernel=151, label=w.name)
+
+
+def test_sde_epilogue_at_full_grid_scale():
+    """the GPU's full chi2(P) array of a long curve (c3: 200 995 periods) fed to
+    the oracle's SDE routine; SDE within 1e-6 absolute, both argmaxes identical.  (The single-CTA
+    reductions of k_sde_stats are what could drift at this size.)"""
+    _cuda()
+    w = gi.make_workload(3)
+    res = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05, sde_kernel=151)
+    chi2 = np.asarray(res.chi2)
+    assert chi2.size > 200_000 and np.all(np.isfinite(chi2))
+    s = oracle.sde(chi2, 151)
+    assert np.abs(np.asarray(res.sde_raw) - s.sde_raw).max() <= SDE_ATOL
+    assert np.abs(np.asarray(res.sde) - s.sde).max() <= SDE_ATOL
+    assert res.summary["best_period_idx"] == s.best_period_idx == int(np.argmin(chi2))
+    assert res.summary["sde_argmax"] == s.sde_argmax
+    assert abs(res.summary["sde_max"] - s.sde.max()) <= SDE_ATOL
+    # and the injected period is where the spectrum peaks (P3 at scale)
+    assert abs(res.summary["best_period"] - w.lc.meta["period"]) < 0.5
 
 
 @pytest.mark.parametrize("cfg,every,hetero,dt0", [
@@ -324,9 +378,20 @@ def test_fp32_in_transit_variant(cfg, every, hetero):
     assert rel <= 1e-6, rel
     b = res.best()
     same = (b["dur_idx"] == ora.best["dur_idx"]) & (b["start"] == ora.best["start"])
-    assert same.mean() >= 0.99
+    # explicit near-tie predicate instead of a quota: wherever the fp32 variant chose another window,
+    # the fp64 chi2 of THAT window (the oracle's literal per-window export) lies within the variant's
+    # asserted error (1e-6 chi2, twice: both candidates carry it) of the oracle's minimum
+    for ip in np.flatnonzero(~same):
+        q = w.durations[ip, b["dur_idx"][ip]] if w.durations.ndim == 2 else w.durations[b["dur_idx"][ip]]
+        st, _, c_out, c_in = oracle.window_chi2_literal(w.lc.t, w.lc.y, w.lc.dy, w.periods[ip], q, w.tmpl, 0.05)
+        k = np.flatnonzero(st == b["start"][ip])
+        assert k.size == 1, (ip, "the chosen start is not a trial position of that duration")
+        assert (c_out + c_in)[k[0]] - ora.chi2[ip] <= 2e-6 * ora.chi2[ip], ip
+    print(f"fp32 variant: {int((~same).sum())} of {same.size} periods chose another (near-tie) window; chi2 max rel err {rel:.2e}")
     s = oracle.sde(ora.chi2, 31)
     assert res.summary["best_period_idx"] == s.best_period_idx and same[s.best_period_idx]
+    # SDE tolerance of the fp32 variant (a reading of this build: north_star states only
+    # chi2 1e-4 for an fp32 variant): chi2 rel 1e-6 -> SR rel 1e-6 -> SDE_raw abs ~1e-6 / sigma_SR <= 1e-3
     assert np.abs(np.asarray(res.sde) - s.sde).max() <= 1e-3
 
 
@@ -349,12 +414,39 @@ def test_top_k_pruning_variant(cfg, every, hetero, dt0, k):
     ok = np.abs(chi2 - ora.chi2) <= CHI2_RTOL * ora.chi2
     b = res.best()
     same = (b["dur_idx"] == ora.best["dur_idx"]) & (b["start"] == ora.best["start"])
-    assert ok.mean() >= 0.99 and same.mean() >= 0.99, (ok.mean(), same.mean())
     assert np.all(ok[same])
+    # explicit near-tie predicate instead of a quota: a period may differ only if, for one of its
+    # durations, the K-th and (K+1)-th deepest running means (direct sums, oracle side) agree to 1e-12
+    for ip in np.flatnonzero(~(ok & same)):
+        assert _topk_boundary_gap(w, ip, k, dt0) <= 1e-12, (ip, "differs without a selection-boundary tie")
+    print(f"top_k={k}: {int((~(ok & same)).sum())} of {same.size} periods differ at a selection-boundary tie")
     assert res.summary["windows_evaluated"] == ora.windows
     # pruning can only raise chi2 relative to the full search (the K starts are among all starts)
     full = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=dt0, sde_kernel=31)
     assert np.all(chi2 >= np.asarray(full.chi2) * (1 - 1e-12))
+
+
+def _topk_boundary_gap(w, ip, k, dt0):
+    """Smallest relative gap, over the durations of period ip, between the K-th and (K+1)-th largest
+    running-mean deficit over all strided starts (plain numpy direct sums on the oracle's permutation)."""
+    n = w.lc.n
+    _, perm = oracle.fold_sort(w.lc.t, [w.periods[ip]], want_phase=False)
+    sig = perm[0]
+    wt = (1.0 / w.lc.dy ** 2)[sig]
+    wr = wt * (1.0 - w.lc.y)[sig]
+    qrow = w.durations[ip] if w.durations.ndim == 2 else w.durations
+    worst = np.inf
+    for q in qrow:
+        d = oracle.points_in_duration(q, n)
+        st = max(1, int(np.floor(d * dt0))) if dt0 > 0 else 1
+        starts = np.arange(0, n, st)
+        if starts.size <= k:
+            continue
+        idx = (starts[:, None] + np.arange(d)[None, :]) % n
+        rbar = wr[idx].sum(axis=1) / wt[idx].sum(axis=1)
+        r = np.sort(rbar)[::-1]
+        worst = min(worst, abs(r[k - 1] - r[k]) / max(np.abs(r).max(), 1e-300))
+    return worst
 
 
 def test_tiny_and_degenerate_inputs(tmpl512):
@@ -415,14 +507,40 @@ def test_sde_epilogue_matches_oracle(kernel, n):
     assert abs(summ["sde_max"] - s.sde.max()) <= 1e-9
 
 
-def test_v1_kernel_still_matches(monkeypatch):
-    """The simple warp-per-window chi2 kernel (GTLS_CHI2_KERNEL=v1) stays a valid A/B path."""
+def test_lsd_sort_path_passes_the_core_parity_subset():
+    """GTLS_SORT=lsd sends every period through the LSD radix path (fold_sort.cu + scan.cu, normally the
+    fallback for clustered phases).  The switch is read once per process, so the subset runs in a child
+    process: fold/sort bit-exactness, prefix sums, and searches with uniform and per-point errors."""
     _cuda()
-    monkeypatch.setenv("GTLS_CHI2_KERNEL", "v1")
-    w = gi.make_workload(2, hetero=True).subset(257)
-    ora = oracle.search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05)
-    res = g.gtls_search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05, sde_kernel=5)
-    _check_search(w, res, ora, sde_kernel=5, label="v1")
+    import os
+    import subprocess
+    import sys
+    env = dict(os.environ, GTLS_SORT="lsd")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-m", "pytest", os.path.join(root, "tests", "test_gpu_parity.py"), "-q", "-x",
+                        "-m", "gpu", "-p", "no:cacheprovider", "-k",
+                        "fold_sort_bit_exact or prefix_sums or search_subsets or ties_and_tiny or tiny_and_degenerate"],
+                       env=env, cwd=root, capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, r.stdout[-3000:] + r.stderr[-2000:]
+    assert " passed" in r.stdout
+
+
+def test_non_finite_weights_and_all_nan_spectrum(tmpl512):
+    """dy so small that 1/dy^2 overflows must be rejected up front (GTLS_ENONFINITE), and an
+    all-NaN chi2 array handed to gtls_sde must come back as a degenerate spectrum, not as an
+    out-of-bounds index on the device."""
+    _cuda()
+    t = np.linspace(0, 10, 60); y = np.ones(60); y[5] = 0.999
+    with pytest.raises(g.GtlsError) as e:
+        g.gtls_search(t, y, np.full(60, 1e-170), np.array([1.0, 2.0]), np.array([0.1]), tmpl512)
+    assert e.value.code == -2
+    raw, sde, summ, code = g.gtls_sde(np.full(500, np.nan), sde_kernel=31)
+    assert code == -6 and summ["best_period_idx"] == 0 and np.all(sde == 0) and np.all(raw == 0)
+    raw, sde, summ, code = g.gtls_sde(np.concatenate([[np.nan] * 5, 4000.0 + np.arange(200.0)]), sde_kernel=31)
+    assert 0 <= summ["best_period_idx"] < 205
+    # the context survived: a normal call still works
+    raw, sde, summ, code = g.gtls_sde(4000.0 + np.cos(np.arange(300.0)), sde_kernel=31)
+    assert code == 0 and np.all(np.isfinite(sde))
 
 
 def test_period_sharded_helper_on_one_gpu():

@@ -228,3 +228,59 @@ def test_top_k(tmpl512):
     fb = oracle.search(t, y, dy, periods, qs, box, dt0=0.0)
     kb = oracle.search(t, y, dy, periods, qs, box, dt0=0.0, top_k=1)
     assert np.array_equal(fb.chi2, kb.chi2) and np.array_equal(fb.best, kb.best)
+
+
+# ------------------------------------------------------------------------------ out_gap (runner-up)
+@pytest.mark.parametrize("seed,dt0", [(3, 0.0), (4, 0.0), (5, 0.3)])
+def test_gap_is_second_smallest_distinct_score_minus_best(seed, dt0, tmpl512):
+    """`gap` (Best::second - best, used by the GPU parity tests' near-tie rule) against a brute force
+    over ALL (duration, start) scores built from the literal per-window export: the smallest score
+    strictly above the minimum, minus the minimum.  A duplicate duration (same D, bit-identical
+    scores) must not count as a runner-up."""
+    t, y, dy = _tiny_curve(seed, n=56)
+    n = t.size
+    periods = np.array([1.3, 2.9, 7.7])
+    qs = np.array([3.2 / n, 6.5 / n, 6.6 / n, 11.0 / n, 20.0 / n])     # D = 3, 6, 6 (duplicate), 11, 20
+    res = oracle.search(t, y, dy, periods, qs, tmpl512, dt0=dt0)
+    chi0 = oracle.chi2_null(y, dy)
+    for ip, period in enumerate(periods):
+        scores = []
+        for q in qs:
+            _, _, c_out, c_in = oracle.window_chi2_literal(t, y, dy, period, q, tmpl512, dt0)
+            scores.append(c_out + c_in)
+        s = np.sort(np.concatenate(scores))
+        best = s[0]
+        # the literal export and the search differ by rounding (~1e-13 chi2): "distinct" = further
+        # apart than that; the duplicate-D pair and any exact repeats of the minimum fall inside it
+        above = s[s > best + 1e-11 * chi0]
+        assert above.size > 0
+        expect = above[0] - best
+        assert abs(res.chi2[ip] - best) <= 1e-12 * chi0
+        assert abs(res.gap[ip] - expect) <= 2e-11 * chi0 + 1e-9 * expect, (ip, res.gap[ip], expect)
+        assert res.gap[ip] > 0.0
+
+
+def test_gap_is_infinite_when_every_score_is_equal(tmpl512):
+    """Flat curve: every window scores exactly chi2_0 = 0, so there is no runner-up (reading G22)."""
+    t = np.linspace(0.0, 10.0, 40)
+    res = oracle.search(t, np.ones(40), np.full(40, 1e-3), [1.1, 2.3], [0.1, 0.2], tmpl512, dt0=0.0)
+    assert np.all(np.isinf(res.gap)) and np.all(res.chi2 == 0.0)
+
+
+def test_gap_of_a_constructed_two_window_problem(tmpl512):
+    """Two dips of different depth, one duration, stride = D: the runner-up is the shallower dip's
+    window and the gap equals the difference of their closed-form box scores (constant template:
+    score = -(sum w r)^2 / sum w)."""
+    n = 40
+    t = np.arange(n, dtype=np.float64)                   # period 40 -> phases i/40, identity order
+    y = np.ones(n)
+    y[8:12] = 1.0 - 3e-3
+    y[24:28] = 1.0 - 2e-3
+    dy = np.full(n, 1e-3)
+    box = np.ones(16)
+    res = oracle.search(t, y, dy, [40.0], [4.0 / n], box, dt0=1.0)      # D = 4, stride 4: starts 0, 4, ..
+    w = 1.0 / dy[0] ** 2
+    s_deep = -(4 * w * 3e-3) ** 2 / (4 * w)
+    s_shallow = -(4 * w * 2e-3) ** 2 / (4 * w)
+    assert res.best["start"][0] == 8 and res.best["dur_idx"][0] == 0
+    assert abs(res.gap[0] - (s_shallow - s_deep)) <= 1e-12 * abs(s_deep)
