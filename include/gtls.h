@@ -103,7 +103,13 @@ typedef struct {
     void*    workspace;          /* optional caller-owned DEVICE scratch (256-byte aligned)        */
     size_t   workspace_bytes;    /* its size; must be >= gtls_workspace_bytes(...)                 */
     int32_t  period_tile;        /* periods processed per tile; 0 = automatic                     */
-    int32_t  path;               /* 0 = automatic, 1 = force fused path, 2 = force general path    */
+    int32_t  path;               /* 0 = automatic; 1 = force the fused small-N path (one CTA per
+                                    (curve, period): fold, sort, pad, scans and chi2 in shared memory),
+                                    GTLS_EUNSUPPORTED where it does not apply: dy not uniform, top_k or
+                                    chi2_fp32 set, n_dur > 32, a window class stride above 31 columns
+                                    (dt0 below ~0.045 with long durations, or dt0 above 31 / D_max), or
+                                    a light curve too long for a CTA's shared memory (n > ~8000);
+                                    2 = force the general tiled path                               */
     gtls_stats* stats;           /* optional, host                                                */
 } gtls_opts;
 

@@ -365,7 +365,7 @@ def gtls_batch_workspace_bytes(curve_offset, period_offset, n_dur: int, period_t
 
 def gtls_search_batch(t, y, dy, curve_offset, period_grid, period_offset, duration_grid, tmpl, *,
                       dt0: float = 0.05, sde_kernel: int = 151, top_k: int = 0, chi2_fp32: int = 0,
-                      period_tile: int = 0, workspace=None, stream=None) -> BatchResult:
+                      period_tile: int = 0, path: int = 0, workspace=None, stream=None) -> BatchResult:
     """Survey mode (``gtls_search_batch`` in include/gtls.h): concatenated light curves and period
     grids with host offset arrays; ``duration_grid`` is [n_dur] (shared) or [total periods, n_dur]."""
     lib = load_library()
@@ -389,7 +389,7 @@ def gtls_search_batch(t, y, dy, curve_offset, period_grid, period_offset, durati
     if per_period and int(kq.shape[0]) != per_total:
         raise ValueError("duration_grid rows must match period_grid")
     o = _opts(dev, kt, stream, dt0=float(dt0), sde_kernel=int(sde_kernel), top_k=int(top_k),
-              chi2_fp32=int(chi2_fp32), dur_per_period=per_period, period_tile=int(period_tile))
+              chi2_fp32=int(chi2_fp32), dur_per_period=per_period, period_tile=int(period_tile), path=int(path))
     if workspace is not None:
         if not (_is_torch(workspace) and workspace.is_cuda):
             raise ValueError("workspace must be a CUDA uint8 tensor")

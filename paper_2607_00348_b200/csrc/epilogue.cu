@@ -188,7 +188,39 @@ __global__ void __launch_bounds__(kRedThreads) k_sde_argmax(const double* __rest
     }
 }
 
+// survey mode: the summary of every curve of a batch, one thread per curve
+__global__ void __launch_bounds__(128) k_batch_summary(int n_curves, const long long* __restrict__ per_off,
+                                                       const SdeScratch* __restrict__ sc, const gtls_best* __restrict__ best,
+                                                       const double* __restrict__ periods, const CurveInfo* __restrict__ info,
+                                                       const unsigned long long* __restrict__ counters, gtls_summary* out) {
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= n_curves) return;
+    const long long p0 = per_off[c];
+    const SdeScratch s = sc[c];
+    const gtls_best b = best[p0 + s.argmin];
+    gtls_summary o;
+    o.best_period_idx = s.argmin;
+    o.best_dur_idx = b.dur_idx;
+    o.best_start = b.start;
+    o.best_period = periods[p0 + s.argmin];
+    o.best_t0 = b.t0;
+    o.best_depth = b.depth;
+    o.chi2_min = s.chi2_min;
+    o.chi2_null = info[c].chi2_0;
+    o.sde_raw_max = s.sde_raw_best;
+    o.sde_max = s.sde_max;
+    o.sde_argmax = s.sde_argmax;
+    o.windows_evaluated = (int64_t)counters[2 * c];
+    out[c] = o;
+}
+
 }  // namespace
+
+void launch_batch_summary(int n_curves, const long long* per_off, const SdeScratch* sc, const gtls_best* best,
+                          const double* periods, const CurveInfo* info, const unsigned long long* counters,
+                          gtls_summary* out, cudaStream_t st) {
+    k_batch_summary<<<(n_curves + 127) / 128, 128, 0, st>>>(n_curves, per_off, sc, best, periods, info, counters, out);
+}
 
 void launch_sde(const double* chi2, long long n_per, int kernel, double* sde_raw, double* sde,
                 SdeScratch* scratch, cudaStream_t st, int* n_launches) {

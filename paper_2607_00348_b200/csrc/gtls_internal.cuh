@@ -199,6 +199,10 @@ SideStream* side_stream(int which);
 
 void launch_curve_pre(const double* t, const double* y, const double* dy, int n, double* wr,
                       double* w, double* wr2, CurveInfo* info, cudaStream_t st);
+// survey mode (api_batch.cu): per-curve arrays + validation flags for every curve of a concatenated batch
+void launch_batch_pre(int n_curves, const double* t, const double* y, const double* dy, const long long* curve_off,
+                      const double* periods, const long long* per_off, const double* durs, int n_dur,
+                      int dur_per_period, double* wr, double* w, double* wr2, CurveInfo* info, cudaStream_t st);
 void launch_grid_check(const double* periods, long long n_per, const double* durs,
                        long long n_durs_total, CurveInfo* info, cudaStream_t st);
 constexpr int kTopKMax = 8;   // largest gtls_opts.top_k the pruning kernel takes (per-lane lists live in registers)
@@ -230,11 +234,40 @@ void launch_gather_refine(const double* periods, const double* durs, int dur_per
 void launch_merge_refined(const long long* sel, int K, const double* chi2b, const gtls_best* bestb, double* chi2,
                           gtls_best* best, cudaStream_t st);
 
+// Fused small-N path (small.cu): a batch of light curves, one work item per (curve, period).
+struct SmallArgs {
+    long long n_items;            // total periods over all curves
+    int n_dur, n_tmpl, dur_per_period;
+    double dt0;
+    const long long* curve_off;   // device [n_curves + 1]: offsets of the curves in t / wr
+    const long long* per_off;     // device [n_curves + 1]: offsets of the curves in periods / outputs
+    const double* t;              // concatenated light-curve times
+    const double* wr;             // concatenated w_i r_i
+    const CurveInfo* info;        // [n_curves]: chi2_0, the common weight (w_min)
+    const double* periods;        // [n_items]
+    const double* durs;           // [n_dur] or [n_items][n_dur]
+    const double* tmpl;
+    const double* gtab;           // sum g_D, sum g_D^2 for every D the grids can ask for
+    double* out_chi2;             // [n_items]
+    gtls_best* out_best;          // [n_items] or nullptr
+    unsigned long long* counters; // [n_curves][2]: windows, window points
+    unsigned long long* queue;    // work counter (zeroed by the caller)
+    int xs_len, n_max;            // set by launch_tls_small
+};
+size_t small_smem_bytes(int n_max, int d_max);
+// dy uniform is the caller's check; this one covers sizes: shared memory, n_dur, class strides <= 31
+bool small_path_fits(int n_max, int d_max, int n_dur, double dt0);
+int launch_tls_small(SmallArgs& a, int n_max, int d_max, int sm_count, cudaStream_t st);   // returns a cudaError_t
+
 struct SdeScratch {      // device scalars of the epilogue
     double chi2_min, mean_sr, sd_sr, sde_raw_best, sde_max;
     long long argmin, sde_argmax;
     int degenerate, pad_;
 };
+// one gtls_summary per curve of a batch from the epilogue scalars, the best records and the window counters
+void launch_batch_summary(int n_curves, const long long* per_off, const SdeScratch* sc, const gtls_best* best,
+                          const double* periods, const CurveInfo* info, const unsigned long long* counters,
+                          gtls_summary* out, cudaStream_t st);
 void launch_sde(const double* chi2, long long n_per, int kernel, double* sde_raw, double* sde,
                 SdeScratch* scratch, cudaStream_t st, int* n_launches);
 

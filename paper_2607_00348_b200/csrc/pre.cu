@@ -13,11 +13,11 @@ __device__ __forceinline__ double warp_sum(double v) {
 }
 
 // One CTA of 1024 threads: deterministic strided accumulation + fixed-shape tree.
-__global__ void __launch_bounds__(1024) k_curve_pre(const double* __restrict__ t,
-                                                    const double* __restrict__ y,
-                                                    const double* __restrict__ dy, int n,
-                                                    double* __restrict__ wr, double* __restrict__ w,
-                                                    double* __restrict__ wr2, CurveInfo* info) {
+__device__ __forceinline__ void curve_pre_body(const double* __restrict__ t,
+                                               const double* __restrict__ y,
+                                               const double* __restrict__ dy, int n,
+                                               double* __restrict__ wr, double* __restrict__ w,
+                                               double* __restrict__ wr2, CurveInfo* info) {
     __shared__ double s_sum[32], s_min[32], s_max[32];
     __shared__ int s_bad[32];
     double acc = 0.0, wmin = 1e300, wmax = 0.0;
@@ -63,6 +63,21 @@ __global__ void __launch_bounds__(1024) k_curve_pre(const double* __restrict__ t
             info->chi2_0 = acc; info->w_min = wmin; info->w_max = wmax; info->bad_curve = bad;
         }
     }
+}
+
+__global__ void __launch_bounds__(1024) k_curve_pre(const double* __restrict__ t, const double* __restrict__ y,
+                                                    const double* __restrict__ dy, int n, double* __restrict__ wr,
+                                                    double* __restrict__ w, double* __restrict__ wr2, CurveInfo* info) {
+    curve_pre_body(t, y, dy, n, wr, w, wr2, info);
+}
+// survey mode: one CTA per light curve of the concatenated batch
+__global__ void __launch_bounds__(1024) k_curve_pre_batch(const double* __restrict__ t, const double* __restrict__ y,
+                                                          const double* __restrict__ dy, const long long* __restrict__ curve_off,
+                                                          double* __restrict__ wr, double* __restrict__ w,
+                                                          double* __restrict__ wr2, CurveInfo* info) {
+    const long long c0 = curve_off[blockIdx.x];
+    curve_pre_body(t + c0, y + c0, dy + c0, (int)(curve_off[blockIdx.x + 1] - c0), wr + c0, w + c0, wr2 + c0,
+                   info + blockIdx.x);
 }
 
 // Many CTAs; integer counters and the max are order independent, so atomics keep it exact.
@@ -238,6 +253,42 @@ __global__ void __launch_bounds__(256) k_bin_trials(TileArgs a) {
 
 }  // namespace
 
+// survey mode: blockIdx.y = curve; periods [per_off[c], per_off[c+1]) and, when dur_per_period, their rows
+__global__ void __launch_bounds__(256) k_grid_check_batch(const double* __restrict__ periods,
+                                                          const long long* __restrict__ per_off,
+                                                          const double* __restrict__ durs, int n_dur,
+                                                          int dur_per_period, CurveInfo* info) {
+    const int c = blockIdx.y;
+    const long long p0 = per_off[c], np = per_off[c + 1] - p0;
+    int bp = 0, bd = 0;
+    double qmax = 0.0;
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long nth = (long long)gridDim.x * blockDim.x;
+    for (long long i = tid; i < np; i += nth) {
+        const double p = periods[p0 + i];
+        bp += (isfinite(p) && p > 0.0) ? 0 : 1;
+    }
+    const long long nd = dur_per_period ? np * n_dur : n_dur;
+    const double* dq = dur_per_period ? durs + p0 * n_dur : durs;
+    for (long long i = tid; i < nd; i += nth) {
+        const double q = dq[i];
+        const bool ok = isfinite(q) && q > 0.0 && q <= 0.5;
+        bd += ok ? 0 : 1;
+        if (ok) qmax = fmax(qmax, q);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        bp += __shfl_xor_sync(0xffffffffu, bp, o);
+        bd += __shfl_xor_sync(0xffffffffu, bd, o);
+        qmax = fmax(qmax, __shfl_xor_sync(0xffffffffu, qmax, o));
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (bp) atomicAdd(&info[c].bad_period, bp);
+        if (bd) atomicAdd(&info[c].bad_duration, bd);
+        atomicMax((unsigned long long*)&info[c].q_max, (unsigned long long)__double_as_longlong(qmax));
+    }
+}
+
 void launch_curve_pre(const double* t, const double* y, const double* dy, int n, double* wr,
                       double* w, double* wr2, CurveInfo* info, cudaStream_t st) {
     k_curve_pre<<<1, 1024, 0, st>>>(t, y, dy, n, wr, w, wr2, info);
@@ -249,6 +300,13 @@ void launch_grid_check(const double* periods, long long n_per, const double* dur
     int blocks = (int)((work + 256 * 8 - 1) / (256 * 8));
     blocks = blocks < 1 ? 1 : (blocks > 1184 ? 1184 : blocks);
     k_grid_check<<<blocks, 256, 0, st>>>(periods, n_per, durs, n_durs_total, info);
+}
+
+void launch_batch_pre(int n_curves, const double* t, const double* y, const double* dy, const long long* curve_off,
+                      const double* periods, const long long* per_off, const double* durs, int n_dur,
+                      int dur_per_period, double* wr, double* w, double* wr2, CurveInfo* info, cudaStream_t st) {
+    k_curve_pre_batch<<<n_curves, 1024, 0, st>>>(t, y, dy, curve_off, wr, w, wr2, info);
+    k_grid_check_batch<<<dim3(8, n_curves), 256, 0, st>>>(periods, per_off, durs, n_dur, dur_per_period, info);
 }
 
 void launch_bin_trials(const TileArgs& a, cudaStream_t st) {
