@@ -199,6 +199,33 @@ def run_survey(args, g, torch, devname):
     ms_loop, _ = timed(loop)
     clocks = sampler.stop()                      # both legs ran with the sampler polling
     found = sum(1 for c, w in enumerate(ws_) if c % 2 == 0 and res.summaries[c]["sde_max"] > 9.0)
+    # per-curve agreement with the oracle (BASELINE.json config 5) on a seeded subset of the curves, in full:
+    # same best period index and |SDE_max difference| <= 1e-6; chi2 and indices as in the parity tests
+    agreement = None
+    if args.survey_check > 0:
+        import oracle
+        rng = np.random.default_rng(20260700348)
+        pick = sorted(rng.choice(len(ws_), size=min(args.survey_check, len(ws_)), replace=False).tolist())
+        chi2_all, sde_all, best_all = res.chi2.cpu().numpy(), res.sde.cpu().numpy(), res.best()
+        rows, t_or = [], 0.0
+        for c in pick:
+            w = ws_[c]
+            t0 = time.perf_counter()
+            ro = oracle.search(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=dt0)
+            so = oracle.sde(ro.chi2, 151)
+            t_or += time.perf_counter() - t0
+            sl = slice(int(po[c]), int(po[c + 1]))
+            strict = ro.gap > 1e-12 * np.abs(ro.chi2)
+            mism = (best_all[sl]["dur_idx"] != ro.best["dur_idx"]) | (best_all[sl]["start"] != ro.best["start"])
+            rows.append({"curve": c, "same_best_period_idx": bool(res.summaries[c]["best_period_idx"] == so.best_period_idx),
+                         "sde_max_abs_diff": float(abs(res.summaries[c]["sde_max"] - so.sde.max())),
+                         "sde_abs_diff_max": float(np.abs(sde_all[sl] - so.sde).max()),
+                         "chi2_max_rel_err": float(np.max(np.abs(chi2_all[sl] - ro.chi2) / ro.chi2)),
+                         "index_mismatches": int(np.sum(mism & strict))})
+        ok = all(r["same_best_period_idx"] and r["sde_max_abs_diff"] <= 1e-6 and r["chi2_max_rel_err"] <= 1e-9 and
+                 r["index_mismatches"] == 0 for r in rows)
+        agreement = {"curves_checked": len(rows), "of": len(ws_), "all_agree": ok, "oracle_seconds": t_or,
+                     "oracle_cores": oracle.num_threads(), "per_curve": rows}
     return {"metric": METRIC, "value": trials / (ms_batch / 1e3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_batch, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -208,6 +235,7 @@ def run_survey(args, g, torch, devname):
             "curves_per_s": len(ws_) / (ms_batch / 1e3), "ms_per_curve": ms_batch / len(ws_),
             "loop_of_single_calls": {"curves_per_s": len(ws_) / (ms_loop / 1e3), "ms_per_curve": ms_loop / len(ws_)},
             "curves_with_injected_transit_above_sde_9": f"{found} of {(len(ws_) + 1) // 2}",
+            "per_curve_agreement": agreement,
             "clocks": clocks}
 
 
@@ -260,6 +288,9 @@ def main():
     ap.add_argument("--peak-fp64", type=float, default=0.0, metavar="SECONDS",
                     help="measure the fp64 FMA rate of this GPU (gtls_peak_fp64: register-only DFMA kernel) as a "
                          "0.1 s burst and sustained over SECONDS, with the clocks seen; prints one JSON line")
+    ap.add_argument("--survey-check", type=int, default=3,
+                    help="survey mode: number of (seeded) curves searched in full by the CPU oracle for the "
+                         "per-curve agreement report (0 = none)")
     ap.add_argument("--survey", type=int, default=0,
                     help="survey mode (BASELINE.json config 5): search this many c5 curves per step with one "
                          "gtls_search_batch call and report curves/s beside trials/s")

@@ -98,12 +98,29 @@ struct SmCls {
     unsigned tab;                  // this warp's window table (kSmTab doubles)
 };
 
+// Template taps of one lane: g_D[m * stp + col] for m = m0 .. m0 + count - 1 (linear interpolation at the cell
+// centres, reading G14) into the lane's column of the warp's emit buffer, 256 bytes per tap.  One copy of this
+// code for every ring size (the kernel is bound by instruction fetch, not by arithmetic).
+__device__ __noinline__ void sm_taps(const unsigned tl, const int m0, const int count, const int stp, const int col,
+                                     const int D, const bool active, const double* __restrict__ tm, const int n_tmpl,
+                                     const double tscale) {
+#pragma unroll 2
+    for (int m = 0; m < count; ++m) {
+        const int j = (m0 + m) * stp + col;
+        sts64(tl + (unsigned)(m * 256), (active && j < D) ? tmpl_lerp(tm, n_tmpl, j, tscale) : 0.0);
+    }
+}
+
 // Score the windows of a table slice (a5 + a8): entry g * SL + o holds the in-transit sum C of the window
 // that completed at row rho_base + o of segment g.  Coalesced over the table: 32 windows per step, every
-// lane busy, four steps in flight.
-__device__ __forceinline__ void sm_score_slice(const SmCls& c, const int G, const int L, const int lsl,
-                                               const int rho_base, const int mb1, const int lane, SmCand& best) {
-    const int SL = 1 << lsl;
+// lane busy, four steps in flight.  Within a lane the starts ascend, so a strict '<' keeps the first of equal
+// scores.  (One copy for every ring size: not inlined, everything passed by value.)
+struct SmScore { unsigned tab, ss; int D, stp, off, nWr, G, L, lsl, kw_base; double G_u, inv_den; };
+__device__ __noinline__ SmCand sm_score_slice(const SmScore c, SmCand best, const int lane) {
+    const int SL = 1 << c.lsl;
+    double bd = best.has ? best.d : __longlong_as_double(0x7ff0000000000000LL), bdepth = best.depth;
+    int bs = best.has ? best.s : -1;
+    const int bs0 = bs;
 #pragma unroll 1
     for (int i0 = 0; i0 < kSmTab; i0 += 128) {
         double C[4], hi[4], lo[4];
@@ -111,10 +128,10 @@ __device__ __forceinline__ void sm_score_slice(const SmCls& c, const int G, cons
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             const int i = i0 + 32 * k + lane;
-            const int g = i >> lsl, o = i & (SL - 1);
-            const int kw = rho_base + o - mb1;
-            const int kap = g * L + kw;
-            const bool ok = g < G && kw >= 0 && kw < L && kap < c.nWr;
+            const int g = i >> c.lsl, o = i & (SL - 1);
+            const int kw = c.kw_base + o;
+            const int kap = g * c.L + kw;
+            const bool ok = g < c.G && kw >= 0 && kw < c.L && kap < c.nWr;
             const int sx = ok ? c.off + kap * c.stp : 0;
             sidx[k] = ok ? sx : -1;
             C[k] = lds64(c.tab + (unsigned)(i * 8));
@@ -126,7 +143,48 @@ __device__ __forceinline__ void sm_score_slice(const SmCls& c, const int G, cons
             const double swr = fmax(hi[k] - lo[k], 0.0);
             const double depth = swr * c.inv_den;
             const double d = -2.0 * depth * C[k] + (depth * depth) * c.G_u;
-            if (sidx[k] >= 0 && (!best.has || d <= best.d)) offer(best, d, sidx[k], depth);
+            // (a lane's previous best from an EARLIER class may have a later start: the lexicographic rule)
+            const bool take = sidx[k] >= 0 && (d < bd || (d == bd && sidx[k] < bs));
+            bd = take ? d : bd; bdepth = take ? depth : bdepth; bs = take ? sidx[k] : bs;
+        }
+    }
+    if (bs != bs0 || bs >= 0) { best.d = bd; best.depth = bdepth; best.s = bs; best.has = bs >= 0 ? 1 : 0; }
+    return best;
+}
+
+// Column sums of one batch: a task = (segment g, window slot sl); R lanes per task, each adding at most four
+// consecutive columns of the emit buffer, then log2(R) shuffle steps; the sum goes into the window table.
+struct SmReduce { unsigned pbase, tab; int stp, G, lsl, o0; };
+__device__ __noinline__ void sm_reduce_batch(const SmReduce c, const int lane) {
+    constexpr int PF = kSmPF;
+    const int R = c.stp <= 4 ? 1 : (c.stp <= 8 ? 2 : (c.stp <= 16 ? 4 : 8));
+    const int ntask = c.G * PF;
+    const int tpr = 32 / R;                        // tasks per round
+    const int tsub = lane / R, r4 = (lane % R) * 4;
+#pragma unroll 1
+    for (int t0 = 0; t0 < ntask; t0 += 2 * tpr) {          // two independent rounds per trip
+        double q[2][4];
+        unsigned ta[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int task = t0 + h * tpr + tsub;
+            const bool tv = task < ntask;
+            const int g = tv ? task / PF : 0, sl = task % PF;
+            const unsigned pr = c.pbase + (unsigned)((sl * kSmPitch + g * c.stp + r4) * 8);
+            const int left = tv ? c.stp - r4 : 0;          // columns of the task from this lane's first one on
+            q[h][0] = left > 0 ? lds64(pr) : 0.0;
+            q[h][1] = left > 1 ? lds64(pr + 8) : 0.0;
+            q[h][2] = left > 2 ? lds64(pr + 16) : 0.0;
+            q[h][3] = left > 3 ? lds64(pr + 24) : 0.0;
+            ta[h] = (tv && r4 == 0) ? c.tab + (unsigned)(((g << c.lsl) + c.o0 + sl) * 8) : 0u;
+        }
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            double v = (q[h][0] + q[h][1]) + (q[h][2] + q[h][3]);
+            if (R >= 2) v += __shfl_xor_sync(0xffffffffu, v, 1);
+            if (R >= 4) v += __shfl_xor_sync(0xffffffffu, v, 2);
+            if (R >= 8) v += __shfl_xor_sync(0xffffffffu, v, 4);
+            if (ta[h]) sts64(ta[h], v);
         }
     }
 }
@@ -148,11 +206,7 @@ __device__ __forceinline__ void sm_march(const SmCls& c, const double* __restric
 #pragma unroll
         for (int h = 0; h < MB; h += 12) {
             constexpr int kHalf = 12;
-#pragma unroll 1
-            for (int m = h; m < min(h + kHalf, MB); ++m) {
-                const int j = m * c.stp + col;
-                sts64(tl + (unsigned)((m - h) * 256), (active && j < c.D) ? tmpl_lerp(tm, n_tmpl, j, tscale) : 0.0);
-            }
+            sm_taps(tl, h, min(kHalf, MB - h), c.stp, col, c.D, active, tm, n_tmpl, tscale);
 #pragma unroll
             for (int m = h; m < h + kHalf; ++m)
                 if (m < MB) T[m] = lds64(tl + (unsigned)((m - h) * 256));
@@ -172,24 +226,19 @@ __device__ __forceinline__ void sm_march(const SmCls& c, const double* __restric
     while ((1 << lg) < G) ++lg;
     const int lsl = 9 - lg;                        // kSmTab = 512 entries
     const int SL = 1 << lsl;
-    // column sums: a task = (segment g, window slot sl) of a batch; R lanes per task, each adding at most
-    // four consecutive columns, then log2(R) shuffle steps: a fixed instruction sequence per round
-    const bool direct = c.stp == 1;                // the lane's ring value is the window sum: straight into the table
-    const int R = c.stp <= 4 ? 1 : (c.stp <= 8 ? 2 : (c.stp <= 16 ? 4 : 8));
-    const int ntask = G * PF;
-    const int tpr = 32 / R;                        // tasks per round
-    const int tsub = lane / R, r4 = (lane % R) * 4;
-    unsigned pcur = c.part + (unsigned)(lane * 8), pother = pcur + (unsigned)(PF * kSmPitch * 8);
-    const unsigned tdir = c.tab + (unsigned)((seg << lsl) * 8);     // direct mode: this lane's table row
+    // (stp >= 2 here: stride-1 classes take sm_march_direct)
+    const unsigned pcur = c.part + (unsigned)(lane * 8);
     int rho_base = 0;
+    SmReduce rd;
+    rd.pbase = c.part; rd.tab = c.tab; rd.stp = c.stp; rd.G = G; rd.lsl = lsl;
+    SmScore sc;
+    sc.tab = c.tab; sc.ss = c.ss; sc.D = c.D; sc.stp = c.stp; sc.off = c.off; sc.nWr = c.nWr; sc.G = G; sc.L = L; sc.lsl = lsl;
+    sc.G_u = c.G_u; sc.inv_den = c.inv_den;
     __syncwarp();
 
 #pragma unroll 1
     for (int b = 0; b < nbat; ++b) {
         PROF_T(pt0);
-        const int o0 = b * PF - rho_base;          // table column of the batch's first row
-        const unsigned ecur = direct ? tdir + (unsigned)(o0 * 8) : pcur;
-        const unsigned estep = direct ? 8u : (unsigned)(kSmPitch * 8);
 #pragma unroll
         for (int u = 0; u < PF; ++u) {
             xq[(u + LA) % XQ] = lds64(c.xs + (unsigned)(min(e, c.zidx) * 8));
@@ -198,46 +247,19 @@ __device__ __forceinline__ void sm_march(const SmCls& c, const double* __restric
 #pragma unroll
             for (int m = MB - 1; m >= 1; --m) acc[m + 1] = fma(T[m], xv, acc[m]);
             acc[1] = T[0] * xv;
-            sts64(ecur + (unsigned)u * estep, acc[MB]);
+            sts64(pcur + (unsigned)(u * kSmPitch * 8), acc[MB]);
         }
         __syncwarp();
         PROF_T(pt1);
         PROF_ADD(4, pt1 - pt0);
-        if (!direct) {
-            const unsigned pbase = pcur - (unsigned)(lane * 8);
-#pragma unroll 1
-            for (int t0 = 0; t0 < ntask; t0 += 2 * tpr) {          // two independent rounds per trip
-                double q[2][4];
-                unsigned ta[2];
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const int task = t0 + h * tpr + tsub;
-                    const bool tv = task < ntask;
-                    const int g = tv ? task / PF : 0, sl = task % PF;
-                    const unsigned pr = pbase + (unsigned)((sl * kSmPitch + g * c.stp + r4) * 8);
-                    const int left = tv ? c.stp - r4 : 0;          // columns of the task from this lane's first one on
-                    q[h][0] = left > 0 ? lds64(pr) : 0.0;
-                    q[h][1] = left > 1 ? lds64(pr + 8) : 0.0;
-                    q[h][2] = left > 2 ? lds64(pr + 16) : 0.0;
-                    q[h][3] = left > 3 ? lds64(pr + 24) : 0.0;
-                    ta[h] = (tv && r4 == 0) ? c.tab + (unsigned)(((g << lsl) + o0 + sl) * 8) : 0u;
-                }
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    double v = (q[h][0] + q[h][1]) + (q[h][2] + q[h][3]);
-                    if (R >= 2) v += __shfl_xor_sync(0xffffffffu, v, 1);
-                    if (R >= 4) v += __shfl_xor_sync(0xffffffffu, v, 2);
-                    if (R >= 8) v += __shfl_xor_sync(0xffffffffu, v, 4);
-                    if (ta[h]) sts64(ta[h], v);
-                }
-            }
-            const unsigned tmp = pcur; pcur = pother; pother = tmp;
-        }
+        rd.o0 = b * PF - rho_base;                 // table column of the batch's first row
+        sm_reduce_batch(rd, lane);
         PROF_T(pt2);
         PROF_ADD(5, pt2 - pt1);
-        if (o0 + PF == SL || b == nbat - 1) {      // the slice is full (or the march ends): score and recycle it
+        if (rd.o0 + PF == SL || b == nbat - 1) {   // the slice is full (or the march ends): score and recycle it
             __syncwarp();
-            sm_score_slice(c, G, L, lsl, rho_base, MB - 1, lane, best);
+            sc.kw_base = rho_base - (MB - 1);
+            best = sm_score_slice(sc, best, lane);
             __syncwarp();
             rho_base += SL;
             PROF_T(pt3);
@@ -246,20 +268,79 @@ __device__ __forceinline__ void sm_march(const SmCls& c, const double* __restric
     }
 }
 
+// Stride-1 classes (stp == 1: every start is a trial position, D <= 24): the lane's ring value IS the window sum,
+// so each row's completed window is scored in place (a5, a8) -- no emit buffer, no table.  32 segments of L
+// consecutive windows, L odd so that the lanes' x1 / S1 reads (L doubles apart) do not share banks; within a
+// lane the starts ascend, so a strict '<' keeps the first of equal scores.
+template <int MB>
+__device__ __forceinline__ void sm_march_direct(const SmCls& c, const double* __restrict__ tm, const int n_tmpl,
+                                                const double tscale, const int lane, SmCand& best) {
+    constexpr int PF = kSmPF, XQ = 4, LA = 3;
+    const int L = ((c.nWr + 31) / 32) | 1;
+    double T[MB];
+    {
+        const unsigned tl = c.part + (unsigned)(lane * 8);
+#pragma unroll
+        for (int h = 0; h < MB; h += 12) {
+            sm_taps(tl, h, min(12, MB - h), 1, 0, c.D, true, tm, n_tmpl, tscale);
+#pragma unroll
+            for (int m = h; m < h + 12; ++m)
+                if (m < MB) T[m] = lds64(tl + (unsigned)((m - h) * 256));
+        }
+    }
+    double acc[MB + 1], xq[XQ];
+#pragma unroll
+    for (int u = 0; u <= MB; ++u) acc[u] = 0.0;
+    const int nbat = (L + MB - 1 + PF - 1) / PF;
+    const int k0 = lane * L;                       // first window of this lane's segment (s = off + kappa, off = 0)
+    int e = c.off + k0;
+#pragma unroll
+    for (int k = 0; k < LA; ++k) { xq[k] = lds64(c.xs + (unsigned)(min(e, c.zidx) * 8)); ++e; }
+    // S1 at the start / end of the window that completes at row rho: S1[k0 + rho - (MB-1)] and the same + D;
+    // clamped below for the warm-up rows (their windows are not scored)
+    double bd = __longlong_as_double(0x7ff0000000000000LL), bdepth = 0.0;
+    int bs = -1;
+#pragma unroll 1
+    for (int b = 0; b < nbat; ++b) {
+#pragma unroll
+        for (int u = 0; u < PF; ++u) {
+            xq[(u + LA) % XQ] = lds64(c.xs + (unsigned)(min(e, c.zidx) * 8));
+            ++e;
+            const int kw = b * PF + u - (MB - 1);
+            const int kap = k0 + kw;
+            const bool ok = kw >= 0 && kw < L && kap < c.nWr;
+            const int s = ok ? c.off + kap : 0;
+            const double hi = lds64(c.ss + (unsigned)((s + c.D) * 8)), lo = lds64(c.ss + (unsigned)(s * 8));
+            const double xv = xq[u % XQ];
+#pragma unroll
+            for (int m = MB - 1; m >= 1; --m) acc[m + 1] = fma(T[m], xv, acc[m]);
+            acc[1] = T[0] * xv;
+            const double swr = fmax(hi - lo, 0.0);
+            const double depth = swr * c.inv_den;
+            const double d = -2.0 * depth * acc[MB] + (depth * depth) * c.G_u;
+            const bool take = ok && d < bd;
+            bd = take ? d : bd; bdepth = take ? depth : bdepth; bs = take ? s : bs;
+        }
+    }
+    if (bs >= 0) offer(best, bd, bs, bdepth);
+}
+
 __device__ __forceinline__ void sm_run_unit(const SmCls& c, const int taps, const double* __restrict__ tm,
                                             const int n_tmpl, const double tscale, const int lane, SmCand& best) {
-    switch (chi2_ring_index(taps)) {
-        case 0: sm_march<24>(c, tm, n_tmpl, tscale, lane, best); break;
-        case 1: sm_march<21>(c, tm, n_tmpl, tscale, lane, best); break;
-        case 2: sm_march<16>(c, tm, n_tmpl, tscale, lane, best); break;
-        case 3: sm_march<12>(c, tm, n_tmpl, tscale, lane, best); break;
-        case 4: sm_march<8>(c, tm, n_tmpl, tscale, lane, best); break;
-        default: sm_march<4>(c, tm, n_tmpl, tscale, lane, best); break;
+    // few ring sizes: the instruction cache, not the FP64 pipe, is what this kernel runs out of (twelve
+    // warps in different phases of different bodies), so a ring is allowed to be up to twice its taps
+    if (c.stp == 1) {
+        if (taps > 12) sm_march_direct<24>(c, tm, n_tmpl, tscale, lane, best);
+        else sm_march_direct<12>(c, tm, n_tmpl, tscale, lane, best);
+        return;
     }
+    if (taps > 16) sm_march<24>(c, tm, n_tmpl, tscale, lane, best);
+    else if (taps > 8) sm_march<16>(c, tm, n_tmpl, tscale, lane, best);
+    else sm_march<8>(c, tm, n_tmpl, tscale, lane, best);
 }
 
 // strict total order (key32, fp64 phase, index) == (fp64 phase, index)
-__device__ __forceinline__ bool sm_key_less(const u64 a, const u64 b, const double* __restrict__ t, const double period) {
+__device__ __noinline__ bool sm_key_less(const u64 a, const u64 b, const double* __restrict__ t, const double period) {
     const u32 ka = (u32)(a >> 32), kb = (u32)(b >> 32);
     if (ka != kb) return ka < kb;
     const double pa = fold_phase(t[(u32)a], period), pb = fold_phase(t[(u32)b], period);
@@ -366,13 +447,13 @@ __global__ void __launch_bounds__(kSmThreads, 1) k_tls_small(SmallArgs a) {
         PROF_T(s0);
         PROF_ADD(8, s0 - k0);
         // ---- a1 fold + a2 sort ------------------------------------------------------------------
-        // (t comes from the L2: eight loads in flight per thread, one latency per eight points)
-        for (int i0 = 0; i0 < n; i0 += 8 * kSmThreads) {
-            double tv[8];
+        // (t comes from the L2: two loads in flight per thread; the division is ~60 instructions, so no wider unroll)
+        for (int i0 = 0; i0 < n; i0 += 2 * kSmThreads) {
+            double tv[2];
 #pragma unroll
-            for (int k = 0; k < 8; ++k) { const int i = i0 + k * kSmThreads + tid; tv[k] = i < n ? t[i] : 0.0; }
+            for (int k = 0; k < 2; ++k) { const int i = i0 + k * kSmThreads + tid; tv[k] = i < n ? t[i] : 0.0; }
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {
+            for (int k = 0; k < 2; ++k) {
                 const int i = i0 + k * kSmThreads + tid;
                 if (i < n) {
                     const u32 k32 = phase_key32(fold_phase(tv[k], period));
@@ -435,12 +516,12 @@ __global__ void __launch_bounds__(kSmThreads, 1) k_tls_small(SmallArgs a) {
         PROF_ADD(12, s4 - s3);
         // ---- a3 gather + wrap pad + zeros, a4 inclusive scan -----------------------------------
         const int len = n + pad;
-        for (int i0 = 0; i0 < a.xs_len; i0 += 8 * kSmThreads) {       // eight L2 loads in flight per thread
-            double v[8];
+        for (int i0 = 0; i0 < a.xs_len; i0 += 4 * kSmThreads) {       // four L2 loads in flight per thread
+            double v[4];
 #pragma unroll
-            for (int k = 0; k < 8; ++k) { const int i = i0 + k * kSmThreads + tid; v[k] = i < len ? wr[perm[i < n ? i : i - n]] : 0.0; }
+            for (int k = 0; k < 4; ++k) { const int i = i0 + k * kSmThreads + tid; v[k] = i < len ? wr[perm[i < n ? i : i - n]] : 0.0; }
 #pragma unroll
-            for (int k = 0; k < 8; ++k) { const int i = i0 + k * kSmThreads + tid; if (i < a.xs_len) xs[i] = v[k]; }
+            for (int k = 0; k < 4; ++k) { const int i = i0 + k * kSmThreads + tid; if (i < a.xs_len) xs[i] = v[k]; }
         }
         __syncthreads();
         PROF_T(s5);
