@@ -65,10 +65,12 @@ typedef struct {
 typedef struct {
     double  ms_total;        /* first kernel to last kernel of the call                           */
     double  ms_pre;          /* a0: per-curve arrays, validation, duration table                  */
-    double  ms_fold;         /* a1: fold + sortable keys                                          */
-    double  ms_sort;         /* a2: radix sort passes + tie fix-up                                */
-    double  ms_scan;         /* a3+a4: gather, wrap pad, prefix sums                              */
-    double  ms_chi2;         /* a5-a7: depth, out-of-transit, in-transit chi2 per window          */
+    double  ms_fold;         /* a1 when it runs as a kernel of its own (LSD sort path); ~0 otherwise */
+    double  ms_sort;         /* general path: the fused a1-a4 stage (fold, bucket sort, gather,
+                                wrap pad, prefix sums are one chain of kernels)                   */
+    double  ms_scan;         /* a3+a4 when separate (LSD sort path); ~0 otherwise                  */
+    double  ms_chi2;         /* a5-a8: trial binning + the ring kernels.  Fused small-N path
+                                (path == 1): the ONE kernel that runs a1-a8                       */
     double  ms_reduce;       /* a8: per-period lexicographic argmin                               */
     double  ms_epilogue;     /* a9: SR, SDE_raw, median detrend, argmax                           */
     int64_t kernel_launches; /* kernels launched by this call                                     */

@@ -524,19 +524,24 @@ def gtls_sde(chi2, *, sde_kernel: int = 151, stream=None):
 
 
 def gtls_search_sharded(t, y, dy, period_grid, duration_grid, tmpl, *, group=None, dt0: float = 0.05,
-                        sde_kernel: int = 151, _search=None, _sde=None, **kw) -> SearchResult:
+                        sde_kernel: int = 151, **kw) -> SearchResult:
     """Period-sharded search over the ranks of a ``torch.distributed`` group (one process per GPU).
 
     Trial periods are independent (the paper reports 1.75x on two GPUs), so
     rank r searches periods r, r+W, r+2W, ... (interleaved: every rank gets the same mix of long and short
     periods, i.e. of durations), the only exchange is ONE all-gather of 32 bytes per period (chi2 + the
     24-byte best record), and every rank then runs the SR / SDE epilogue (``gtls_sde``) over the full
-    spectrum in grid order.  Every rank passes the same full arrays and gets the same full result.
-    ``_search`` / ``_sde`` replace the two library calls in the CPU (gloo) test of this plumbing."""
+    spectrum in grid order.  Every rank passes the same full arrays and gets the same full result."""
+    return _sharded_search(gtls_search, gtls_sde, t, y, dy, period_grid, duration_grid, tmpl, group=group, dt0=dt0,
+                           sde_kernel=sde_kernel, **kw)
+
+
+def _sharded_search(search, sde_fn, t, y, dy, period_grid, duration_grid, tmpl, *, group=None, dt0: float = 0.05,
+                    sde_kernel: int = 151, **kw) -> SearchResult:
+    """The plumbing of gtls_search_sharded around the two library calls (`search`, `sde_fn`); the CPU (gloo)
+    test of the shard / all-gather / unshard logic calls this private helper with stand-ins for them."""
     import torch
     import torch.distributed as dist
-    search = _search or gtls_search
-    sde_fn = _sde or gtls_sde
     world, rank = dist.get_world_size(group), dist.get_rank(group)
     n_per = int(period_grid.shape[0])
     per_period = duration_grid.ndim == 2

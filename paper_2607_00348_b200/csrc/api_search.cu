@@ -112,7 +112,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     if (!t || !y || !dy || !period_grid || !duration_grid || !tmpl || !out_chi2) return GTLS_EINVAL;
     if (n < 3 || n > 0x3fffffff || n_per < 1 || n_dur < 1 || n_dur > 4096 || n_tmpl < 2) return GTLS_EINVAL;
     if (!(o.dt0 >= 0.0) || o.sde_kernel < 0 || (o.sde_kernel > 1 && o.sde_kernel % 2 == 0)) return GTLS_EINVAL;
-    if (o.path < 0 || o.path > 2 || o.period_tile < 0) return GTLS_EINVAL;
+    if (o.path < 0 || o.path > 2 || o.period_tile < 0 || o.period_tile > 65535) return GTLS_EINVAL;   // (a tile is gridDim.y of the sort kernels)
     if (o.top_k < 0) return GTLS_EINVAL;
     if (o.top_k > kTopKMax || (o.top_k > 0 && o.chi2_fp32)) return GTLS_EUNSUPPORTED;
     if (o.chi2_fp32 != 0 && o.chi2_fp32 != 1) return GTLS_EINVAL;
@@ -173,8 +173,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
 
     Timer tm;
     tm.init(o.stats != nullptr, st);
-    cudaEvent_t ev_begin = nullptr, ev_end = nullptr;
-    if (o.stats) { cudaEventCreate(&ev_begin); cudaEventCreate(&ev_end); cudaEventRecord(ev_begin, st); }
+    tm.mark(9);                                   // begin of the call (events 9 / 10 belong to the Timer: no leak on early returns)
     gtls_stats stats;
     memset(&stats, 0, sizeof(stats));
 
@@ -312,7 +311,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     tm.mark(1);
     CU(cudaMemcpyAsync(&sc, d_sde_sc, sizeof(sc), cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(counters, d_counters, sizeof(counters), cudaMemcpyDeviceToHost, st));
-    if (o.stats) cudaEventRecord(ev_end, st);
+    tm.mark(10);
     CU(cudaStreamSynchronize(st));
     CU(cudaGetLastError());
     if (o.stats) stats.ms_epilogue = tm.ms(0, 1);
@@ -344,9 +343,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
         CU(cudaStreamSynchronize(st));
     }
     if (o.stats) {
-        float f = 0.f;
-        cudaEventElapsedTime(&f, ev_begin, ev_end);
-        stats.ms_total = f;
+        stats.ms_total = tm.ms(9, 10);
         stats.windows = (int64_t)counters[0];
         stats.window_points = (int64_t)counters[1];
         stats.period_points = n * n_per;
@@ -354,7 +351,6 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
         stats.path = use_small ? 1 : 2;
         stats.uniform_dy = uniform ? 1 : 0;
         *o.stats = stats;
-        cudaEventDestroy(ev_begin); cudaEventDestroy(ev_end);
     }
     io.idle = ws.idle = true;                 // the stream was synchronised after the last use of both
     return sc.degenerate ? GTLS_EDEGENERATE : GTLS_OK;

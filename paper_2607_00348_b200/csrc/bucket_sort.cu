@@ -401,13 +401,11 @@ void launch_bucket_sort_head(const BucketArgs& b, cudaStream_t st) {
 }
 
 void launch_bucket_sort_tail(const BucketArgs& b, bool has0, bool has2, bool sort_only, cudaStream_t st) {
-    static bool attr_set = false;
-    if (!attr_set) {
+    {   // per device and cheap: set on every call (a process-wide flag would miss a second device)
         cudaFuncSetAttribute(k_bucket_finish<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFinSmem);
         cudaFuncSetAttribute(k_bucket_finish<true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFinSmem);
         cudaFuncSetAttribute(k_bucket_finish<true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFinSmem);
         cudaFuncSetAttribute(k_bucket_finish<false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFinSmem);
-        attr_set = true;
     }
     k_bucket_scatter<<<count_grid(b), kCountThreads, 0, st>>>(b);
     const dim3 fgrid(b.tile);

@@ -762,11 +762,8 @@ static void launch_variant_t(const TileArgs& a, int v, cudaStream_t st) {
     // (c4: 60 -> 36 GB of DRAM reads per 4144-period tile of the dominant variant, SM clock under the power cap 1845 -> 1890 MHz)
     if (!NARROW && grid > kGridCapWide) grid = kGridCapWide;
     const size_t sm = (size_t)(kRW * kWarpSmem) * sizeof(double);
-    static bool set = false;
-    if (!set) {
-        cudaFuncSetAttribute(k_chi2_ring<MB, NARROW, UNIFORM, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-        set = true;
-    }
+    // (per device, cheap: set on every launch rather than behind a process-wide flag)
+    cudaFuncSetAttribute(k_chi2_ring<MB, NARROW, UNIFORM, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     k_chi2_ring<MB, NARROW, UNIFORM, F><<<grid, kRT, sm, st>>>(a, a.trial_list + (long long)v * trials, a.trial_count + v,
                                                              a.trial_count + kChi2Variants * (1 + kBinBlocks) + v);
 }

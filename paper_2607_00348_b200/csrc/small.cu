@@ -50,7 +50,7 @@ constexpr int kSmBinBits = 11;
 constexpr int kSmBins = 1 << kSmBinBits;
 constexpr int kSmPF = 8;                       // rows per batch of the march
 constexpr int kSmPitch = 36;                   // doubles per row of the emit buffer
-constexpr int kSmPart = 2 * kSmPF * kSmPitch;  // emit buffer doubles per warp (two batches)
+constexpr int kSmPart = kSmPF * kSmPitch;      // emit buffer doubles per warp (one batch: it is summed before the next one starts)
 constexpr int kSmTab = 512;                    // window-table doubles per warp
 constexpr int kSmMaxDur = 32;
 constexpr int kSmTmpl = 512;
@@ -115,14 +115,14 @@ __device__ __noinline__ void sm_taps(const unsigned tl, const int m0, const int 
 // that completed at row rho_base + o of segment g.  Coalesced over the table: 32 windows per step, every
 // lane busy, four steps in flight.  Within a lane the starts ascend, so a strict '<' keeps the first of equal
 // scores.  (One copy for every ring size: not inlined, everything passed by value.)
-struct SmScore { unsigned tab, ss; int D, stp, off, nWr, G, L, lsl, kw_base; double G_u, inv_den; };
+struct SmScore { unsigned tab, ss; int D, stp, off, nWr, G, L, lsl, kw_base, count; double G_u, inv_den; };
 __device__ __noinline__ SmCand sm_score_slice(const SmScore c, SmCand best, const int lane) {
     const int SL = 1 << c.lsl;
     double bd = best.has ? best.d : __longlong_as_double(0x7ff0000000000000LL), bdepth = best.depth;
     int bs = best.has ? best.s : -1;
     const int bs0 = bs;
 #pragma unroll 1
-    for (int i0 = 0; i0 < kSmTab; i0 += 128) {
+    for (int i0 = 0; i0 < c.count; i0 += 128) {
         double C[4], hi[4], lo[4];
         int sidx[4];
 #pragma unroll
@@ -152,43 +152,6 @@ __device__ __noinline__ SmCand sm_score_slice(const SmScore c, SmCand best, cons
     return best;
 }
 
-// Column sums of one batch: a task = (segment g, window slot sl); R lanes per task, each adding at most four
-// consecutive columns of the emit buffer, then log2(R) shuffle steps; the sum goes into the window table.
-struct SmReduce { unsigned pbase, tab; int stp, G, lsl, o0; };
-__device__ __noinline__ void sm_reduce_batch(const SmReduce c, const int lane) {
-    constexpr int PF = kSmPF;
-    const int R = c.stp <= 4 ? 1 : (c.stp <= 8 ? 2 : (c.stp <= 16 ? 4 : 8));
-    const int ntask = c.G * PF;
-    const int tpr = 32 / R;                        // tasks per round
-    const int tsub = lane / R, r4 = (lane % R) * 4;
-#pragma unroll 1
-    for (int t0 = 0; t0 < ntask; t0 += 2 * tpr) {          // two independent rounds per trip
-        double q[2][4];
-        unsigned ta[2];
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const int task = t0 + h * tpr + tsub;
-            const bool tv = task < ntask;
-            const int g = tv ? task / PF : 0, sl = task % PF;
-            const unsigned pr = c.pbase + (unsigned)((sl * kSmPitch + g * c.stp + r4) * 8);
-            const int left = tv ? c.stp - r4 : 0;          // columns of the task from this lane's first one on
-            q[h][0] = left > 0 ? lds64(pr) : 0.0;
-            q[h][1] = left > 1 ? lds64(pr + 8) : 0.0;
-            q[h][2] = left > 2 ? lds64(pr + 16) : 0.0;
-            q[h][3] = left > 3 ? lds64(pr + 24) : 0.0;
-            ta[h] = (tv && r4 == 0) ? c.tab + (unsigned)(((g << c.lsl) + c.o0 + sl) * 8) : 0u;
-        }
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            double v = (q[h][0] + q[h][1]) + (q[h][2] + q[h][3]);
-            if (R >= 2) v += __shfl_xor_sync(0xffffffffu, v, 1);
-            if (R >= 4) v += __shfl_xor_sync(0xffffffffu, v, 2);
-            if (R >= 8) v += __shfl_xor_sync(0xffffffffu, v, 4);
-            if (ta[h]) sts64(ta[h], v);
-        }
-    }
-}
-
 template <int MB>
 __device__ __forceinline__ void sm_march(const SmCls& c, const double* __restrict__ tm, const int n_tmpl,
                                          const double tscale, const int lane, SmCand& best) {
@@ -202,7 +165,7 @@ __device__ __forceinline__ void sm_march(const SmCls& c, const double* __restric
     // column of the still unused emit buffer, 12 at a time, then loaded into registers
     double T[MB];
     {
-        const unsigned tl = c.part + (unsigned)(lane * 8);
+        const unsigned tl = c.tab + (unsigned)(lane * 8);       // (the window table is not in use yet)
 #pragma unroll
         for (int h = 0; h < MB; h += 12) {
             constexpr int kHalf = 12;
@@ -224,16 +187,34 @@ __device__ __forceinline__ void sm_march(const SmCls& c, const double* __restric
     // window table: a time slice of SL rows for each of the G segments (SL a power of two)
     int lg = 0;
     while ((1 << lg) < G) ++lg;
-    const int lsl = 9 - lg;                        // kSmTab = 512 entries
+    int lsl = 9 - lg;                              // kSmTab = 512 entries
+    while (lsl > 3 && (1 << (lsl - 1)) >= nbat * PF) --lsl;      // short marches: a smaller slice, fewer entries to score
     const int SL = 1 << lsl;
     // (stp >= 2 here: stride-1 classes take sm_march_direct)
     const unsigned pcur = c.part + (unsigned)(lane * 8);
     int rho_base = 0;
-    SmReduce rd;
-    rd.pbase = c.part; rd.tab = c.tab; rd.stp = c.stp; rd.G = G; rd.lsl = lsl;
+    // column sums of a batch: a task = (segment g, window slot sl); R lanes per task, each adding at most four
+    // consecutive columns of the emit buffer, then log2(R) shuffle steps.  stp >= 2 means at most four rounds
+    // of 32 / R tasks; what a lane does in round k never changes, so its addresses are set up once here.
+    const int R = c.stp <= 4 ? 1 : (c.stp <= 8 ? 2 : (c.stp <= 16 ? 4 : 8));
+    const int ntask = G * PF, tpr = 32 / R;
+    const int nround = (ntask + tpr - 1) / tpr;          // <= 4
+    const int r4 = (lane % R) * 4;
+    unsigned rsrc[4];                                    // emit-buffer address of the lane's first column
+    int rdst[4], rleft[4];                               // table offset (or -1), columns to add (0 .. 4)
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int task = k * tpr + lane / R;
+        const bool tv = task < ntask;
+        const int g = tv ? task / PF : 0, sl = task % PF;
+        rsrc[k] = c.part + (unsigned)((sl * kSmPitch + g * c.stp + r4) * 8);
+        rleft[k] = tv ? min(max(c.stp - r4, 0), 4) : 0;
+        rdst[k] = (tv && r4 == 0) ? ((g << lsl) + sl) * 8 : -1;
+    }
     SmScore sc;
     sc.tab = c.tab; sc.ss = c.ss; sc.D = c.D; sc.stp = c.stp; sc.off = c.off; sc.nWr = c.nWr; sc.G = G; sc.L = L; sc.lsl = lsl;
     sc.G_u = c.G_u; sc.inv_den = c.inv_den;
+    sc.count = min(kSmTab, G << lsl);              // table entries in use
     __syncwarp();
 
 #pragma unroll 1
@@ -252,11 +233,26 @@ __device__ __forceinline__ void sm_march(const SmCls& c, const double* __restric
         __syncwarp();
         PROF_T(pt1);
         PROF_ADD(4, pt1 - pt0);
-        rd.o0 = b * PF - rho_base;                 // table column of the batch's first row
-        sm_reduce_batch(rd, lane);
+        const int o0 = b * PF - rho_base;          // table column of the batch's first row
+        const unsigned tb = c.tab + (unsigned)(o0 * 8);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (k < nround) {                      // (warp uniform)
+                const double q0 = rleft[k] > 0 ? lds64(rsrc[k]) : 0.0;
+                const double q1 = rleft[k] > 1 ? lds64(rsrc[k] + 8) : 0.0;
+                const double q2 = rleft[k] > 2 ? lds64(rsrc[k] + 16) : 0.0;
+                const double q3 = rleft[k] > 3 ? lds64(rsrc[k] + 24) : 0.0;
+                double v = (q0 + q1) + (q2 + q3);
+                if (R >= 2) v += __shfl_xor_sync(0xffffffffu, v, 1);
+                if (R >= 4) v += __shfl_xor_sync(0xffffffffu, v, 2);
+                if (R >= 8) v += __shfl_xor_sync(0xffffffffu, v, 4);
+                if (rdst[k] >= 0) sts64(tb + (unsigned)rdst[k], v);
+            }
+        }
+        __syncwarp();                              // the emit buffer is free for the next batch
         PROF_T(pt2);
         PROF_ADD(5, pt2 - pt1);
-        if (rd.o0 + PF == SL || b == nbat - 1) {   // the slice is full (or the march ends): score and recycle it
+        if (o0 + PF == SL || b == nbat - 1) {      // the slice is full (or the march ends): score and recycle it
             __syncwarp();
             sc.kw_base = rho_base - (MB - 1);
             best = sm_score_slice(sc, best, lane);
@@ -279,7 +275,7 @@ __device__ __forceinline__ void sm_march_direct(const SmCls& c, const double* __
     const int L = ((c.nWr + 31) / 32) | 1;
     double T[MB];
     {
-        const unsigned tl = c.part + (unsigned)(lane * 8);
+        const unsigned tl = c.tab + (unsigned)(lane * 8);       // (the window table is not in use yet)
 #pragma unroll
         for (int h = 0; h < MB; h += 12) {
             sm_taps(tl, h, min(12, MB - h), 1, 0, c.D, true, tm, n_tmpl, tscale);

@@ -85,8 +85,8 @@ def _shard_worker(rank, world, port, out):
     import gtls_inputs as gi
     import paper_2607_00348_b200 as g
     w = gi.make_workload(1).subset(29)                   # 106 periods: not a multiple of the world size
-    r = g.gtls_search_sharded(w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations, w.tmpl, dt0=0.05, sde_kernel=31,
-                              _search=_oracle_search_stub, _sde=_oracle_sde_stub)
+    r = g._sharded_search(_oracle_search_stub, _oracle_sde_stub, w.lc.t, w.lc.y, w.lc.dy, w.periods, w.durations,
+                          w.tmpl, dt0=0.05, sde_kernel=31)
     out.put((rank, np.asarray(r.chi2), r.best().copy(), np.asarray(r.sde), r.summary))
     dist.barrier()
     dist.destroy_process_group()
