@@ -268,6 +268,32 @@ size_t gtls_workspace_bytes(int64_t n, int64_t n_per, int32_t n_dur, const gtls_
  * them.  Caller-owned memory is never retained. */
 void gtls_release_cache(void);
 
+/* The search for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): the fused small-N path of gtls_search (opts->path = 1: fold, sort, pad, scans and
+ * the chi2 rings of a period in one CTA's shared memory; then SR / SDE, Eq. 17) with ALL of
+ * its scratch in one static device array of gtls_static_scratch_bytes() (~263 KB) that every GPU which loads
+ * the library holds until exit.  It calls no cudaMalloc / cudaFree / allocating library routine and does not
+ * use the block pool or opts->workspace.
+ *   - Every array argument is a DEVICE pointer (opts->pointers_on_device is ignored); out_chi2, out_best,
+ *     out_sde_raw and out_sde are all required ([n_per] each); out_summary (host) may be NULL.
+ *   - Limits: 3 <= n <= GTLS_STATIC_MAX_N, n_dur <= 32, uniform dy, opts->top_k == 0, opts->chi2_fp32 == 0, and
+ *     the limits of the fused kernel (window class strides <= 31 columns for this dt0, the folded arrays within
+ *     one CTA's shared memory: n <= ~8000 for duration fractions up to 0.15).  Anything beyond returns
+ *     GTLS_EUNSUPPORTED with the reason in gtls_last_cuda_error(): n, n_dur and the options before anything is
+ *     launched, the rest after the two validation kernels (which is where dy and the durations are read).
+ *   - Uses opts->dt0, dur_per_period, sde_kernel, device, stream.  Synchronises opts->stream (validation
+ *     flags, summary), like gtls_search.  Results are those of gtls_search with path = 1, bit for bit.
+ *   - The array is shared by ALL calls in the process on that GPU and keeps the previous call's contents (the
+ *     call clears what must start at zero): calls that overlap on one GPU -- other threads, other streams --
+ *     race on it.  Serialise them. */
+#define GTLS_STATIC_MAX_N 8192
+int gtls_search_static(const double* t, const double* y, const double* dy, int64_t n,
+                       const double* period_grid, int64_t n_per, const double* duration_grid,
+                       int32_t n_dur, const double* tmpl, int32_t n_tmpl, const gtls_opts* opts,
+                       double* out_chi2, gtls_best* out_best, double* out_sde_raw, double* out_sde,
+                       gtls_summary* out_summary);
+size_t gtls_static_scratch_bytes(void);
+
 /* Measurement aid (bench.py --peak-fp64), not part of the search: runs a register-only fp64 FMA kernel
  * (16 independent chains per thread, three distinct register operands per DFMA, 16 warps per SM) back to
  * back on opts->stream for about `seconds` (0 < seconds <= 60) of device time and returns the sustained

@@ -20,7 +20,7 @@ from typing import Any, Optional
 
 import numpy as np
 
-__all__ = ["gtls_search", "gtls_search_two_stage", "gtls_search_batch", "gtls_batch_workspace_bytes",
+__all__ = ["gtls_search", "gtls_search_static", "gtls_static_scratch_bytes", "gtls_search_two_stage", "gtls_search_batch", "gtls_batch_workspace_bytes",
            "gtls_period_grid_size", "gtls_period_grid", "gtls_duration_grid", "BatchResult", "gtls_search_sharded", "gtls_fold_sort", "gtls_fold_scan", "gtls_window_chi2", "gtls_sde",
            "gtls_workspace_bytes", "gtls_release_cache", "gtls_peak_fp64", "gtls_strerror", "gtls_version", "GtlsError", "SearchResult",
            "BEST_DTYPE", "lib_path", "load_library"]
@@ -99,6 +99,10 @@ def load_library():
     lib.gtls_search.argtypes = [dp, dp, dp, C.c_int64, dp, C.c_int64, dp, C.c_int32, dp, C.c_int32,
                                 C.POINTER(GtlsOpts), dp, vp, dp, dp, C.POINTER(GtlsSummary)]
     lib.gtls_search.restype = C.c_int
+    lib.gtls_search_static.argtypes = lib.gtls_search.argtypes
+    lib.gtls_search_static.restype = C.c_int
+    lib.gtls_static_scratch_bytes.argtypes = []
+    lib.gtls_static_scratch_bytes.restype = C.c_size_t
     lib.gtls_search_two_stage.argtypes = [dp, dp, dp, C.c_int64, dp, C.c_int64, dp, C.c_int32, dp, C.c_int32,
                                           C.POINTER(GtlsOpts), C.c_int32, dp, vp, dp, dp, vp,
                                           C.POINTER(GtlsSummary)]
@@ -284,6 +288,42 @@ def gtls_search(t, y, dy, period_grid, duration_grid, tmpl, *, dt0: float = 0.05
         raise GtlsError(rc, "gtls_search")
     return SearchResult(chi2, sde_raw, sde, best, summ.as_dict(), rc,
                         st.as_dict() if stats else None, [kt, ky, kd, kp, kq, km])
+
+
+def gtls_search_static(t, y, dy, period_grid, duration_grid, tmpl, *, dt0: float = 0.05, sde_kernel: int = 151,
+                       out=None, stream=None) -> SearchResult:
+    """The allocation-free search (``gtls_search_static`` in include/gtls.h): CUDA tensors only; the library
+    uses its static scratch array and allocates nothing.  ``out`` = (chi2, best_raw, sde_raw, sde) tensors to
+    write into (float64[n_per], uint8[n_per, 24], float64[n_per] x 2); created here when None."""
+    lib = load_library()
+    kt, pt, dev = _prep(t)
+    ky, py, d2 = _prep(y)
+    kd, pd, d3 = _prep(dy)
+    kp, pp, d4 = _prep(period_grid)
+    kq, pq, d5 = _prep(duration_grid)
+    km, pm, d6 = _prep(tmpl)
+    if not all((dev, d2, d3, d4, d5, d6)):
+        raise ValueError("gtls_search_static takes CUDA tensors only")
+    n, n_per, n_tmpl = int(kt.shape[0]), int(kp.shape[0]), int(km.shape[0])
+    per_period = 1 if kq.ndim == 2 else 0
+    n_dur = int(kq.shape[-1])
+    if per_period and int(kq.shape[0]) != n_per:
+        raise ValueError("duration_grid rows must match period_grid")
+    o = _opts(True, kt, stream, dt0=float(dt0), sde_kernel=int(sde_kernel), dur_per_period=per_period)
+    if out is None:
+        out = (_empty((n_per,), kt), _empty((n_per, BEST_DTYPE.itemsize), kt, np.uint8), _empty((n_per,), kt),
+               _empty((n_per,), kt))
+    chi2, best, sde_raw, sde = out
+    summ = GtlsSummary()
+    rc = lib.gtls_search_static(pt, py, pd, n, pp, n_per, pq, n_dur, pm, n_tmpl, C.byref(o), _ptr(chi2),
+                                _ptr(best), _ptr(sde_raw), _ptr(sde), C.byref(summ))
+    if rc not in (GTLS_OK, GTLS_EDEGENERATE):
+        raise GtlsError(rc, "gtls_search_static")
+    return SearchResult(chi2, sde_raw, sde, best, summ.as_dict(), rc, None, [kt, ky, kd, kp, kq, km])
+
+
+def gtls_static_scratch_bytes() -> int:
+    return int(load_library().gtls_static_scratch_bytes())
 
 
 def gtls_period_grid_size(span: float, r_star: float = 1.0, m_star: float = 1.0, oversampling: float = 3.0,
