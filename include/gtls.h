@@ -25,6 +25,9 @@
  *     must already be normalised to mean ~1.
  *   - Thread safety: concurrent calls are safe when they use distinct streams and distinct
  *     workspaces (or let the library allocate its own).
+ *   - Process state: every entry point makes `opts->device` the calling thread's current CUDA device
+ *     (cudaSetDevice) and leaves it current on return; a caller that works on another device sets it
+ *     again.  Nothing else of the caller's CUDA state is changed.
  */
 #ifndef GTLS_H_
 #define GTLS_H_
@@ -179,6 +182,19 @@ int gtls_search_two_stage(const double* t, const double* y, const double* dy, in
                           double* out_chi2, gtls_best* out_best,
                           double* out_sde_raw, double* out_sde,
                           int64_t* out_refined, gtls_summary* out_summary);
+
+/* Parity / debug export of steps a5-a8 AS THE HOT KERNEL COMPUTES THEM: runs the general tiled path of
+ * gtls_search (fold, sort, pad, scans, trial binning, the register-ring chi2 kernel of this trial's variant,
+ * instantiated to dump its scores) for ONE (period, duration fraction q) and returns, for every strided start
+ * k*stride < n (Eq. 18), the start index, the depth a (Eq. 12-13) and dchi2 = chi2(window) - chi2_0 =
+ * -2 a C + a^2 G (Eq. 15 + 16 minus the Eq. 11 edge term) exactly as the kernel's scoring step saw them --
+ * including every non-minimal window, which gtls_search reduces away.  Host pointers only
+ * (opts->pointers_on_device => GTLS_EUNSUPPORTED); uses opts->dt0, device, stream; arrays must hold
+ * ceil(n/stride) entries (n is always enough); *out_chi2_null (may be NULL) = chi2_0.  A window the kernel
+ * never scored comes back as NaN.  Returns the number of starts (>= 1) or a negative error code. */
+int64_t gtls_ring_window_chi2(const double* t, const double* y, const double* dy, int64_t n, double period,
+                              double q, const double* tmpl, int32_t n_tmpl, const gtls_opts* opts,
+                              int32_t* out_start, double* out_depth, double* out_dchi2, double* out_chi2_null);
 
 /* Parity / debug export of steps a1-a2: phases (Eq. 10) and the stable phase-sort permutation
  * for each period.  out_phase [n_per*n] may be NULL; out_perm [n_per*n] (int32) is required.

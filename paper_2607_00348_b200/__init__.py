@@ -21,7 +21,7 @@ from typing import Any, Optional
 import numpy as np
 
 __all__ = ["gtls_search", "gtls_search_static", "gtls_static_scratch_bytes", "gtls_search_two_stage", "gtls_search_batch", "gtls_batch_workspace_bytes",
-           "gtls_period_grid_size", "gtls_period_grid", "gtls_duration_grid", "BatchResult", "gtls_search_sharded", "gtls_fold_sort", "gtls_fold_scan", "gtls_window_chi2", "gtls_sde",
+           "gtls_period_grid_size", "gtls_period_grid", "gtls_duration_grid", "BatchResult", "gtls_search_sharded", "gtls_fold_sort", "gtls_fold_scan", "gtls_window_chi2", "gtls_ring_window_chi2", "gtls_sde",
            "gtls_workspace_bytes", "gtls_release_cache", "gtls_peak_fp64", "gtls_strerror", "gtls_version", "GtlsError", "SearchResult",
            "BEST_DTYPE", "lib_path", "load_library"]
 
@@ -115,6 +115,9 @@ def load_library():
     lib.gtls_window_chi2.argtypes = [dp, dp, dp, C.c_int64, C.c_double, C.c_double, dp, C.c_int32,
                                      C.POINTER(GtlsOpts), ip, dp, dp, dp]
     lib.gtls_window_chi2.restype = C.c_int64
+    lib.gtls_ring_window_chi2.argtypes = [dp, dp, dp, C.c_int64, C.c_double, C.c_double, dp, C.c_int32,
+                                          C.POINTER(GtlsOpts), ip, dp, dp, C.POINTER(C.c_double)]
+    lib.gtls_ring_window_chi2.restype = C.c_int64
     lib.gtls_sde.argtypes = [dp, C.c_int64, C.POINTER(GtlsOpts), dp, dp, C.POINTER(GtlsSummary)]
     lib.gtls_sde.restype = C.c_int
     lib.gtls_period_grid_size.argtypes = [C.c_double] * 5
@@ -546,6 +549,27 @@ def gtls_window_chi2(t, y, dy, period: float, q: float, tmpl, *, dt0: float = 0.
         raise GtlsError(int(k), "gtls_window_chi2")
     k = int(k)
     return start[:k], depth[:k], c_out[:k], c_in[:k]
+
+
+def gtls_ring_window_chi2(t, y, dy, period: float, q: float, tmpl, *, dt0: float = 0.0):
+    """Every window of one (period, duration fraction) as the ring kernel of the general path scores it
+    (``gtls_ring_window_chi2`` in include/gtls.h; host arrays): (start, depth, dchi2, chi2_null)."""
+    lib = load_library()
+    t, y, dy, tmpl = (np.ascontiguousarray(a, dtype=np.float64) for a in (t, y, dy, tmpl))
+    n = int(t.shape[0])
+    o = GtlsOpts()
+    lib.gtls_opts_default(C.byref(o))
+    o.dt0 = float(dt0)
+    start = np.empty(n, dtype=np.int32)
+    depth, dchi2 = np.empty(n), np.empty(n)
+    c0 = C.c_double(0.0)
+    k = lib.gtls_ring_window_chi2(t.ctypes.data, y.ctypes.data, dy.ctypes.data, n, float(period), float(q),
+                                  tmpl.ctypes.data, int(tmpl.shape[0]), C.byref(o), start.ctypes.data,
+                                  depth.ctypes.data, dchi2.ctypes.data, C.byref(c0))
+    if k < 0:
+        raise GtlsError(int(k), "gtls_ring_window_chi2")
+    k = int(k)
+    return start[:k], depth[:k], dchi2[:k], c0.value
 
 
 def gtls_sde(chi2, *, sde_kernel: int = 151, stream=None):

@@ -91,22 +91,14 @@ void run_fold_sort_scan(TileArgs& a, const SortScratch& sc, double* x2, double* 
 using namespace gtls;
 using namespace gtls::api;
 
-extern "C" {
+// The search (gtls_search) and, with dbg_d / dbg_a set, its per-window debug export (gtls_ring_window_chi2: DEVICE
+// arrays of ceil(n / stride) doubles for the ONE trial of a 1 period x 1 duration call on the general path).
+static int search_impl(const double* t, const double* y, const double* dy, int64_t n,
+                       const double* period_grid, int64_t n_per, const double* duration_grid,
+                       int32_t n_dur, const double* tmpl, int32_t n_tmpl, const gtls_opts* opts,
+                       double* out_chi2, gtls_best* out_best, double* out_sde_raw, double* out_sde,
+                       gtls_summary* out_summary, double* dbg_d, double* dbg_a) {
 
-size_t gtls_workspace_bytes(int64_t n, int64_t n_per, int32_t n_dur, const gtls_opts* opts) {
-    if (n < 3 || n_per < 1 || n_dur < 1) return 0;
-    const gtls_opts o = resolve_opts(opts);
-    const Sizes s = workspace_sizes(n, n_per, n_dur, 0.5, false);     // worst case
-    const int tile = o.period_tile > 0 ? (int)(o.period_tile < n_per ? o.period_tile : n_per)
-                                       : auto_tile(n_per, s, kDefaultTileBudget);
-    return s.fixed + (size_t)tile * align_up(s.per_period) + 64 * 256;
-}
-
-int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
-                const double* period_grid, int64_t n_per, const double* duration_grid,
-                int32_t n_dur, const double* tmpl, int32_t n_tmpl, const gtls_opts* opts,
-                double* out_chi2, gtls_best* out_best, double* out_sde_raw, double* out_sde,
-                gtls_summary* out_summary) {
     api::cuda_err_buf()[0] = 0;
     const gtls_opts o = resolve_opts(opts);
     if (!t || !y || !dy || !period_grid || !duration_grid || !tmpl || !out_chi2) return GTLS_EINVAL;
@@ -212,7 +204,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     const bool small_ok = uniform && o.top_k == 0 && o.chi2_fp32 == 0 && n <= 65535 &&
                           small_path_fits((int)n, gtab_max, n_dur, o.dt0);
     if (o.path == 1 && !small_ok) return GTLS_EUNSUPPORTED;
-    const bool use_small = small_ok && o.path != 2;
+    const bool use_small = small_ok && o.path != 2 && !dbg_d;
     int tile = 0;
     SdeScratch sc;
     unsigned long long counters[2];
@@ -255,6 +247,7 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
         a.pitch = pitch_for(n, info.q_max); a.spitch = a.pitch + 8;
         a.t = d_t; a.wr = d_wr; a.w = d_w; a.wr2 = d_wr2; a.periods = d_per; a.durs = d_dur;
         a.tmpl = d_tmpl; a.chi2_0 = &d_info->chi2_0;
+        a.dbg_dchi2 = dbg_d; a.dbg_depth = dbg_a;
         const int nt = (int)((n + kRadixTile - 1) / kRadixTile);
         a.keys_a = ws.take<u64>((size_t)tile * n);
         a.keys_b = ws.take<u64>((size_t)tile * n);
@@ -354,6 +347,67 @@ int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
     }
     io.idle = ws.idle = true;                 // the stream was synchronised after the last use of both
     return sc.degenerate ? GTLS_EDEGENERATE : GTLS_OK;
+}
+
+
+extern "C" {
+
+size_t gtls_workspace_bytes(int64_t n, int64_t n_per, int32_t n_dur, const gtls_opts* opts) {
+    if (n < 3 || n_per < 1 || n_dur < 1) return 0;
+    const gtls_opts o = resolve_opts(opts);
+    const Sizes s = workspace_sizes(n, n_per, n_dur, 0.5, false);     // worst case
+    const int tile = o.period_tile > 0 ? (int)(o.period_tile < n_per ? o.period_tile : n_per)
+                                       : auto_tile(n_per, s, kDefaultTileBudget);
+    return s.fixed + (size_t)tile * align_up(s.per_period) + 64 * 256;
+}
+
+int gtls_search(const double* t, const double* y, const double* dy, int64_t n,
+                const double* period_grid, int64_t n_per, const double* duration_grid,
+                int32_t n_dur, const double* tmpl, int32_t n_tmpl, const gtls_opts* opts,
+                double* out_chi2, gtls_best* out_best, double* out_sde_raw, double* out_sde,
+                gtls_summary* out_summary) {
+    return search_impl(t, y, dy, n, period_grid, n_per, duration_grid, n_dur, tmpl, n_tmpl, opts, out_chi2, out_best,
+                       out_sde_raw, out_sde, out_summary, nullptr, nullptr);
+}
+
+int64_t gtls_ring_window_chi2(const double* t, const double* y, const double* dy, int64_t n, double period,
+                              double q, const double* tmpl, int32_t n_tmpl, const gtls_opts* opts,
+                              int32_t* out_start, double* out_depth, double* out_dchi2, double* out_chi2_null) {
+    cuda_err_buf()[0] = 0;
+    gtls_opts o = resolve_opts(opts);
+    if (!t || !y || !dy || !tmpl || !out_start || !out_depth || !out_dchi2) return GTLS_EINVAL;
+    if (n < 3 || n > 0x3fffffff || n_tmpl < 2 || !(period > 0.0) || !(q > 0.0) || !(q <= 0.5) || !(o.dt0 >= 0.0)) return GTLS_EINVAL;
+    if (o.pointers_on_device) return GTLS_EUNSUPPORTED;          // a host-pointer debug export
+    if (o.top_k != 0 || o.chi2_fp32 != 0) return GTLS_EUNSUPPORTED;
+    CU(cudaSetDevice(o.device));
+    cudaStream_t st = (cudaStream_t)o.stream;
+    long long D = (long long)(q * (double)n);
+    D = D < 1 ? 1 : (D > n - 1 ? n - 1 : D);
+    long long stride = o.dt0 > 0.0 ? (long long)((double)D * o.dt0) : 1;
+    if (stride < 1) stride = 1;
+    const long long nW = (n + stride - 1) / stride;
+    Arena ar;
+    int rc = alloc_arena(ar, 2 * align_up(nW * 8) + 1024);
+    if (rc) return rc;
+    double* d_d = ar.take<double>(nW);
+    double* d_a = ar.take<double>(nW);
+    if (!d_a) return GTLS_ENOMEM;
+    CU(cudaMemsetAsync(d_d, 0xff, nW * 8, st));                   // NaN: a window the kernel did not score stays visible
+    CU(cudaMemsetAsync(d_a, 0xff, nW * 8, st));
+    o.path = 2; o.sde_kernel = 0; o.period_tile = 0; o.dur_per_period = 0; o.stats = nullptr;
+    o.workspace = nullptr; o.workspace_bytes = 0;
+    double chi2 = 0.0;
+    gtls_summary summ;
+    memset(&summ, 0, sizeof(summ));
+    rc = search_impl(t, y, dy, n, &period, 1, &q, 1, tmpl, n_tmpl, &o, &chi2, nullptr, nullptr, nullptr, &summ, d_d, d_a);
+    if (rc != GTLS_OK && rc != GTLS_EDEGENERATE) return rc;
+    CU(cudaMemcpyAsync(out_dchi2, d_d, nW * 8, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(out_depth, d_a, nW * 8, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    ar.idle = true;
+    for (long long k = 0; k < nW; ++k) out_start[k] = (int32_t)(k * stride);
+    if (out_chi2_null) *out_chi2_null = summ.chi2_null;
+    return nW;
 }
 
 int gtls_search_two_stage(const double* t, const double* y, const double* dy, int64_t n,

@@ -97,11 +97,14 @@ struct Cls {
     unsigned part;                       // shared-space address of the [kPartRows][kPartPitch] emit buffer
     unsigned fifo;                       // shared-space address of the [kFifoRows][32] X FIFO
     int Kt;                              // table entries per quantity (C, and G when dy is not uniform)
+    // debug instantiation only (gtls_ring_window_chi2): every window's dchi2 / depth, indexed by start / st0
+    double* dbg_d; double* dbg_a; int st0;
 };
 
 // a5 + a8 for one window kappa of the class (start s = off + kappa*stp): hi/lo are the prefix sums
 // at s+D and s.  a = max(rbar, 0) / mean(g_D) with rbar = swr / sw.  Uniform dy: sw * mean(g_D) is a
 // constant of the trial, so a = max(swr, 0) * inv_den (one multiply); otherwise one division.
+template <bool DBG = false>
 __device__ __forceinline__ void score_one(const Cls& c, Cand& best, const int s, const double hi1,
                                           const double lo1, const double hi0, const double lo0,
                                           const double C, const double Gt) {
@@ -109,9 +112,11 @@ __device__ __forceinline__ void score_one(const Cls& c, Cand& best, const int s,
     const double depth = c.uniform ? swr * c.inv_den_u : __ddiv_rn(swr, (hi0 - lo0) * c.gbar);
     const double Gv = c.uniform ? c.G_u : Gt;
     const double d = -2.0 * depth * C + (depth * depth) * Gv;
+    if constexpr (DBG) { c.dbg_d[s / c.st0] = d; c.dbg_a[s / c.st0] = depth; }
     if (d <= best.d || !best.has) cand_offer(best, d, s, depth);     // rarely taken after the first windows
 }
 // Wide path: score the windows [k0, k0 + nWt) of the class from table entries [0, nWt).
+template <bool DBG = false>
 __device__ __forceinline__ void score_wide(const Cls& c, Cand& best, const int lane, const int k0,
                                            const int nWt, const int toff) {
     for (int i0 = 0; i0 < nWt; i0 += 128) {
@@ -134,7 +139,7 @@ __device__ __forceinline__ void score_wide(const Cls& c, Cand& best, const int l
             const int w = i0 + 32 * u + lane;
             if (w < nWt) {
                 const unsigned ta = c.ctab + (unsigned)((w + toff) * 8);
-                score_one(c, best, c.off + (k0 + w) * c.stp, hi1[u], lo1[u], hi0[u], lo0[u], lds64(ta),
+                score_one<DBG>(c, best, c.off + (k0 + w) * c.stp, hi1[u], lo1[u], hi0[u], lo0[u], lds64(ta),
                           c.uniform ? 0.0 : lds64(ta + (unsigned)(c.Kt * 8)));
             }
         }
@@ -142,6 +147,7 @@ __device__ __forceinline__ void score_wide(const Cls& c, Cand& best, const int l
 }
 
 // Narrow path: table entry seg*SL + o holds window kw = kw_base + o of segment seg (kappa = seg*L + kw).
+template <bool DBG = false>
 __device__ __forceinline__ void score_narrow(const Cls& c, Cand& best, const int lane, const int G,
                                              const int SL, const int SLn, const float invSL,
                                              const int kw_base, const int L) {
@@ -171,7 +177,7 @@ __device__ __forceinline__ void score_narrow(const Cls& c, Cand& best, const int
         for (int u = 0; u < 4; ++u) {
             if (sidx[u] >= 0) {
                 const unsigned ta = c.ctab + (unsigned)((i0 + 32 * u + lane) * 8);
-                score_one(c, best, sidx[u], hi1[u], lo1[u], hi0[u], lo0[u], lds64(ta),
+                score_one<DBG>(c, best, sidx[u], hi1[u], lo1[u], hi0[u], lo0[u], lds64(ta),
                           c.uniform ? 0.0 : lds64(ta + (unsigned)(c.Kt * 8)));
             }
         }
@@ -229,7 +235,7 @@ __device__ __forceinline__ void reduce_batch(const Cls& c, const It& it, const i
 // >= rows_valid read as 0 (rows_min = the smallest rows_valid of the warp, so batches below it need
 // no predicate).  Taps T[m] multiply row (window + m).  Narrow path: every KB blocks the table slice
 // is scored and recycled.
-template <int MB, bool NARROW, typename F>
+template <int MB, bool NARROW, typename F, bool DBG = false>
 __device__ __forceinline__ void march(const Cls& c, const It& it, const double* __restrict__ xp,
                                       const int rows_valid, const int rows_min, const int nblk,
                                       const F (&T)[MB], const int lane, Cand& best) {
@@ -291,7 +297,7 @@ __device__ __forceinline__ void march(const Cls& c, const It& it, const double* 
         }
         if (NARROW && ++bis == it.KB) {
             __syncwarp();
-            score_narrow(c, best, lane, it.G, it.SL, it.SLn, it.invSL, kw_base, it.L);
+            score_narrow<DBG>(c, best, lane, it.G, it.SL, it.SLn, it.invSL, kw_base, it.L);
             __syncwarp();
             kw_base += it.SLn;
             bis = 0;
@@ -300,7 +306,7 @@ __device__ __forceinline__ void march(const Cls& c, const It& it, const double* 
     cp_async_wait<0>();
     if (NARROW && bis > 0) {
         __syncwarp();
-        score_narrow(c, best, lane, it.G, it.SL, it.SLn, it.invSL, kw_base, it.L);
+        score_narrow<DBG>(c, best, lane, it.G, it.SL, it.SLn, it.invSL, kw_base, it.L);
         __syncwarp();
     }
 }
@@ -311,7 +317,7 @@ __device__ __forceinline__ void march(const Cls& c, const It& it, const double* 
 // ring sizes up to 16.  Batches of kDualPF rows per stream, the two streams share the FIFO half and half;
 // the emit buffer holds the C partials in rows [0, PF) and the G partials in rows [PF, 2 PF).
 constexpr int kDualPF = 4;
-template <int MB, typename F>
+template <int MB, typename F, bool DBG = false>
 __device__ __forceinline__ void march_dual(const Cls& c, const It& it, const double* __restrict__ xp1,
                                            const double* __restrict__ xp0, const int rows_valid,
                                            const int rows_min, const int nblk, const F (&T)[MB],
@@ -400,7 +406,7 @@ __device__ __forceinline__ void march_dual(const Cls& c, const It& it, const dou
         }
         if (++bis == it.KB) {
             __syncwarp();
-            score_narrow(c, best, lane, it.G, it.SL, it.SLn, it.invSL, kw_base, it.L);
+            score_narrow<DBG>(c, best, lane, it.G, it.SL, it.SLn, it.invSL, kw_base, it.L);
             __syncwarp();
             kw_base += it.SLn;
             bis = 0;
@@ -409,7 +415,7 @@ __device__ __forceinline__ void march_dual(const Cls& c, const It& it, const dou
     cp_async_wait<0>();
     if (bis > 0) {
         __syncwarp();
-        score_narrow(c, best, lane, it.G, it.SL, it.SLn, it.invSL, kw_base, it.L);
+        score_narrow<DBG>(c, best, lane, it.G, it.SL, it.SLn, it.invSL, kw_base, it.L);
         __syncwarp();
     }
 }
@@ -554,7 +560,7 @@ __device__ __forceinline__ double tmpl_lerp(const double* __restrict__ tm, int n
 
 // One march of the lanes' (segment, column) slots: taps, bounds, then the ring.
 //   seg/col: this lane's slot (active == false: an idle lane, zero taps);  row0: first row of seg.
-template <int MB, bool NARROW, typename F, bool DUAL = false>
+template <int MB, bool NARROW, typename F, bool DUAL = false, bool DBG = false>
 __device__ __forceinline__ void run_march(const Cls& c, const It& it, const int n, const int n_tmpl,
                                           const double tscale, const double* __restrict__ tm,
                                           const double* __restrict__ x, const bool square,
@@ -579,11 +585,11 @@ __device__ __forceinline__ void run_march(const Cls& c, const It& it, const int 
         rows_valid = rv > rows_all ? rows_all : (int)rv;
     }
     const int rows_min = __reduce_min_sync(0xffffffffu, rows_valid);
-    if constexpr (DUAL) march_dual<MB, F>(c, it, x + ebase, xw + ebase, rows_valid, rows_min, nblk, T, lane, best);
-    else march<MB, NARROW, F>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane, best);
+    if constexpr (DUAL) march_dual<MB, F, DBG>(c, it, x + ebase, xw + ebase, rows_valid, rows_min, nblk, T, lane, best);
+    else march<MB, NARROW, F, DBG>(c, it, x + ebase, rows_valid, rows_min, nblk, T, lane, best);
 }
 
-template <int MB, bool NARROW, bool UNIFORM, typename F>
+template <int MB, bool NARROW, bool UNIFORM, typename F, bool DBG = false>
 __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n_tmpl, const double tscale,
                                           const double* __restrict__ tm, const double* __restrict__ x1,
                                           const double* __restrict__ x0, const int lane, Cand& best) {
@@ -605,9 +611,9 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
         const int seg = min(lane / c.stp, it.G - 1);
         const int col = lane - seg * c.stp;      // idle lanes read on behind the last segment (zero taps)
         if constexpr (UNIFORM)
-            run_march<MB, true, F>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best);
+            run_march<MB, true, F, false, DBG>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best);
         else
-            run_march<MB, true, F, true>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best, x0);
+            run_march<MB, true, F, true, DBG>(c, it, n, n_tmpl, tscale, tm, x1, false, active, seg * it.L, col, lane, best, x0);
     } else {
     // ---- wide: window tiles of the table size; the tile's stp columns are cut into nc balanced chunks of
     // at most 32 lanes, one shift march per chunk over all rows of the tile (one segment per warp: a few idle
@@ -653,13 +659,13 @@ __device__ __forceinline__ void run_class(const Cls& c, const int n, const int n
             }
         }
         __syncwarp();
-        score_wide(c, best, lane, k0, nWt, MB - 1);
+        score_wide<DBG>(c, best, lane, k0, nWt, MB - 1);
         __syncwarp();
     }
     }
 }
 
-template <int MB, bool NARROW, bool UNIFORM, typename F>
+template <int MB, bool NARROW, bool UNIFORM, typename F, bool DBG = false>
 __global__ void __launch_bounds__(kRT, 6) k_chi2_ring(TileArgs a, const int* __restrict__ list,
                                                       const int* __restrict__ count, int* __restrict__ next) {
     extern __shared__ double dsm[];                 // per warp: emit buffer, X FIFO, window table
@@ -723,6 +729,7 @@ __global__ void __launch_bounds__(kRT, 6) k_chi2_ring(TileArgs a, const int* __r
     c.fifo = c.part + (unsigned)(kPartRows * kPartPitch * 8);
     c.ctab = c.fifo + (unsigned)(kFifoRows * 32 * 8);
     c.Kt = UNIFORM ? kCW : kCW / 2;
+    c.dbg_d = a.dbg_dchi2; c.dbg_a = a.dbg_depth; c.st0 = st;
     const double tscale = __ddiv_rn((double)(a.n_tmpl - 1), (double)e.D);
     const double* __restrict__ tm = tmpl_in_smem ? s_tmpl : a.tmpl;
     const double* __restrict__ x1 = a.x1 + (long long)pl * a.pitch;
@@ -732,7 +739,7 @@ __global__ void __launch_bounds__(kRT, 6) k_chi2_ring(TileArgs a, const int* __r
     for (int r = 0; r < ncls; ++r) {
         c.off = r * st;
         c.nWr = nW > r ? (nW - r + ncls - 1) / ncls : 0;
-        run_class<MB, NARROW, UNIFORM, F>(c, a.n, a.n_tmpl, tscale, tm, x1, x0, lane, best);
+        run_class<MB, NARROW, UNIFORM, F, DBG>(c, a.n, a.n_tmpl, tscale, tm, x1, x0, lane, best);
     }
 
     // warp-wide lexicographic min on (d, s)
@@ -764,6 +771,14 @@ static void launch_variant_t(const TileArgs& a, int v, cudaStream_t st) {
     const size_t sm = (size_t)(kRW * kWarpSmem) * sizeof(double);
     // (per device, cheap: set on every launch rather than behind a process-wide flag)
     cudaFuncSetAttribute(k_chi2_ring<MB, NARROW, UNIFORM, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if constexpr (sizeof(F) == 8) {
+        if (a.dbg_dchi2) {       // gtls_ring_window_chi2: the same kernel, instantiated to dump every window's score
+            cudaFuncSetAttribute(k_chi2_ring<MB, NARROW, UNIFORM, F, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+            k_chi2_ring<MB, NARROW, UNIFORM, F, true><<<grid, kRT, sm, st>>>(a, a.trial_list + (long long)v * trials, a.trial_count + v,
+                                                                           a.trial_count + kChi2Variants * (1 + kBinBlocks) + v);
+            return;
+        }
+    }
     k_chi2_ring<MB, NARROW, UNIFORM, F><<<grid, kRT, sm, st>>>(a, a.trial_list + (long long)v * trials, a.trial_count + v,
                                                              a.trial_count + kChi2Variants * (1 + kBinBlocks) + v);
 }

@@ -164,6 +164,8 @@ struct TileArgs {
     int chi2_fp32;         // 1: fp32 ring arithmetic in the chi2 kernels (gtls_opts.chi2_fp32)
     const double* gtab;    // [2*(gtab_max+1)] sum g_D, sum g_D^2 for D = 1 .. gtab_max (k_gtab)
     int gtab_max;
+    double* dbg_dchi2;     // debug export only (gtls_ring_window_chi2): per-window dchi2 / depth written by the ring
+    double* dbg_depth;     // kernels' scoring, indexed by start / stride; nullptr in every search
 };
 
 // Arguments of the fused fold / bucket sort / gather / scan fast path (bucket_sort.cu).

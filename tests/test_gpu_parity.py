@@ -161,6 +161,55 @@ def test_window_terms_match_literal_oracle(dt0, tmpl512):
         assert np.allclose(c_out + c_in, co_o + ci_o, rtol=1e-10, atol=0)
 
 
+@pytest.mark.parametrize("cfg,hetero,period,q,dt0", [
+    (3, False, 127.0, 0.0300, 0.05),      # wide 21-ring, one chunk of columns (stride 97)
+    (3, False, 300.0, 0.1000, 0.05),      # wide 21-ring, many chunks (stride 325), several window tiles
+    (3, False, 90.0, 0.0041, 0.05),       # narrow, stride 13 (21-ring)
+    (3, False, 90.0, 0.0015, 0.05),       # narrow, stride 4 (24-ring)
+    (2, False, 11.2, 0.0065, 0.05),       # narrow, stride 1 (direct), D = 27: two classes
+    (2, False, 11.2, 0.0300, 0.01),       # stride 1, five classes of the 21-ring
+    (2, False, 3.3, 0.0800, 0.3),         # few taps: 4-ring wide
+    (2, False, 3.3, 0.0200, 0.11),        # 12-ring narrow
+    (3, True, 127.0, 0.0300, 0.05),       # dy not uniform: wide, C and G marches
+    (2, True, 11.2, 0.0065, 0.05),        # dy not uniform: narrow dual march, stride 1
+    (2, True, 20.0, 0.0450, 0.05),        # dy not uniform: narrow dual march, stride 9
+])
+def test_ring_kernel_scores_every_window_like_the_literal_oracle(cfg, hetero, period, q, dt0):
+    """Every window the hot kernel scores -- not only the per-period minimum: the debug instantiation of
+    k_chi2_ring dumps (dchi2, depth) of each strided start of one trial (gtls_ring_window_chi2); compared with
+    the oracle's literal O(N)-per-window form (Eq. 15 + Eq. 16 - Eq. 11, pinned on the CPU against numpy)."""
+    _cuda()
+    w = gi.make_workload(cfg, hetero=hetero)
+    lc = w.lc
+    st, dep, dchi2, chi0 = g.gtls_ring_window_chi2(lc.t, lc.y, lc.dy, period, q, w.tmpl, dt0=dt0)
+    st_o, dep_o, co_o, ci_o = oracle.window_chi2_literal(lc.t, lc.y, lc.dy, period, q, w.tmpl, dt0)
+    assert np.array_equal(st, st_o)
+    assert not np.any(np.isnan(dchi2)) and not np.any(np.isnan(dep)), "a window the kernel never scored"
+    assert abs(chi0 / oracle.chi2_null(lc.y, lc.dy) - 1) < 1e-12
+    chi2_o = co_o + ci_o
+    assert np.max(np.abs((chi0 + dchi2) - chi2_o) / chi2_o) <= CHI2_RTOL
+    # depths.  (a) Against the literal form: it averages FLUXES ~ 1 (Eq. 12 as printed), and a sum of D nearly
+    # equal terms carries up to D * eps relative error, i.e. D * eps ABSOLUTE in 1 - mean flux (measured on c3,
+    # D = 6501: 1.5e-13, the same for every window); the kernels average deficits.  (b) Against plain numpy
+    # long-double sums of the deficits over the oracle's permutation, on a sample of windows: 1e-9 relative, or
+    # 1e-9 of the deepest window for shallow ones (a window sum is a difference of prefix sums, Eq. 14).
+    n = lc.n
+    D = oracle.points_in_duration(q, n)
+    _, gbar = oracle.resample_template(w.tmpl, D)
+    assert np.allclose(dep, dep_o, rtol=1e-9, atol=4 * D * np.finfo(float).eps / gbar)
+    _, perm = oracle.fold_sort(lc.t, [period], want_phase=False)
+    wt = (1.0 / lc.dy ** 2)[perm[0]].astype(np.longdouble)
+    wr = wt * (1.0 - lc.y)[perm[0]].astype(np.longdouble)
+    pick = np.unique(np.linspace(0, st.size - 1, 64).astype(int))
+    ref = np.array([float(max(wr[(s0 + np.arange(D)) % n].sum() / wt[(s0 + np.arange(D)) % n].sum(), 0) / gbar)
+                    for s0 in st[pick]])
+    assert np.allclose(dep[pick], ref, rtol=1e-9, atol=1e-9 * ref.max())
+    # and the minimum over these windows is what the search reports for this one-trial grid
+    res = g.gtls_search(lc.t, lc.y, lc.dy, np.array([period]), np.array([q]), w.tmpl, dt0=dt0, sde_kernel=0, path=2)
+    k = int(np.argmin(chi0 + dchi2))
+    assert res.best()["start"][0] == st[k] and abs(res.chi2[0] / (chi0 + dchi2[k]) - 1) < 1e-14
+
+
 # ------------------------------------------------------------------------- whole path
 def test_search_c1_full():
     _cuda()
