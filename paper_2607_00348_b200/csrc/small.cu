@@ -235,18 +235,28 @@ __device__ __forceinline__ void sm_march(const SmCls& c, const double* __restric
         PROF_ADD(4, pt1 - pt0);
         const int o0 = b * PF - rho_base;          // table column of the batch's first row
         const unsigned tb = c.tab + (unsigned)(o0 * 8);
+        // two rounds at a time, their loads first: the shared-memory accesses are volatile asm statements that the
+        // compiler keeps in order, so a store between two rounds' loads serialises their latencies
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            if (k < nround) {                      // (warp uniform)
-                const double q0 = rleft[k] > 0 ? lds64(rsrc[k]) : 0.0;
-                const double q1 = rleft[k] > 1 ? lds64(rsrc[k] + 8) : 0.0;
-                const double q2 = rleft[k] > 2 ? lds64(rsrc[k] + 16) : 0.0;
-                const double q3 = rleft[k] > 3 ? lds64(rsrc[k] + 24) : 0.0;
-                double v = (q0 + q1) + (q2 + q3);
-                if (R >= 2) v += __shfl_xor_sync(0xffffffffu, v, 1);
-                if (R >= 4) v += __shfl_xor_sync(0xffffffffu, v, 2);
-                if (R >= 8) v += __shfl_xor_sync(0xffffffffu, v, 4);
-                if (rdst[k] >= 0) sts64(tb + (unsigned)rdst[k], v);
+        for (int k0 = 0; k0 < 4; k0 += 2) {
+            if (k0 < nround) {                     // (warp uniform)
+                double q[2][4], v[2];
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int k = k0 + h;
+                    q[h][0] = rleft[k] > 0 ? lds64(rsrc[k]) : 0.0;
+                    q[h][1] = rleft[k] > 1 ? lds64(rsrc[k] + 8) : 0.0;
+                    q[h][2] = rleft[k] > 2 ? lds64(rsrc[k] + 16) : 0.0;
+                    q[h][3] = rleft[k] > 3 ? lds64(rsrc[k] + 24) : 0.0;
+                }
+#pragma unroll
+                for (int h = 0; h < 2; ++h) v[h] = (q[h][0] + q[h][1]) + (q[h][2] + q[h][3]);
+                if (R >= 2) { v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1); v[1] += __shfl_xor_sync(0xffffffffu, v[1], 1); }
+                if (R >= 4) { v[0] += __shfl_xor_sync(0xffffffffu, v[0], 2); v[1] += __shfl_xor_sync(0xffffffffu, v[1], 2); }
+                if (R >= 8) { v[0] += __shfl_xor_sync(0xffffffffu, v[0], 4); v[1] += __shfl_xor_sync(0xffffffffu, v[1], 4); }
+#pragma unroll
+                for (int h = 0; h < 2; ++h)
+                    if (rdst[k0 + h] >= 0) sts64(tb + (unsigned)rdst[k0 + h], v[h]);
             }
         }
         __syncwarp();                              // the emit buffer is free for the next batch
