@@ -189,7 +189,8 @@ int gtls_search_two_stage(const double* t, const double* y, const double* dy, in
  * k*stride < n (Eq. 18), the start index, the depth a (Eq. 12-13) and dchi2 = chi2(window) - chi2_0 =
  * -2 a C + a^2 G (Eq. 15 + 16 minus the Eq. 11 edge term) exactly as the kernel's scoring step saw them --
  * including every non-minimal window, which gtls_search reduces away.  Host pointers only
- * (opts->pointers_on_device => GTLS_EUNSUPPORTED); uses opts->dt0, device, stream; arrays must hold
+ * (opts->pointers_on_device => GTLS_EUNSUPPORTED); uses opts->dt0, device, stream and opts->path (1: the fused
+ * small-N kernel of gtls_search's path = 1, with its limits; anything else: the general path); arrays must hold
  * ceil(n/stride) entries (n is always enough); *out_chi2_null (may be NULL) = chi2_0.  A window the kernel
  * never scored comes back as NaN.  Returns the number of starts (>= 1) or a negative error code. */
 int64_t gtls_ring_window_chi2(const double* t, const double* y, const double* dy, int64_t n, double period,

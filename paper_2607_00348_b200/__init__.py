@@ -551,15 +551,17 @@ def gtls_window_chi2(t, y, dy, period: float, q: float, tmpl, *, dt0: float = 0.
     return start[:k], depth[:k], c_out[:k], c_in[:k]
 
 
-def gtls_ring_window_chi2(t, y, dy, period: float, q: float, tmpl, *, dt0: float = 0.0):
-    """Every window of one (period, duration fraction) as the ring kernel of the general path scores it
-    (``gtls_ring_window_chi2`` in include/gtls.h; host arrays): (start, depth, dchi2, chi2_null)."""
+def gtls_ring_window_chi2(t, y, dy, period: float, q: float, tmpl, *, dt0: float = 0.0, path: int = 2):
+    """Every window of one (period, duration fraction) as the hot kernel scores it (``gtls_ring_window_chi2`` in
+    include/gtls.h; host arrays): (start, depth, dchi2, chi2_null).  path = 2: the ring kernel of the general
+    path; path = 1: the fused small-N kernel."""
     lib = load_library()
     t, y, dy, tmpl = (np.ascontiguousarray(a, dtype=np.float64) for a in (t, y, dy, tmpl))
     n = int(t.shape[0])
     o = GtlsOpts()
     lib.gtls_opts_default(C.byref(o))
     o.dt0 = float(dt0)
+    o.path = int(path)
     start = np.empty(n, dtype=np.int32)
     depth, dchi2 = np.empty(n), np.empty(n)
     c0 = C.c_double(0.0)

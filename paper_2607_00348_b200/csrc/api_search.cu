@@ -204,7 +204,7 @@ static int search_impl(const double* t, const double* y, const double* dy, int64
     const bool small_ok = uniform && o.top_k == 0 && o.chi2_fp32 == 0 && n <= 65535 &&
                           small_path_fits((int)n, gtab_max, n_dur, o.dt0);
     if (o.path == 1 && !small_ok) return GTLS_EUNSUPPORTED;
-    const bool use_small = small_ok && o.path != 2 && !dbg_d;
+    const bool use_small = small_ok && o.path != 2 && (!dbg_d || o.path == 1);   // (the debug export names its path)
     int tile = 0;
     SdeScratch sc;
     unsigned long long counters[2];
@@ -221,6 +221,7 @@ static int search_impl(const double* t, const double* y, const double* dy, int64
         sa.curve_off = d_off; sa.per_off = d_off + 2;
         sa.t = d_t; sa.wr = d_wr; sa.info = d_info; sa.periods = d_per; sa.durs = d_dur; sa.tmpl = d_tmpl;
         sa.gtab = gtab_dev; sa.out_chi2 = d_chi2; sa.out_best = d_best; sa.counters = d_counters; sa.queue = d_queue;
+        sa.dbg_dchi2 = dbg_d; sa.dbg_depth = dbg_a;
         int sms = 0;
         CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, o.device));
         tm.mark(4);
@@ -394,7 +395,8 @@ int64_t gtls_ring_window_chi2(const double* t, const double* y, const double* dy
     if (!d_a) return GTLS_ENOMEM;
     CU(cudaMemsetAsync(d_d, 0xff, nW * 8, st));                   // NaN: a window the kernel did not score stays visible
     CU(cudaMemsetAsync(d_a, 0xff, nW * 8, st));
-    o.path = 2; o.sde_kernel = 0; o.period_tile = 0; o.dur_per_period = 0; o.stats = nullptr;
+    o.path = o.path == 1 ? 1 : 2;          // 1: the fused small-N kernel (GTLS_EUNSUPPORTED where it does not apply)
+    o.sde_kernel = 0; o.period_tile = 0; o.dur_per_period = 0; o.stats = nullptr;
     o.workspace = nullptr; o.workspace_bytes = 0;
     double chi2 = 0.0;
     gtls_summary summ;

@@ -255,6 +255,8 @@ struct SmallArgs {
     unsigned long long* counters; // [n_curves][2]: windows, window points
     unsigned long long* queue;    // work counter (zeroed by the caller)
     int xs_len, n_max;            // set by launch_tls_small
+    double* dbg_dchi2;            // debug export only (gtls_ring_window_chi2, path = 1): per-window dchi2 / depth of a
+    double* dbg_depth;            // one-curve, one-period, one-duration call, indexed by start / stride; nullptr otherwise
 };
 size_t small_smem_bytes(int n_max, int d_max);
 // dy uniform is the caller's check; this one covers sizes: shared memory, n_dur, class strides <= 31

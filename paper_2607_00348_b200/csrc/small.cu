@@ -96,6 +96,8 @@ struct SmCls {
     int zidx;                      // index of a zero cell of x1 (reads beyond the pad are redirected to it)
     unsigned part;                 // this warp's emit buffer
     unsigned tab;                  // this warp's window table (kSmTab doubles)
+    // debug instantiation only (gtls_ring_window_chi2 with path = 1): every window's dchi2 / depth by start / st0
+    double* dbg_d; double* dbg_a; int st0;
 };
 
 // Template taps of one lane: g_D[m * stp + col] for m = m0 .. m0 + count - 1 (linear interpolation at the cell
@@ -115,7 +117,8 @@ __device__ __noinline__ void sm_taps(const unsigned tl, const int m0, const int 
 // that completed at row rho_base + o of segment g.  Coalesced over the table: 32 windows per step, every
 // lane busy, four steps in flight.  Within a lane the starts ascend, so a strict '<' keeps the first of equal
 // scores.  (One copy for every ring size: not inlined, everything passed by value.)
-struct SmScore { unsigned tab, ss; int D, stp, off, nWr, G, L, lsl, kw_base, count; double G_u, inv_den; };
+struct SmScore { unsigned tab, ss; int D, stp, off, nWr, G, L, lsl, kw_base, count; double G_u, inv_den; double* dbg_d; double* dbg_a; int st0; };
+template <bool DBG>
 __device__ __noinline__ SmCand sm_score_slice(const SmScore c, SmCand best, const int lane) {
     const int SL = 1 << c.lsl;
     double bd = best.has ? best.d : __longlong_as_double(0x7ff0000000000000LL), bdepth = best.depth;
@@ -143,6 +146,7 @@ __device__ __noinline__ SmCand sm_score_slice(const SmScore c, SmCand best, cons
             const double swr = fmax(hi[k] - lo[k], 0.0);
             const double depth = swr * c.inv_den;
             const double d = -2.0 * depth * C[k] + (depth * depth) * c.G_u;
+            if constexpr (DBG) { if (sidx[k] >= 0) { c.dbg_d[sidx[k] / c.st0] = d; c.dbg_a[sidx[k] / c.st0] = depth; } }
             // (a lane's previous best from an EARLIER class may have a later start: the lexicographic rule)
             const bool take = sidx[k] >= 0 && (d < bd || (d == bd && sidx[k] < bs));
             bd = take ? d : bd; bdepth = take ? depth : bdepth; bs = take ? sidx[k] : bs;
@@ -152,7 +156,7 @@ __device__ __noinline__ SmCand sm_score_slice(const SmScore c, SmCand best, cons
     return best;
 }
 
-template <int MB>
+template <int MB, bool DBG>
 __device__ __forceinline__ void sm_march(const SmCls& c, const double* __restrict__ tm, const int n_tmpl,
                                          const double tscale, const int lane, SmCand& best) {
     constexpr int PF = kSmPF, XQ = 4, LA = 3;
@@ -213,7 +217,7 @@ __device__ __forceinline__ void sm_march(const SmCls& c, const double* __restric
     }
     SmScore sc;
     sc.tab = c.tab; sc.ss = c.ss; sc.D = c.D; sc.stp = c.stp; sc.off = c.off; sc.nWr = c.nWr; sc.G = G; sc.L = L; sc.lsl = lsl;
-    sc.G_u = c.G_u; sc.inv_den = c.inv_den;
+    sc.G_u = c.G_u; sc.inv_den = c.inv_den; sc.dbg_d = c.dbg_d; sc.dbg_a = c.dbg_a; sc.st0 = c.st0;
     sc.count = min(kSmTab, G << lsl);              // table entries in use
     __syncwarp();
 
@@ -265,7 +269,7 @@ __device__ __forceinline__ void sm_march(const SmCls& c, const double* __restric
         if (o0 + PF == SL || b == nbat - 1) {      // the slice is full (or the march ends): score and recycle it
             __syncwarp();
             sc.kw_base = rho_base - (MB - 1);
-            best = sm_score_slice(sc, best, lane);
+            best = sm_score_slice<DBG>(sc, best, lane);
             __syncwarp();
             rho_base += SL;
             PROF_T(pt3);
@@ -278,7 +282,7 @@ __device__ __forceinline__ void sm_march(const SmCls& c, const double* __restric
 // so each row's completed window is scored in place (a5, a8) -- no emit buffer, no table.  32 segments of L
 // consecutive windows, L odd so that the lanes' x1 / S1 reads (L doubles apart) do not share banks; within a
 // lane the starts ascend, so a strict '<' keeps the first of equal scores.
-template <int MB>
+template <int MB, bool DBG>
 __device__ __forceinline__ void sm_march_direct(const SmCls& c, const double* __restrict__ tm, const int n_tmpl,
                                                 const double tscale, const int lane, SmCand& best) {
     constexpr int PF = kSmPF, XQ = 4, LA = 3;
@@ -324,6 +328,7 @@ __device__ __forceinline__ void sm_march_direct(const SmCls& c, const double* __
             const double swr = fmax(hi - lo, 0.0);
             const double depth = swr * c.inv_den;
             const double d = -2.0 * depth * acc[MB] + (depth * depth) * c.G_u;
+            if constexpr (DBG) { if (ok) { c.dbg_d[s / c.st0] = d; c.dbg_a[s / c.st0] = depth; } }
             const bool take = ok && d < bd;
             bd = take ? d : bd; bdepth = take ? depth : bdepth; bs = take ? s : bs;
         }
@@ -331,18 +336,19 @@ __device__ __forceinline__ void sm_march_direct(const SmCls& c, const double* __
     if (bs >= 0) offer(best, bd, bs, bdepth);
 }
 
+template <bool DBG>
 __device__ __forceinline__ void sm_run_unit(const SmCls& c, const int taps, const double* __restrict__ tm,
                                             const int n_tmpl, const double tscale, const int lane, SmCand& best) {
     // few ring sizes: the instruction cache, not the FP64 pipe, is what this kernel runs out of (twelve
     // warps in different phases of different bodies), so a ring is allowed to be up to twice its taps
     if (c.stp == 1) {
-        if (taps > 12) sm_march_direct<24>(c, tm, n_tmpl, tscale, lane, best);
-        else sm_march_direct<12>(c, tm, n_tmpl, tscale, lane, best);
+        if (taps > 12) sm_march_direct<24, DBG>(c, tm, n_tmpl, tscale, lane, best);
+        else sm_march_direct<12, DBG>(c, tm, n_tmpl, tscale, lane, best);
         return;
     }
-    if (taps > 16) sm_march<24>(c, tm, n_tmpl, tscale, lane, best);
-    else if (taps > 8) sm_march<16>(c, tm, n_tmpl, tscale, lane, best);
-    else sm_march<8>(c, tm, n_tmpl, tscale, lane, best);
+    if (taps > 16) sm_march<24, DBG>(c, tm, n_tmpl, tscale, lane, best);
+    else if (taps > 8) sm_march<16, DBG>(c, tm, n_tmpl, tscale, lane, best);
+    else sm_march<8, DBG>(c, tm, n_tmpl, tscale, lane, best);
 }
 
 // strict total order (key32, fp64 phase, index) == (fp64 phase, index)
@@ -354,6 +360,7 @@ __device__ __noinline__ bool sm_key_less(const u64 a, const u64 b, const double*
     return (u32)a < (u32)b;
 }
 
+template <bool DBG>
 __global__ void __launch_bounds__(kSmThreads, 1) k_tls_small(SmallArgs a) {
     extern __shared__ __align__(16) unsigned char sm_raw[];
     double* const xs = reinterpret_cast<double*>(sm_raw);                       // [a.xs_len]  (keysB during the sort)
@@ -580,7 +587,8 @@ __global__ void __launch_bounds__(kSmThreads, 1) k_tls_small(SmallArgs a) {
                 if (c.nWr > 0) {
                     const int taps = (e.D + c.stp - 1) / c.stp;
                     const double tscale = __ddiv_rn((double)(a.n_tmpl - 1), (double)e.D);
-                    sm_run_unit(c, taps, tm, a.n_tmpl, tscale, lane, best);
+                    c.dbg_d = a.dbg_dchi2; c.dbg_a = a.dbg_depth; c.st0 = e.st;
+                    sm_run_unit<DBG>(c, taps, tm, a.n_tmpl, tscale, lane, best);
                 }
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) {
@@ -680,10 +688,16 @@ int launch_tls_small(SmallArgs& a, int n_max, int d_max, int sm_count, cudaStrea
     a.xs_len = (int)(((size_t)n_max + d_max + 48 + 1) & ~(size_t)1);
     a.n_max = n_max;
     const size_t sm = small_smem_bytes(n_max, d_max);
-    cudaError_t e = cudaFuncSetAttribute(k_tls_small, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    if (e != cudaSuccess) return (int)e;
     long long grid = a.n_items < sm_count ? a.n_items : sm_count;
-    k_tls_small<<<(unsigned)grid, kSmThreads, sm, st>>>(a);
+    if (a.dbg_dchi2) {             // gtls_ring_window_chi2 with path = 1: the instantiation that dumps every window's score
+        cudaError_t e = cudaFuncSetAttribute(k_tls_small<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+        if (e != cudaSuccess) return (int)e;
+        k_tls_small<true><<<(unsigned)grid, kSmThreads, sm, st>>>(a);
+        return (int)cudaGetLastError();
+    }
+    cudaError_t e = cudaFuncSetAttribute(k_tls_small<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (e != cudaSuccess) return (int)e;
+    k_tls_small<false><<<(unsigned)grid, kSmThreads, sm, st>>>(a);
 #ifdef GTLS_SMALL_PROF
     cudaStreamSynchronize(st);
     small_prof_dump();

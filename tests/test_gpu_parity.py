@@ -161,27 +161,35 @@ def test_window_terms_match_literal_oracle(dt0, tmpl512):
         assert np.allclose(c_out + c_in, co_o + ci_o, rtol=1e-10, atol=0)
 
 
-@pytest.mark.parametrize("cfg,hetero,period,q,dt0", [
-    (3, False, 127.0, 0.0300, 0.05),      # wide 21-ring, one chunk of columns (stride 97)
-    (3, False, 300.0, 0.1000, 0.05),      # wide 21-ring, many chunks (stride 325), several window tiles
-    (3, False, 90.0, 0.0041, 0.05),       # narrow, stride 13 (21-ring)
-    (3, False, 90.0, 0.0015, 0.05),       # narrow, stride 4 (24-ring)
-    (2, False, 11.2, 0.0065, 0.05),       # narrow, stride 1 (direct), D = 27: two classes
-    (2, False, 11.2, 0.0300, 0.01),       # stride 1, five classes of the 21-ring
-    (2, False, 3.3, 0.0800, 0.3),         # few taps: 4-ring wide
-    (2, False, 3.3, 0.0200, 0.11),        # 12-ring narrow
-    (3, True, 127.0, 0.0300, 0.05),       # dy not uniform: wide, C and G marches
-    (2, True, 11.2, 0.0065, 0.05),        # dy not uniform: narrow dual march, stride 1
-    (2, True, 20.0, 0.0450, 0.05),        # dy not uniform: narrow dual march, stride 9
+@pytest.mark.parametrize("cfg,hetero,period,q,dt0,path", [
+    (2, False, 11.2, 0.0040, 0.05, 1),    # fused kernel: stride 1, D = 16, scored in place (24-ring)
+    (2, False, 11.2, 0.0022, 0.05, 1),    # fused kernel: stride 1, D = 9 (12-ring)
+    (2, False, 11.2, 0.0200, 0.05, 1),    # fused kernel: stride 4, eight segments (24-ring)
+    (2, False, 30.0, 0.0700, 0.05, 1),    # fused kernel: stride 14, two segments, four lanes per column sum
+    (2, False, 30.0, 0.1400, 0.05, 1),    # fused kernel: stride 29, one segment, eight lanes per column sum
+    (2, False, 30.0, 0.0300, 0.00, 1),    # fused kernel: every start, D = 125 in six classes (stride 6)
+    (1, False, 3.7, 0.0500, 0.12, 1),     # fused kernel: nine taps (16-ring), c1
+    (3, False, 127.0, 0.0300, 0.05, 2),   # wide 21-ring, one chunk of columns (stride 97)
+    (3, False, 300.0, 0.1000, 0.05, 2),      # wide 21-ring, many chunks (stride 325), several window tiles
+    (3, False, 90.0, 0.0041, 0.05, 2),       # narrow, stride 13 (21-ring)
+    (3, False, 90.0, 0.0015, 0.05, 2),       # narrow, stride 4 (24-ring)
+    (2, False, 11.2, 0.0065, 0.05, 2),       # narrow, stride 1 (direct), D = 27: two classes
+    (2, False, 11.2, 0.0300, 0.01, 2),       # stride 1, five classes of the 21-ring
+    (2, False, 3.3, 0.0800, 0.3, 2),         # few taps: 4-ring wide
+    (2, False, 3.3, 0.0200, 0.11, 2),        # 12-ring narrow
+    (3, True, 127.0, 0.0300, 0.05, 2),       # dy not uniform: wide, C and G marches
+    (2, True, 11.2, 0.0065, 0.05, 2),        # dy not uniform: narrow dual march, stride 1
+    (2, True, 20.0, 0.0450, 0.05, 2),        # dy not uniform: narrow dual march, stride 9
 ])
-def test_ring_kernel_scores_every_window_like_the_literal_oracle(cfg, hetero, period, q, dt0):
-    """Every window the hot kernel scores -- not only the per-period minimum: the debug instantiation of
-    k_chi2_ring dumps (dchi2, depth) of each strided start of one trial (gtls_ring_window_chi2); compared with
+def test_ring_kernel_scores_every_window_like_the_literal_oracle(cfg, hetero, period, q, dt0, path):
+    """Every window the hot kernels score -- not only the per-period minimum: the debug instantiations of
+    k_chi2_ring (path 2) and of the fused k_tls_small (path 1) dump (dchi2, depth) of each strided start of one
+    trial (gtls_ring_window_chi2); compared with
     the oracle's literal O(N)-per-window form (Eq. 15 + Eq. 16 - Eq. 11, pinned on the CPU against numpy)."""
     _cuda()
     w = gi.make_workload(cfg, hetero=hetero)
     lc = w.lc
-    st, dep, dchi2, chi0 = g.gtls_ring_window_chi2(lc.t, lc.y, lc.dy, period, q, w.tmpl, dt0=dt0)
+    st, dep, dchi2, chi0 = g.gtls_ring_window_chi2(lc.t, lc.y, lc.dy, period, q, w.tmpl, dt0=dt0, path=path)
     st_o, dep_o, co_o, ci_o = oracle.window_chi2_literal(lc.t, lc.y, lc.dy, period, q, w.tmpl, dt0)
     assert np.array_equal(st, st_o)
     assert not np.any(np.isnan(dchi2)) and not np.any(np.isnan(dep)), "a window the kernel never scored"
@@ -205,7 +213,7 @@ def test_ring_kernel_scores_every_window_like_the_literal_oracle(cfg, hetero, pe
                     for s0 in st[pick]])
     assert np.allclose(dep[pick], ref, rtol=1e-9, atol=1e-9 * ref.max())
     # and the minimum over these windows is what the search reports for this one-trial grid
-    res = g.gtls_search(lc.t, lc.y, lc.dy, np.array([period]), np.array([q]), w.tmpl, dt0=dt0, sde_kernel=0, path=2)
+    res = g.gtls_search(lc.t, lc.y, lc.dy, np.array([period]), np.array([q]), w.tmpl, dt0=dt0, sde_kernel=0, path=path)
     k = int(np.argmin(chi0 + dchi2))
     assert res.best()["start"][0] == st[k] and abs(res.chi2[0] / (chi0 + dchi2[k]) - 1) < 1e-14
 
