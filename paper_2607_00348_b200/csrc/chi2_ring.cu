@@ -47,11 +47,14 @@ constexpr int kPartPitch = 36;           // doubles per slot row of the per-warp
 constexpr int kPartRows = 16;            // two emit buffers of max PfRows rows (pipelined column sums)
 constexpr int kFifoBatches = 3;          // batches of PfRows rows per lane in the cp.async FIFO
 constexpr int kFifoRows = 24;            // >= kFifoBatches * max PfRows
-constexpr int kCW = 704;                 // window-table doubles per warp (>= 32 * 21)
+constexpr int kCW = 704;                 // window-table doubles per warp, narrow variants (>= 32 * 21)
+constexpr int kCWWide = 2488;            // wide variants: window tiles of 2 460 windows (fewer warm-up rows, tap set-ups and FIFO primes
+                                         // per trial).  Measured on c4, chi2 stage: 704 entries / 4 CTAs per SM 4.63 s, 1720 / 4: 4.61 s,
+                                         // 2488 / 3: 4.52 s, 3128 / 3: 4.66 s (the tile's span outgrows what stays in the L2 between chunks)
 constexpr int kTmplSmem = 512;           // template nodes cached in shared memory
 constexpr unsigned kGridCap = 148u * 6u;   // CTAs per launch: the 6 resident CTAs per SM, persistent (dynamic trial queue)
-constexpr unsigned kGridCapWide = 148u * 4u;
-constexpr int kWarpSmem = kPartRows * kPartPitch + kFifoRows * 32 + kCW;   // doubles per warp
+constexpr unsigned kGridCapWide = 148u * 3u;
+template <bool NARROW> struct WarpSmem { static constexpr int v = kPartRows * kPartPitch + kFifoRows * 32 + (NARROW ? kCW : kCWWide); };   // doubles per warp
 
 struct Cand { double d; double depth; int s; int has; };
 
@@ -724,11 +727,11 @@ __global__ void __launch_bounds__(kRT, 6) k_chi2_ring(TileArgs a, const int* __r
     c.inv_den_u = __ddiv_rn(1.0, ((double)e.D * a.w_uniform) * e.gbar);
     c.s1 = a.s1 + (long long)pl * a.spitch;
     c.s0 = a.s0 + (long long)pl * a.spitch;
-    double* const wsm = dsm + warp * kWarpSmem;
+    double* const wsm = dsm + warp * WarpSmem<NARROW>::v;
     c.part = (unsigned)__cvta_generic_to_shared(wsm);
     c.fifo = c.part + (unsigned)(kPartRows * kPartPitch * 8);
     c.ctab = c.fifo + (unsigned)(kFifoRows * 32 * 8);
-    c.Kt = UNIFORM ? kCW : kCW / 2;
+    c.Kt = NARROW ? (UNIFORM ? kCW : kCW / 2) : (UNIFORM ? kCWWide : kCWWide / 2);
     c.dbg_d = a.dbg_dchi2; c.dbg_a = a.dbg_depth; c.st0 = st;
     const double tscale = __ddiv_rn((double)(a.n_tmpl - 1), (double)e.D);
     const double* __restrict__ tm = tmpl_in_smem ? s_tmpl : a.tmpl;
@@ -764,11 +767,11 @@ static void launch_variant_t(const TileArgs& a, int v, cudaStream_t st) {
     const long long trials = (long long)a.tile * a.n_dur;
     unsigned grid = (unsigned)((trials + kRW - 1) / kRW);           // surplus CTAs exit at once
     if (grid > kGridCap) grid = kGridCap;                           // one wave of persistent CTAs
-    // wide variants: 4 of the 6 CTA slots per SM.  The shift march hides its latencies inside a warp (8 warps per SM
-    // run within 1 % of 12), and fewer trials in flight are fewer periods whose x1 competes for the L2
+    // wide variants: 3 CTAs per SM (their 60 KB of shared memory each: kCWWide).  The shift march hides its latencies
+    // inside a warp (6 - 8 warps per SM run within 1 % of 12), and fewer trials in flight are fewer periods whose x1 competes for the L2
     // (c4: 60 -> 36 GB of DRAM reads per 4144-period tile of the dominant variant, SM clock under the power cap 1845 -> 1890 MHz)
     if (!NARROW && grid > kGridCapWide) grid = kGridCapWide;
-    const size_t sm = (size_t)(kRW * kWarpSmem) * sizeof(double);
+    const size_t sm = (size_t)(kRW * WarpSmem<NARROW>::v) * sizeof(double);
     // (per device, cheap: set on every launch rather than behind a process-wide flag)
     cudaFuncSetAttribute(k_chi2_ring<MB, NARROW, UNIFORM, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if constexpr (sizeof(F) == 8) {
