@@ -92,6 +92,12 @@ inline int pitch_for(long long n, double q_max) {
     return (int)((n + dmax + 7) / 8 * 8);
 }
 
+// per-period bytes of the bucket sort's scratch (16-bit CTA histograms, bucket starts, CTA offsets, flags)
+inline size_t sort_scratch_bytes(long long n) {
+    const size_t nbk = (size_t)bucket_count_for((int)n), ncta = (size_t)bucket_cta_count((int)n);
+    return ncta * nbk * (sizeof(unsigned short) + sizeof(u32)) + (nbk + 3) * sizeof(u32) + 64;
+}
+
 inline Sizes workspace_sizes(long long n, long long n_per, int n_dur, double q_max, bool uniform) {
     Sizes s;
     const int pitch = pitch_for(n, q_max);
@@ -105,7 +111,7 @@ inline Sizes workspace_sizes(long long n, long long n_per, int n_dur, double q_m
               2 * align_up(kXMargin * sizeof(double));
     s.per_period = 2 * n * sizeof(u64) + 256ull * nt * sizeof(u32) + n_dur * sizeof(DurEntry) +
                    n_dur * sizeof(Partial) + (size_t)kChi2Variants * n_dur * sizeof(int) +
-                   n * sizeof(u32) + (4ull * kMaxBuckets + 3) * sizeof(u32) + 3ull * kMaxBuckets * sizeof(double) +
+                   n * sizeof(u32) + sort_scratch_bytes(n) +
                    (uniform ? 1 : 2) * ((size_t)pitch + spitch) * sizeof(double);
     return s;
 }
@@ -118,8 +124,8 @@ constexpr long long kFinishSlots = GTLS_FIN_SLOTS;
 inline int auto_tile(long long n_per, const Sizes& s, size_t budget) {
     long long t = (long long)(budget / s.per_period);
     if (t > 8192) t = 8192;
-    // k_bucket_finish runs one CTA per period, kFinishSlots of them at a time (148 SMs x 5 CTAs): a tile
-    // that is a multiple of that leaves no partly filled last round
+    // k_bucket_prefix and k_pad_scan run one CTA per period, 2 - 4 per SM at a time: a tile that is a multiple of
+    // kFinishSlots (148 SMs x 4) leaves no partly filled last round
     if (t >= kFinishSlots && t < n_per) t -= t % kFinishSlots;
     if (t > n_per) t = n_per;
     if (t < 1) t = 1;
@@ -129,8 +135,8 @@ inline int auto_tile(long long n_per, const Sizes& s, size_t budget) {
 constexpr size_t kDefaultTileBudget = 24ull << 30;  // bytes of per-tile scratch when automatic
 
 
-struct SortScratch { u32* hist; u32* start; u32* cursor; int* fb_flag; int* fb_list; int* fb_count; };
-bool take_sort_scratch(Arena& ar, size_t tile, int nbk, SortScratch& sc);
+struct SortScratch { unsigned short* hist; u32* start; u32* rel; int* fb_flag; int* fb_list; int* fb_count; };
+bool take_sort_scratch(Arena& ar, size_t tile, int n, SortScratch& sc);
 // Steps a1-a4 for the tile described by `a` (api_search.cu)
 void run_fold_sort_scan(TileArgs& a, const SortScratch& sc, double* x2, double* s2, int pad_override,
                         bool sort_only, double* phase_out, cudaStream_t st, int* launches);

@@ -16,9 +16,8 @@ int gtls_fold_sort(const double* t, int64_t n, const double* periods, int64_t n_
     cudaStream_t st = (cudaStream_t)o.stream;
     const bool dev = o.pointers_on_device != 0;
     const int nt = (int)((n + kRadixTile - 1) / kRadixTile);
-    const int nbk = bucket_count_for((int)n);
     const size_t per_period = 2 * n * sizeof(u64) + 256ull * nt * sizeof(u32) + n * sizeof(u32) +
-                              (4ull * nbk + 1) * sizeof(u32) + 3ull * nbk * sizeof(double) +
+                              sort_scratch_bytes(n) + 1024 +
                               (dev ? 0 : n * (sizeof(double) + sizeof(int32_t))) + 1024;
     long long tile = (long long)((1ull << 30) / per_period);
     if (o.period_tile > 0) tile = o.period_tile;
@@ -37,7 +36,7 @@ int gtls_fold_sort(const double* t, int64_t n, const double* periods, int64_t n_
     a.keys_b = ar.take<u64>((size_t)tile * n);
     a.counts = ar.take<u32>((size_t)tile * 256 * nt);
     SortScratch ssc;
-    if (!take_sort_scratch(ar, (size_t)tile, nbk, ssc)) return GTLS_ENOMEM;
+    if (!take_sort_scratch(ar, (size_t)tile, (int)n, ssc)) return GTLS_ENOMEM;
     double* d_phase = dev ? nullptr : (out_phase ? ar.take<double>((size_t)tile * n) : nullptr);
     int32_t* d_perm = dev ? nullptr : ar.take<int32_t>((size_t)tile * n);
     if (!a.counts || (!dev && !d_perm)) return GTLS_ENOMEM;
@@ -97,7 +96,7 @@ static int one_period_scan(const double* t, const double* y, const double* dy, i
     a.keys_a = ar.take<u64>(n); a.keys_b = ar.take<u64>(n); a.counts = ar.take<u32>(256ull * nt);
     a.perm = ar.take<u32>(n);
     SortScratch ssc;
-    if (!take_sort_scratch(ar, 1, bucket_count_for((int)n), ssc)) return GTLS_ENOMEM;
+    if (!take_sort_scratch(ar, 1, (int)n, ssc)) return GTLS_ENOMEM;
     a.x1 = ar.take<double>(pitch); a.x0 = ar.take<double>(pitch);
     double* x2 = ar.take<double>(pitch);
     a.s1 = ar.take<double>(spitch); a.s0 = ar.take<double>(spitch);

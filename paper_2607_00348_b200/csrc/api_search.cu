@@ -7,10 +7,11 @@
 namespace gtls {
 namespace api {
 
-bool take_sort_scratch(Arena& ar, size_t tile, int nbk, SortScratch& sc) {
-    sc.hist = ar.take<u32>(tile * nbk);
+bool take_sort_scratch(Arena& ar, size_t tile, int n, SortScratch& sc) {
+    const size_t nbk = (size_t)bucket_count_for(n), ncta = (size_t)bucket_cta_count(n);
+    sc.hist = ar.take<unsigned short>(tile * ncta * nbk);
     sc.start = ar.take<u32>(tile * (nbk + 1));
-    sc.cursor = ar.take<u32>(tile * nbk);
+    sc.rel = ar.take<u32>(tile * ncta * nbk);
     sc.fb_flag = ar.take<int>(tile);
     sc.fb_list = ar.take<int>(tile);
     sc.fb_count = ar.take<int>(1);
@@ -38,11 +39,12 @@ void run_fold_sort_scan(TileArgs& a, const SortScratch& sc, double* x2, double* 
         memset(&b, 0, sizeof(b));
         b.n = a.n; b.tile = a.tile; b.p0 = a.p0; b.n_dur = a.n_dur; b.pad_override = pad_override;
         b.nbk = bucket_count_for(a.n);
+        b.ncta = bucket_cta_count(a.n);
         int lg = 0; while ((1 << lg) < b.nbk) ++lg;
         b.shift = 32 - lg;
         b.pitch = a.pitch; b.spitch = a.spitch;
         b.t = a.t; b.wr = a.wr; b.w = a.w; b.wr2 = a.wr2; b.periods = a.periods; b.durtab = a.durtab;
-        b.hist = sc.hist; b.start = sc.start; b.cursor = sc.cursor;
+        b.hist = sc.hist; b.start = sc.start; b.rel = sc.rel;
         b.fb_flag = sc.fb_flag; b.fb_list = sc.fb_list; b.fb_count = sc.fb_count;
         b.keys = a.keys_b; b.perm = a.perm;
         b.x1 = a.x1; b.s1 = a.s1; b.x0 = a.x0; b.s0 = a.s0; b.x2 = x2; b.s2 = s2;
@@ -255,7 +257,7 @@ static int search_impl(const double* t, const double* y, const double* dy, int64
         a.counts = ws.take<u32>((size_t)tile * 256 * nt);
         a.perm = ws.take<u32>((size_t)tile * n);
         SortScratch ssc;
-        if (!take_sort_scratch(ws, (size_t)tile, bucket_count_for((int)n), ssc)) return GTLS_ENOMEM;
+        if (!take_sort_scratch(ws, (size_t)tile, (int)n, ssc)) return GTLS_ENOMEM;
         a.durtab = ws.take<DurEntry>((size_t)tile * n_dur);
         a.gtab = gtab_dev; a.gtab_max = gtab_max;
         a.partial = ws.take<Partial>((size_t)tile * n_dur);

@@ -69,10 +69,10 @@ __host__ __device__ __forceinline__ int chi2_ring_index(int taps) {
 }
 
 // bucket sort (bucket_sort.cu)
-constexpr int kMaxBuckets = 256;      // buckets per period (power of two)
+constexpr int kMaxBuckets = 2048;     // buckets per period (power of two)
 #ifndef GTLS_BUCKET_TARGET
-#define GTLS_BUCKET_TARGET 1100
-#define GTLS_BUCKET_CAP 1536
+#define GTLS_BUCKET_TARGET 280
+#define GTLS_BUCKET_CAP 384
 #endif
 constexpr int kBucketTarget = GTLS_BUCKET_TARGET;   // aimed-at mean bucket size
 constexpr int kBucketCap = GTLS_BUCKET_CAP;      // largest bucket the shared-memory sort takes; beyond: LSD fallback
@@ -171,15 +171,16 @@ struct TileArgs {
 // Arguments of the fused fold / bucket sort / gather / scan fast path (bucket_sort.cu).
 struct BucketArgs {
     int n, tile, nbk, shift;   // points, periods in the tile, buckets per period, 32 - log2(nbk)
+    int ncta;                  // count / scatter CTAs per period (bucket_cta_count(n))
     long long p0;
     int n_dur, pad_override;   // pad = max D of the period's durtab row unless pad_override >= 0
     int pitch, spitch;
     const double* t; const double* wr; const double* w; const double* wr2;
     const double* periods;
     const DurEntry* durtab;
-    u32* hist;                 // [tile*nbk]
+    unsigned short* hist;      // [tile*ncta*nbk] keys of every count CTA per bucket
     u32* start;                // [tile*(nbk+1)]
-    u32* cursor;               // [tile*nbk]
+    u32* rel;                  // [tile*ncta*nbk] where a CTA's keys start inside the bucket
     int* fb_flag;              // [tile] 1: a bucket of this period exceeded kBucketCap (LSD path takes it)
     int* fb_list;              // [tile] those periods, any order
     int* fb_count;             // [1]
@@ -188,6 +189,7 @@ struct BucketArgs {
     double* x1; double* s1; double* x0; double* s0; double* x2; double* s2;
 };
 int bucket_count_for(int n);
+int bucket_cta_count(int n);
 // count + bucket starts + fallback list; then (after the caller forked the fallback path) scatter + finish + pad
 void launch_bucket_sort_head(const BucketArgs& b, cudaStream_t st);
 void launch_bucket_sort_tail(const BucketArgs& b, bool has0, bool has2, bool sort_only, cudaStream_t st);

@@ -78,7 +78,8 @@ def test_fold_sort_ties_and_tiny_inputs():
     ph, perm = g.gtls_fold_sort(t, np.array([1.0, 0.5]))
     ph_o, pm_o = oracle.fold_sort(t, np.array([1.0, 0.5]))
     assert np.array_equal(perm, pm_o) and np.array_equal(ph.view(np.uint64), ph_o.view(np.uint64))
-    for n in (1, 2, 3, 31, 33, 2047, 2048, 2049):           # ragged tails around the radix tile
+    # ragged tails around the radix tile (2048) and around the count / scatter CTAs of the bucket path (4096)
+    for n in (1, 2, 3, 31, 33, 2047, 2048, 2049, 4095, 4096, 4097, 8193, 12289):
         t = np.sort(rng.uniform(0, 50, n))
         _, perm = g.gtls_fold_sort(t, np.array([0.7, 3.3]))
         _, pm_o = oracle.fold_sort(t, np.array([0.7, 3.3]))
@@ -86,7 +87,7 @@ def test_fold_sort_ties_and_tiny_inputs():
 
 
 def test_fold_sort_clustered_phases_take_the_lsd_fallback(tmpl512):
-    """More than kBucketCap (1536) points share one phase bucket: the bucket fast path raises its
+    """More than kBucketCap (384) points share one phase bucket: the bucket fast path raises its
     fallback flag and the call is repeated on the LSD radix path; results must not change."""
     _cuda()
     rng = np.random.default_rng(11)
@@ -243,8 +244,8 @@ def test_search_c2_full():
 def test_search_c4_one_full_automatic_tile():
     """The 3000-day curve on 4144 + 600 CONSECUTIVE periods from the middle of the Ofir grid: one full
     automatic period tile (period_tile == 4144, the launch configuration bench.py times: 124 320 trials
-    binned per tile, the persistent ring-kernel grids, the side stream, 592 resident k_bucket_finish
-    CTAs) plus a ragged second tile, every chi2, index, t0 and depth against the oracle."""
+    binned per tile, the persistent ring-kernel grids, the side stream, 2.1 M (period, bucket) sort
+    units) plus a ragged second tile, every chi2, index, t0 and depth against the oracle."""
     _cuda()
     w0 = gi.make_workload(4)
     p0 = 150_000
@@ -329,16 +330,18 @@ def test_search_large_skip_fractions(dt0):
     _check_search(w, res, ora, sde_kernel=5, label=f"dt0={dt0}")
 
 
-def test_fold_sort_very_long_curve_uses_lsd_path():
-    """n beyond 256 buckets x 1536 keys: every period overflows its buckets and goes through the LSD path."""
+def test_fold_sort_very_long_curves():
+    """420 000 points: 2048 buckets of ~205 keys, still the bucket fast path (103 count / scatter CTAs per period);
+    800 000 points: beyond 2048 buckets x 384 keys, every period overflows its buckets and goes through the
+    LSD path."""
     _cuda()
     rng = np.random.default_rng(21)
-    n = 420_000
-    t = np.sort(rng.uniform(0, 3000, n))
-    periods = np.array([1.2345, 77.7])
-    _, perm = g.gtls_fold_sort(t, periods, want_phase=False)
-    _, pm_o = oracle.fold_sort(t, periods, want_phase=False)
-    assert np.array_equal(perm, pm_o)
+    for n in (420_000, 800_000):
+        t = np.sort(rng.uniform(0, 3000, n))
+        periods = np.array([1.2345, 77.7])
+        _, perm = g.gtls_fold_sort(t, periods, want_phase=False)
+        _, pm_o = oracle.fold_sort(t, periods, want_phase=False)
+        assert np.array_equal(perm, pm_o), n
 
 
 def test_search_shared_duration_grid_and_small_tiles(tmpl512):
