@@ -4,21 +4,22 @@
 // scan.cu, kept as the fallback):
 //
 //   k_bucket_count    fold every point; one histogram of the top KBITS bits of floor(phase * 2^32) per CTA
-//                     (4096 points), written out as 16-bit counts -- no global atomics
+//                     (2048 points), written out as 16-bit counts -- no global atomics
 //   k_bucket_scan     per period: for every bucket the running sum of the CTAs' counts (where a CTA's keys
 //                     start inside the bucket) and the bucket starts; a bucket larger than kBucketCap
 //                     (clustered phases) puts the period on the tile's fallback list, which the LSD path
 //                     processes instead
 //   k_bucket_scatter  fold again (t is L2 resident, the division is cheaper than 16 B of HBM) and write
 //                     (key32 << 32 | index) to bucket start + CTA offset + rank inside the CTA's share
-//                     (shared-memory atomics only; any order inside the bucket)
-//   k_bucket_finish   one WARP per period walks through the period's buckets (~260 keys each) in order,
-//                     with warp-private shared memory and no CTA barrier: counting sort on the next 8 key
-//                     bits, an exact rank inside every run of equal 8-bit codes by (key32, fp64 phase,
-//                     index), then gather and scan with the running sums carried from bucket to bucket:
-//                     permutation, x1 = w r (x0 = w) and the final S1 (S0) in one pass, every global
-//                     access coalesced.
-//   k_pad_scan        wrap padding (Fig. 3): the first D_m sorted entries again, the sums run on.
+//                     (shared-memory atomics only; the CTA's keys are staged in bucket order in shared
+//                     memory and written by consecutive threads; any order inside the bucket)
+//   k_bucket_sort     one WARP per (period, 8 consecutive buckets of ~260 keys) with warp-private shared memory
+//                     and no CTA barrier: counting sort on the next 8 key bits, an exact rank inside every run
+//                     of equal 8-bit codes by (key32, fp64 phase, index), then the permutation and the gathered
+//                     x1 = w r (x0 = w, x2 = w r^2) go out coalesced.  Units are independent, so periods with
+//                     clustered phases (long runs) are balanced over the GPU by the CTA scheduler.
+//   k_bucket_prefix   one CTA per period: S1 (S0, S2) over the n sorted entries and on over the wrap padding
+//                     (Fig. 3: the first D_m sorted entries again), coalesced, fixed addition tree.
 //
 // The order inside a bucket before the local sort is irrelevant because the local sort orders by the
 // full (phase, index) key, so the permutation is identical to a stable sort by fp64 phase
@@ -29,22 +30,26 @@ namespace gtls {
 
 namespace {
 
-constexpr int kCountThreads = 512;
+constexpr int kCountThreads = 256;
 constexpr int kCountItems = 8;                       // points per thread in count / scatter
-constexpr int kCtaKeys = kCountThreads * kCountItems;   // 4096 points per CTA (a 16-bit count holds it)
+constexpr int kCtaKeys = kCountThreads * kCountItems;   // 2048 points per CTA (a 16-bit count holds it)
 constexpr int kFinWarps = 4;                         // periods per CTA of the finish kernel
 constexpr int kFinSlots = kBucketCap / 32;           // keys per lane and bucket (12)
 constexpr int kUnitsPerWarp = 8;                     // consecutive buckets of a period a warp sorts (<= 31)
-constexpr int kPrefThreads = 512, kPrefItems = 8;    // prefix-sum kernel: 4096 entries per chunk
-constexpr int kPadThreads = 512;
-constexpr int kSubBits = 8;
+constexpr int kPrefThreads = 256, kPrefItems = 8;    // prefix-sum kernel: 2048 entries per chunk
+#ifndef GTLS_SUB_BITS
+#define GTLS_SUB_BITS 8
+#endif
+constexpr int kSubBits = GTLS_SUB_BITS;
 constexpr int kSub = 1 << kSubBits;                  // sub-buckets of the warp's counting sort
-constexpr int kScanItems = 4;                        // pad scan: entries per thread and round
+static_assert(kSub % 128 == 0, "sort: whole uint4 groups of counts per lane");
 static_assert(kBucketCap % 32 == 0 && kCtaKeys < 65536, "bucket slots / 16-bit counts");
 static_assert(kMaxBuckets % kCountThreads == 0, "scatter: whole buckets per thread in the scan");
 
-__device__ __forceinline__ u32 key32_of(const double* __restrict__ t, int i, double period) {
-    return phase_key32(fold_phase(t[i], period));
+// (A reciprocal-multiply quotient with two residual corrections and an exact-residual check that proves it equal
+//  to the IEEE quotient was measured in place of the division: the folds got slower, DESIGN.md section 10 item 4.)
+__device__ __forceinline__ u32 key32_of(double t, double period) {
+    return phase_key32(fold_phase(t, period));
 }
 
 __global__ void __launch_bounds__(kCountThreads) k_bucket_count(BucketArgs b) {
@@ -53,11 +58,14 @@ __global__ void __launch_bounds__(kCountThreads) k_bucket_count(BucketArgs b) {
     for (int k = threadIdx.x; k < b.nbk; k += kCountThreads) h[k] = 0;
     __syncthreads();
     const double period = b.periods[b.p0 + pl];
-    const int base = blockIdx.x * kCtaKeys;
+    const int base = blockIdx.x * kCtaKeys + threadIdx.x;
+    double tv[kCountItems];
+#pragma unroll
+    for (int e = 0; e < kCountItems; ++e) tv[e] = base + e * kCountThreads < b.n ? b.t[base + e * kCountThreads] : 0.0;
 #pragma unroll
     for (int e = 0; e < kCountItems; ++e) {
-        const int i = base + e * kCountThreads + threadIdx.x;
-        if (i < b.n) atomicAdd(&h[(u32)((u64)key32_of(b.t, i, period) >> b.shift)], 1u);
+        const u32 key = key32_of(tv[e], period);
+        if (base + e * kCountThreads < b.n) atomicAdd(&h[(u32)((u64)key >> b.shift)], 1u);
     }
     __syncthreads();
     unsigned short* hist = b.hist + ((long long)pl * b.ncta + blockIdx.x) * b.nbk;
@@ -108,15 +116,15 @@ __global__ void __launch_bounds__(256) k_bucket_scan(BucketArgs b) {
     }
 }
 
-// The CTA's 4096 keys are put in bucket order in shared memory first (their rank inside the CTA's share of a
+// The CTA's 2048 keys are put in bucket order in shared memory first (their rank inside the CTA's share of a
 // bucket comes from the histogram atomics), then written out by consecutive threads: a warp's 32 stores fall
 // into four or five runs of consecutive addresses instead of 32 buckets (the kernel is bound by L2 write
 // transactions otherwise).
 __global__ void __launch_bounds__(kCountThreads) k_bucket_scatter(BucketArgs b) {
     extern __shared__ __align__(16) unsigned char scat_smem[];
     u64* const stage = reinterpret_cast<u64*>(scat_smem);                 // [kCtaKeys]
-    __shared__ u32 cnt[kMaxBuckets];           // keys of this CTA per bucket, then the bucket's first staged position
-    __shared__ u32 basepos[kMaxBuckets];       // bucket start + where this CTA's keys start inside the bucket
+    u32* const cnt = reinterpret_cast<u32*>(stage + kCtaKeys);            // [nbk] keys of this CTA per bucket, then the bucket's first staged position
+    u32* const basepos = cnt + b.nbk;                                     // [nbk] bucket start + where this CTA's keys start inside the bucket
     __shared__ u32 s_wsum[kCountThreads / 32];
     const int pl = blockIdx.y;
     if (b.fb_flag[pl]) return;
@@ -135,7 +143,7 @@ __global__ void __launch_bounds__(kCountThreads) k_bucket_scatter(BucketArgs b) 
     for (int e = 0; e < kCountItems; ++e) tv[e] = base + e * kCountThreads < b.n ? b.t[base + e * kCountThreads] : 0.0;
     u32 key[kCountItems], rank[kCountItems];
 #pragma unroll
-    for (int e = 0; e < kCountItems; ++e) key[e] = phase_key32(fold_phase(tv[e], period));
+    for (int e = 0; e < kCountItems; ++e) key[e] = key32_of(tv[e], period);
 #pragma unroll
     for (int e = 0; e < kCountItems; ++e)
         rank[e] = base + e * kCountThreads < b.n ? atomicAdd(&cnt[(u32)((u64)key[e] >> b.shift)], 1u) : 0u;
@@ -243,20 +251,27 @@ __global__ void __launch_bounds__(kFinWarps * 32, 7) k_bucket_sort(BucketArgs b)
                 if (j * 32 + lane < M) atomicAdd(&sm.H[((u32)(kc[j] >> 32) >> subshift) & (kSub - 1)], 1u);
         }
         __syncwarp();
-        // 3. exclusive scan of the kSub counts (8 per lane)
+        // 3. exclusive scan of the kSub counts (kSub / 32 consecutive counts per lane)
         {
-            uint4 c0 = *reinterpret_cast<const uint4*>(&sm.H[lane * 8]);
-            uint4 c1 = *reinterpret_cast<const uint4*>(&sm.H[lane * 8 + 4]);
-            const u32 sum = c0.x + c0.y + c0.z + c0.w + c1.x + c1.y + c1.z + c1.w;
+            constexpr int PB = kSub / 32;
+            u32 c[PB], sum = 0;
+#pragma unroll
+            for (int q = 0; q < PB / 4; ++q) {
+                const uint4 v = *reinterpret_cast<const uint4*>(&sm.H[lane * PB + 4 * q]);
+                c[4 * q] = v.x; c[4 * q + 1] = v.y; c[4 * q + 2] = v.z; c[4 * q + 3] = v.w;
+                sum += v.x + v.y + v.z + v.w;
+            }
             u32 x = sum;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) { const u32 y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
             u32 base = x - sum;
-            uint4 e0, e1;
-            e0.x = base; base += c0.x; e0.y = base; base += c0.y; e0.z = base; base += c0.z; e0.w = base; base += c0.w;
-            e1.x = base; base += c1.x; e1.y = base; base += c1.y; e1.z = base; base += c1.z; e1.w = base;
-            *reinterpret_cast<uint4*>(&sm.H[lane * 8]) = e0;
-            *reinterpret_cast<uint4*>(&sm.H[lane * 8 + 4]) = e1;
+#pragma unroll
+            for (int q = 0; q < PB / 4; ++q) {
+                uint4 v;
+                v.x = base; base += c[4 * q]; v.y = base; base += c[4 * q + 1];
+                v.z = base; base += c[4 * q + 2]; v.w = base; base += c[4 * q + 3];
+                *reinterpret_cast<uint4*>(&sm.H[lane * PB + 4 * q]) = v;
+            }
         }
         __syncwarp();
         // 4. counting-sort scatter (order inside a sub-bucket is arbitrary)
@@ -303,7 +318,7 @@ __global__ void __launch_bounds__(kFinWarps * 32, 7) k_bucket_sort(BucketArgs b)
 }
 
 // a4 (Eq. 14): S[i + 1] = x[0] + .. + x[i] for the n sorted entries of every period; one CTA per period walks
-// the period in chunks of 4096 entries.  A warp owns 256 consecutive entries of the chunk: it loads and stores
+// the period in chunks of 2048 entries.  A warp owns 256 consecutive entries of the chunk: it loads and stores
 // them lane-strided (coalesced; the next chunk's loads are issued before the current chunk is scanned) and
 // turns them through a padded warp-private tile of shared memory so that a lane scans 8 consecutive entries;
 // the warps' totals meet in shared memory, a running carry links the chunks.  Fixed addition tree.
@@ -314,8 +329,15 @@ __global__ void __launch_bounds__(kPrefThreads) k_bucket_prefix(BucketArgs b) {
     __shared__ double s_w[2][NARR][NW];
     const int pl = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (b.fb_flag[pl]) return;
-    const double* xs[3] = {b.x1 + (long long)pl * b.pitch, NARR > 1 ? b.x0 + (long long)pl * b.pitch : nullptr,
-                           NARR > 2 ? b.x2 + (long long)pl * b.pitch : nullptr};
+    double* xs[3] = {b.x1 + (long long)pl * b.pitch, NARR > 1 ? b.x0 + (long long)pl * b.pitch : nullptr,
+                     NARR > 2 ? b.x2 + (long long)pl * b.pitch : nullptr};
+    // wrap padding (Fig. 3): entries n .. n + pad - 1 repeat entries 0 .. pad - 1 and the sums run on
+    int pad = b.pad_override;
+    if (pad < 0) {
+        pad = 0;
+        for (int jd = 0; jd < b.n_dur; ++jd) pad = max(pad, b.durtab[(long long)pl * b.n_dur + jd].D);
+    }
+    const int nt = b.n + pad;
     double* ss[3] = {b.s1 + (long long)pl * b.spitch, NARR > 1 ? b.s0 + (long long)pl * b.spitch : nullptr,
                      NARR > 2 ? b.s2 + (long long)pl * b.spitch : nullptr};
     double carry[NARR];
@@ -328,11 +350,19 @@ __global__ void __launch_bounds__(kPrefThreads) k_bucket_prefix(BucketArgs b) {
 #pragma unroll
         for (int a = 0; a < NARR; ++a)
 #pragma unroll
-            for (int e = 0; e < kPrefItems; ++e) nx[a][e] = g + e * 32 < b.n ? xs[a][g + e * 32] : 0.0;
+            for (int e = 0; e < kPrefItems; ++e) {
+                const int i = g + e * 32;
+                if (c0 + CH <= b.n) {                                    // (CTA uniform) loads only: all in flight at once
+                    nx[a][e] = __ldg(xs[a] + i);
+                } else {
+                    nx[a][e] = i < nt ? xs[a][i < b.n ? i : i - b.n] : 0.0;
+                    if (i >= b.n && i < nt) xs[a][i] = nx[a][e];
+                }
+            }
     };
     load(0);
     int par = 0;
-    for (int c0 = 0; c0 < b.n; c0 += CH, par ^= 1) {
+    for (int c0 = 0; c0 < nt; c0 += CH, par ^= 1) {
         double v[NARR][kPrefItems], tot[NARR], incl[NARR];
 #pragma unroll
         for (int a = 0; a < NARR; ++a) {
@@ -344,7 +374,7 @@ __global__ void __launch_bounds__(kPrefThreads) k_bucket_prefix(BucketArgs b) {
             for (int e = 0; e < kPrefItems; ++e) v[a][e] = T[lane * (kPrefItems + 1) + e];
             __syncwarp();
         }
-        if (c0 + CH < b.n) load(c0 + CH);
+        if (c0 + CH < nt) load(c0 + CH);
 #pragma unroll
         for (int a = 0; a < NARR; ++a) {
 #pragma unroll
@@ -379,77 +409,11 @@ __global__ void __launch_bounds__(kPrefThreads) k_bucket_prefix(BucketArgs b) {
 #pragma unroll
             for (int e = 0; e < kPrefItems; ++e) {
                 const int j = e * 32 + lane;
-                if (g + e * 32 < b.n) dst[e * 32] = T[j + (j >> 3)];
+                if (g + e * 32 < nt) dst[e * 32] = T[j + (j >> 3)];
             }
             __syncwarp();
             carry[a] = all;
         }
-    }
-}
-
-// Wrap padding (Fig. 3): entries n .. n+pad-1 repeat entries 0 .. pad-1, the prefix sums run on.
-template <bool HAS0, bool HAS2>
-__global__ void __launch_bounds__(kPadThreads) k_pad_scan(BucketArgs b) {
-    __shared__ double s_w[3][32];
-    const int pl = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (b.fb_flag[pl]) return;
-    constexpr int NW = kPadThreads / 32;
-    int pad = b.pad_override;
-    if (pad < 0) {
-        pad = 0;
-        for (int jd = 0; jd < b.n_dur; ++jd) pad = max(pad, b.durtab[(long long)pl * b.n_dur + jd].D);
-    }
-    double* x1 = b.x1 + (long long)pl * b.pitch;
-    double* s1 = b.s1 + (long long)pl * b.spitch;
-    double* x0 = HAS0 ? b.x0 + (long long)pl * b.pitch : nullptr;
-    double* s0 = HAS0 ? b.s0 + (long long)pl * b.spitch : nullptr;
-    double* x2 = HAS2 ? b.x2 + (long long)pl * b.pitch : nullptr;
-    double* s2 = HAS2 ? b.s2 + (long long)pl * b.spitch : nullptr;
-    double c1 = s1[b.n], c0 = HAS0 ? s0[b.n] : 0.0, c2 = HAS2 ? s2[b.n] : 0.0;
-    for (int r0 = 0; r0 < pad; r0 += kPadThreads * kScanItems) {
-        const int cnt = min(kPadThreads * kScanItems, pad - r0);
-        double v1[kScanItems], v0[kScanItems], v2[kScanItems];
-        const int first = threadIdx.x * kScanItems;
-#pragma unroll
-        for (int e = 0; e < kScanItems; ++e) {
-            v1[e] = 0.0; v0[e] = 0.0; v2[e] = 0.0;
-            if (first + e < cnt) {
-                v1[e] = x1[r0 + first + e];
-                x1[b.n + r0 + first + e] = v1[e];
-                if (HAS0) { v0[e] = x0[r0 + first + e]; x0[b.n + r0 + first + e] = v0[e]; }
-                if (HAS2) { v2[e] = x2[r0 + first + e]; x2[b.n + r0 + first + e] = v2[e]; }
-            }
-        }
-#pragma unroll
-        for (int e = 1; e < kScanItems; ++e) { v1[e] += v1[e - 1]; v0[e] += v0[e - 1]; v2[e] += v2[e - 1]; }
-        double t1 = v1[kScanItems - 1], t0 = v0[kScanItems - 1], t2 = v2[kScanItems - 1];
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const double u1 = __shfl_up_sync(0xffffffffu, t1, o);
-            const double u0 = __shfl_up_sync(0xffffffffu, t0, o);
-            const double u2 = __shfl_up_sync(0xffffffffu, t2, o);
-            if (lane >= o) { t1 += u1; t0 += u0; t2 += u2; }
-        }
-        if (lane == 31) { s_w[0][warp] = t1; s_w[1][warp] = t0; s_w[2][warp] = t2; }
-        __syncthreads();
-        double w1 = c1, w0 = c0, w2 = c2, a1 = c1, a0 = c0, a2 = c2;
-#pragma unroll
-        for (int k = 0; k < NW; ++k) {
-            if (k < warp) { w1 += s_w[0][k]; w0 += s_w[1][k]; w2 += s_w[2][k]; }
-            a1 += s_w[0][k]; a0 += s_w[1][k]; a2 += s_w[2][k];
-        }
-        const double o1 = w1 + (t1 - v1[kScanItems - 1]), o0 = w0 + (t0 - v0[kScanItems - 1]),
-                     o2 = w2 + (t2 - v2[kScanItems - 1]);
-#pragma unroll
-        for (int e = 0; e < kScanItems; ++e) {
-            if (first + e < cnt) {
-                s1[b.n + r0 + first + e + 1] = o1 + v1[e];
-                if (HAS0) s0[b.n + r0 + first + e + 1] = o0 + v0[e];
-                if (HAS2) s2[b.n + r0 + first + e + 1] = o2 + v2[e];
-            }
-        }
-        c1 = a1; c0 = a0; c2 = a2;
-        __syncthreads();
     }
 }
 
@@ -462,6 +426,7 @@ int bucket_count_for(int n) {
 }
 
 static dim3 count_grid(const BucketArgs& b) { return dim3(b.ncta, b.tile); }
+static size_t scatter_smem(const BucketArgs& b) { return kCtaKeys * sizeof(u64) + 2 * (size_t)b.nbk * sizeof(u32); }
 
 int bucket_cta_count(int n) { return (n + kCtaKeys - 1) / kCtaKeys; }
 
@@ -473,8 +438,8 @@ void launch_bucket_sort_head(const BucketArgs& b, cudaStream_t st) {
 
 void launch_bucket_sort_tail(const BucketArgs& b, bool has0, bool has2, bool sort_only, cudaStream_t st) {
     // (per device and cheap: set on every call)
-    cudaFuncSetAttribute(k_bucket_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kCtaKeys * sizeof(u64)));
-    k_bucket_scatter<<<count_grid(b), kCountThreads, kCtaKeys * sizeof(u64), st>>>(b);
+    cudaFuncSetAttribute(k_bucket_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)scatter_smem(b));
+    k_bucket_scatter<<<count_grid(b), kCountThreads, scatter_smem(b), st>>>(b);
     const long long groups = (long long)b.tile * ((b.nbk + kUnitsPerWarp - 1) / kUnitsPerWarp);
     const dim3 fgrid((unsigned)((groups + kFinWarps - 1) / kFinWarps));
     constexpr int kFinThreads = kFinWarps * 32;
@@ -482,15 +447,12 @@ void launch_bucket_sort_tail(const BucketArgs& b, bool has0, bool has2, bool sor
     if (has2) {
         k_bucket_sort<true, true, false><<<fgrid, kFinThreads, 0, st>>>(b);
         k_bucket_prefix<3><<<b.tile, kPrefThreads, 0, st>>>(b);
-        k_pad_scan<true, true><<<b.tile, kPadThreads, 0, st>>>(b);
     } else if (has0) {
         k_bucket_sort<true, false, false><<<fgrid, kFinThreads, 0, st>>>(b);
         k_bucket_prefix<2><<<b.tile, kPrefThreads, 0, st>>>(b);
-        k_pad_scan<true, false><<<b.tile, kPadThreads, 0, st>>>(b);
     } else {
         k_bucket_sort<false, false, false><<<fgrid, kFinThreads, 0, st>>>(b);
         k_bucket_prefix<1><<<b.tile, kPrefThreads, 0, st>>>(b);
-        k_pad_scan<false, false><<<b.tile, kPadThreads, 0, st>>>(b);
     }
 }
 
