@@ -275,8 +275,10 @@ size_t gtls_batch_workspace_bytes(int32_t n_curves, const int64_t* curve_offset,
                                   const int64_t* period_offset, int32_t n_dur, const gtls_opts* opts);
 
 /* Device scratch needed by gtls_search for these sizes and options (tile = opts->period_tile
- * or the automatic choice).  Pass a buffer of at least this size in opts->workspace to avoid
- * allocation inside the call. */
+ * or the automatic choice: enough for the worst case -- per-point errors, durations up to half a
+ * period -- at its automatic tile, and for the common case -- one common error bar, durations up
+ * to a fifth of a period -- at ITS larger automatic tile).  Pass a buffer of at least this size
+ * in opts->workspace to avoid allocation inside the call. */
 size_t gtls_workspace_bytes(int64_t n, int64_t n_per, int32_t n_dur, const gtls_opts* opts);
 
 /* Device blocks the library allocates itself (the staged copies of host arrays, the scratch when

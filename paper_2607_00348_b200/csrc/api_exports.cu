@@ -20,7 +20,8 @@ int gtls_fold_sort(const double* t, int64_t n, const double* periods, int64_t n_
                               sort_scratch_bytes(n) + 1024 +
                               (dev ? 0 : n * (sizeof(double) + sizeof(int32_t))) + 1024;
     long long tile = (long long)((1ull << 30) / per_period);
-    if (o.period_tile > 0) tile = o.period_tile;
+    if (tile > 8192) tile = 8192;                               // (a tile is gridDim.y of the sort kernels: <= 65535)
+    if (o.period_tile > 0) tile = o.period_tile < 65535 ? o.period_tile : 65535;
     if (tile > n_per) tile = n_per;
     if (tile < 1) tile = 1;
     Arena ar;

@@ -330,6 +330,18 @@ def test_search_large_skip_fractions(dt0):
     _check_search(w, res, ora, sde_kernel=5, label=f"dt0={dt0}")
 
 
+def test_fold_sort_many_periods_of_a_tiny_curve():
+    """70 000 periods of a 50-point curve: the export's automatic period tile is capped (a tile is gridDim.y of
+    the sort kernels), so the call runs nine tiles; every permutation against the oracle."""
+    _cuda()
+    rng = np.random.default_rng(5)
+    t = np.sort(rng.uniform(0, 30, 50))
+    periods = np.linspace(0.3, 12.0, 70_000)
+    _, perm = g.gtls_fold_sort(t, periods, want_phase=False)
+    _, pm_o = oracle.fold_sort(t, periods, want_phase=False)
+    assert np.array_equal(perm, pm_o)
+
+
 def test_fold_sort_very_long_curves():
     """420 000 points: 2048 buckets of ~205 keys, still the bucket fast path (103 count / scatter CTAs per period);
     800 000 points: beyond 2048 buckets x 384 keys, every period overflows its buckets and goes through the
