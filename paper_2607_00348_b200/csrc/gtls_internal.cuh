@@ -190,7 +190,7 @@ struct BucketArgs {
 };
 int bucket_count_for(int n);
 int bucket_cta_count(int n);
-// count + bucket starts + fallback list; then (after the caller forked the fallback path) scatter + finish + pad
+// count + bucket starts + fallback list; then (after the caller forked the fallback path) scatter + sort + prefix / pad
 void launch_bucket_sort_head(const BucketArgs& b, cudaStream_t st);
 void launch_bucket_sort_tail(const BucketArgs& b, bool has0, bool has2, bool sort_only, cudaStream_t st);
 
